@@ -1,0 +1,164 @@
+"""ctypes wrapper around oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  It builds oracle/liboracle.so with gcc on first use (plain C, -O2,
+OpenMP over directions) and exposes the oracle's entry points with numpy host arrays.
+Nothing here touches CUDA or the paper_1410_0763_b200 package.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lock = threading.Lock()
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile oracle.c -> liboracle.so (idempotent)."""
+    with _lock:
+        if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+            tmp = _LIB + ".tmp%d" % os.getpid()
+            cmd = ["gcc", "-O2", "-fPIC", "-shared", "-fopenmp", "-std=c11", "-Wall", "-o", tmp, _SRC, "-lm"]
+            subprocess.run(cmd, check=True)
+            os.replace(tmp, _LIB)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(_LIB)
+        dp, fp, ip = C.POINTER(C.c_double), C.POINTER(C.c_float), C.POINTER(C.c_int)
+        up, i64p = C.POINTER(C.c_uint32), C.POINTER(C.c_int64)
+        L.orc_healpix_dirs.argtypes = [C.c_int, dp]
+        L.orc_healpix_dirs.restype = C.c_int
+        L.orc_dir_record.argtypes = [dp, ip, ip, i64p, i64p, dp]
+        L.orc_dir_record.restype = C.c_int
+        L.orc_sweep.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, fp, fp, dp, C.c_int, dp, C.c_double,
+                                dp, dp, dp, C.POINTER(C.c_ulonglong), up, ip, C.c_int, up, dp, dp, C.c_int]
+        L.orc_sweep.restype = C.c_int
+        L.orc_trace_direction.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, fp, fp, dp, dp, C.c_double,
+                                          ip, dp, dp, C.POINTER(C.c_long)]
+        L.orc_trace_direction.restype = C.c_int
+        L.orc_sweep_cells.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, fp, fp, dp, C.c_int, dp, C.c_double,
+                                      ip, C.c_int, dp, dp, up, C.c_int]
+        L.orc_sweep_cells.restype = C.c_int
+        L.orc_num_threads.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _p(a, ct):
+    return None if a is None else a.ctypes.data_as(C.POINTER(ct))
+
+
+def _fields(kappa, S):
+    kappa = np.ascontiguousarray(kappa, dtype=np.float32)
+    S = np.ascontiguousarray(S, dtype=np.float32)
+    if kappa.ndim == 3:
+        kappa, S = kappa[None], S[None]
+    assert kappa.ndim == 4 and kappa.shape == S.shape, "fields must be [nbins][nz][ny][nx]"
+    return kappa, S
+
+
+def healpix_dirs(nside: int) -> np.ndarray:
+    """HEALPix RING-order pixel centres, [12 nside^2][3] fp64 (oracle.c orc_healpix_dirs)."""
+    out = np.empty((12 * nside * nside, 3), dtype=np.float64)
+    n = lib().orc_healpix_dirs(nside, _p(out, C.c_double))
+    assert n == out.shape[0]
+    return out
+
+
+def dir_record(n) -> dict:
+    """Dominant axis, reflections, quantised slopes and slab length of one direction (O2)."""
+    n = np.ascontiguousarray(n, dtype=np.float64)
+    a = C.c_int()
+    refl = (C.c_int * 3)()
+    Mb, Mc, L = C.c_int64(), C.c_int64(), C.c_double()
+    rc = lib().orc_dir_record(_p(n, C.c_double), C.byref(a), refl, C.byref(Mb), C.byref(Mc), C.byref(L))
+    if rc != 0:
+        raise ValueError("zero direction vector")
+    return {"a": a.value, "refl": tuple(refl), "Mb": Mb.value, "Mc": Mc.value, "L": L.value}
+
+
+def sweep(kappa, S, dirs, Ibc=None, cell_width: float = 1.0, count_dirs=(), nthreads: int = 0,
+          want_counts: bool = True) -> dict:
+    """Full sweep.  Returns dict(Jin, J, sum_ds, seg_total, cnt_sum, cnt_dirs, min_den, max_den)."""
+    kappa, S = _fields(kappa, S)
+    nb, nz, ny, nx = kappa.shape
+    dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
+    nd = dirs.shape[0]
+    Jin = np.empty(kappa.shape, dtype=np.float64)
+    J = np.empty(kappa.shape, dtype=np.float64)
+    sum_ds = np.empty(nd, dtype=np.float64)
+    min_den = np.empty(nd, dtype=np.float64)
+    max_den = np.empty(nd, dtype=np.float64)
+    seg = C.c_ulonglong(0)
+    cnt_sum = np.empty((nz, ny, nx), dtype=np.uint32) if want_counts else None
+    cd = np.ascontiguousarray(list(count_dirs), dtype=np.int32)
+    cnt_out = np.zeros((len(cd), nz, ny, nx), dtype=np.uint32) if len(cd) else None
+    ibc = None if Ibc is None else np.ascontiguousarray(Ibc, dtype=np.float64)
+    rc = lib().orc_sweep(nx, ny, nz, nb, _p(kappa, C.c_float), _p(S, C.c_float), _p(dirs, C.c_double), nd,
+                         _p(ibc, C.c_double), float(cell_width), _p(Jin, C.c_double), _p(J, C.c_double),
+                         _p(sum_ds, C.c_double), C.byref(seg), _p(cnt_sum, C.c_uint32),
+                         _p(cd, C.c_int) if len(cd) else None, len(cd), _p(cnt_out, C.c_uint32),
+                         _p(min_den, C.c_double), _p(max_den, C.c_double), int(nthreads))
+    if rc != 0:
+        raise RuntimeError("orc_sweep failed: %d" % rc)
+    return {"Jin": Jin, "J": J, "sum_ds": sum_ds, "seg_total": int(seg.value), "cnt_sum": cnt_sum,
+            "cnt_dirs": cnt_out, "min_den": min_den, "max_den": max_den}
+
+
+def trace_direction(kappa, S, n, Ibc=None, cell_width: float = 1.0, check_groups: bool = False) -> dict:
+    """One direction: per-ray exit intensity and in-box chord over the whole launch lattice (+ P9 check)."""
+    kappa, S = _fields(kappa, S)
+    nb, nz, ny, nx = kappa.shape
+    n = np.ascontiguousarray(n, dtype=np.float64)
+    lat = (C.c_int * 4)()
+    ibc = None if Ibc is None else np.ascontiguousarray(Ibc, dtype=np.float64)
+    L = lib()
+    args = [nx, ny, nz, nb, _p(kappa, C.c_float), _p(S, C.c_float), _p(n, C.c_double), _p(ibc, C.c_double),
+            float(cell_width), lat]
+    rc = L.orc_trace_direction(*args, None, None, None)
+    assert rc == 0
+    pmin, qmin, np_, nq = lat
+    exitI = np.zeros((nq, np_, nb), dtype=np.float64)
+    chord = np.zeros((nq, np_), dtype=np.float64)
+    conf = C.c_long(0)
+    rc = L.orc_trace_direction(*args, _p(exitI, C.c_double), _p(chord, C.c_double),
+                               C.byref(conf) if check_groups else None)
+    if rc != 0:
+        raise RuntimeError("orc_trace_direction failed: %d" % rc)
+    return {"pmin": pmin, "qmin": qmin, "exitI": exitI, "chord": chord, "conflicts": int(conf.value)}
+
+
+def sweep_cells(kappa, S, dirs, cells, Ibc=None, cell_width: float = 1.0, nthreads: int = 0) -> dict:
+    """J_in / J at sampled cells (x,y,z), tracing only the rays that touch them."""
+    kappa, S = _fields(kappa, S)
+    nb, nz, ny, nx = kappa.shape
+    dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
+    cells = np.ascontiguousarray(cells, dtype=np.int32).reshape(-1, 3)
+    nc = cells.shape[0]
+    Jin = np.empty((nb, nc), dtype=np.float64)
+    J = np.empty((nb, nc), dtype=np.float64)
+    cnt = np.empty(nc, dtype=np.uint32)
+    ibc = None if Ibc is None else np.ascontiguousarray(Ibc, dtype=np.float64)
+    rc = lib().orc_sweep_cells(nx, ny, nz, nb, _p(kappa, C.c_float), _p(S, C.c_float), _p(dirs, C.c_double),
+                               dirs.shape[0], _p(ibc, C.c_double), float(cell_width), _p(cells, C.c_int), nc,
+                               _p(Jin, C.c_double), _p(J, C.c_double), _p(cnt, C.c_uint32), int(nthreads))
+    if rc != 0:
+        raise RuntimeError("orc_sweep_cells failed: %d" % rc)
+    return {"Jin": Jin, "J": J, "cnt": cnt}
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())

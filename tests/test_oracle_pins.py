@@ -1,0 +1,363 @@
+"""Pins of the CPU oracle (oracle/oracle.c) against things other than itself.
+
+Each test names the pin (P1..P11) and what mistake it would catch.
+No GPU, no CUDA library: these run in the `-m "not gpu"` suite.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from tests import bruteforce as bf
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "worked_example.txt")
+
+
+def rand_fields(dims, seed, kmin=0.05, kmax=2.0):
+    nx, ny, nz = dims
+    rng = np.random.default_rng(seed)
+    kap = rng.uniform(kmin, kmax, size=(1, nz, ny, nx)).astype(np.float32)
+    S = rng.uniform(0.0, 1.0, size=(1, nz, ny, nx)).astype(np.float32)
+    return kap, S
+
+
+# ---------------------------------------------------------------- P1: direction generator
+@pytest.mark.parametrize("nside", [1, 2, 4, 8, 16])
+def test_p1_healpix_count_norm_symmetry(orc, nside):
+    d = orc.healpix_dirs(nside)
+    assert d.shape == (12 * nside * nside, 3)                       # N_d = 12 Nside^2
+    assert np.abs(np.linalg.norm(d, axis=1) - 1.0).max() < 1e-15
+    assert np.abs(d.sum(axis=0)).max() < 1e-11                      # isotropic set: sum n = 0
+    key = lambda a: sorted(map(tuple, np.round(a, 12) + 0.0))
+    base = key(d)
+    for ax in range(3):                                             # invariant under mirror of each axis
+        m = d.copy()
+        m[:, ax] *= -1
+        assert key(m) == base
+    assert key(d[:, [1, 0, 2]]) == base                             # and under x <-> y
+    # RING order: z non-increasing
+    assert np.all(np.diff(d[:, 2]) <= 1e-15)
+
+
+def test_p1_healpix_nside1_base_pixels(orc):
+    """Nside = 1: the 12 base-pixel centres: z = +-2/3 at phi = pi/4 + k pi/2, z = 0 at phi = k pi/2."""
+    d = orc.healpix_dirs(1)
+    z = d[:, 2]
+    assert np.allclose(z[:4], 2.0 / 3.0, atol=1e-15) and np.allclose(z[8:], -2.0 / 3.0, atol=1e-15)
+    assert np.allclose(z[4:8], 0.0, atol=1e-15)
+    phi = np.mod(np.arctan2(d[:, 1], d[:, 0]), 2 * np.pi)
+    assert np.allclose(np.sort(phi[:4]), np.pi / 4 + np.arange(4) * np.pi / 2, atol=1e-14)
+    eq = {tuple(np.round(v, 12) + 0.0) for v in d[4:8]}
+    assert eq == {(1.0, 0.0, 0.0), (-1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (0.0, -1.0, 0.0)}
+
+
+@pytest.mark.parametrize("nside", [2, 4, 16])
+def test_p1_healpix_equal_area_rings(orc, nside):
+    """Equal-area pixels on iso-latitude rings: the pixels north of the boundary between ring i and
+    ring i+1 tile a cap of area 2 pi (1 - z_edge); with equal areas their count fixes z_edge, and
+    every ring centre must lie strictly between consecutive edges.  Also ring z from the closed form."""
+    d = orc.healpix_dirs(nside)
+    npix = d.shape[0]
+    zs, counts = np.unique(np.round(d[:, 2], 13), return_counts=True)
+    zs, counts = zs[::-1], counts[::-1]
+    assert len(zs) == 4 * nside - 1
+    assert abs(zs[0] - (1 - 1 / (3 * nside ** 2))) < 1e-12          # ring 1
+    assert abs(zs[2 * nside - 1]) < 1e-12                           # ring 2 Nside is the equator
+    cum = np.cumsum(counts)
+    z_edge = 1.0 - 2.0 * cum / npix                                 # cap area fraction = (1 - z)/2
+    upper = np.concatenate([[1.0], z_edge[:-1]])
+    assert np.all(zs < upper + 1e-12) and np.all(zs > z_edge - 1e-12)
+
+
+def test_p1_direction_record(orc):
+    r = orc.dir_record([0.3, -0.9, 0.2])
+    assert r["a"] == 1 and r["refl"] == (0, 1, 0)
+    assert r["Mb"] == round(0.3 / 0.9 * 2 ** 20) and r["Mc"] == round(0.2 / 0.9 * 2 ** 20)
+    assert abs(r["L"] - math.sqrt(1 + (r["Mb"] / 2 ** 20) ** 2 + (r["Mc"] / 2 ** 20) ** 2)) < 1e-15
+    assert orc.dir_record([1.0, 1.0, 1.0])["a"] == 0                # ties -> lowest axis (A5)
+    assert orc.dir_record([0.0, 1.0, 1.0])["a"] == 1
+    assert orc.dir_record([6e-17, 1.0, 0.0])["Mb"] == 0             # cos(pi/2) noise quantises to 0 (A6)
+    with pytest.raises(ValueError):
+        orc.dir_record([0.0, 0.0, 0.0])
+    # agreement with the brute-force module's separately written record
+    rng = np.random.default_rng(5)
+    for n in rng.normal(size=(50, 3)):
+        a, b, c, refl, Mb, Mc, L = bf.dir_record(n)
+        r = orc.dir_record(n)
+        assert (r["a"], r["Mb"], r["Mc"]) == (a, Mb, Mc) and r["refl"] == tuple(int(x) for x in refl)
+
+
+# ---------------------------------------------------------------- P2: axis-aligned hand enumeration
+def test_p2_axis_aligned_4cubed(orc):
+    """6 axis directions on a 4^3 mesh: every cell has one segment of length 1 per direction;
+    along each row I follows the textbook recurrence; J_in = (1/6) sum_dir I_in f(kappa) (eqs. 7, 8, 13)."""
+    dims = (4, 4, 4)
+    kap, S = rand_fields(dims, 11)
+    dirs = np.array([[1, 0, 0], [-1, 0, 0], [0, 1, 0], [0, -1, 0], [0, 0, 1], [0, 0, -1]], dtype=np.float64)
+    r = orc.sweep(kap, S, dirs, count_dirs=range(6))
+    assert r["seg_total"] == 6 * 64
+    assert np.all(r["cnt_dirs"] == 1)
+    assert np.allclose(r["sum_ds"], 64.0, rtol=0, atol=1e-12)
+    k3, s3 = kap[0].astype(np.float64), S[0].astype(np.float64)
+    expect = np.zeros((4, 4, 4))
+    for axis in range(3):                      # numpy axis of [z][y][x]: 0=z,1=y,2=x
+        for sign in (+1, -1):
+            kk = np.moveaxis(k3, axis, 0)
+            ss = np.moveaxis(s3, axis, 0)
+            out = np.zeros_like(kk)
+            order = range(4) if sign > 0 else range(3, -1, -1)
+            I = np.zeros(kk.shape[1:])
+            for i in order:
+                tau = kk[i]
+                out[i] = I * (1 - np.exp(-tau)) / tau
+                I = I * np.exp(-tau) + ss[i] * (1 - np.exp(-tau))
+            expect += np.moveaxis(out, 0, axis) / 6.0
+    assert np.allclose(r["Jin"][0], expect, rtol=1e-13, atol=0)
+    assert np.allclose(r["J"][0], expect + s3, rtol=1e-13, atol=0)          # eq. 12
+
+
+# ---------------------------------------------------------------- P3 / P4: lattice invariants
+@pytest.mark.parametrize("dims", [(8, 8, 8), (16, 8, 4), (4, 8, 16), (6, 5, 4)])
+def test_p3_per_cell_sum_ds_equals_L(orc, dims):
+    """Equally spaced rays: per cell and direction sum_j ds_j = L exactly, hence
+    sum ds = N_m L = mesh volume / per-ray cross-section (north_star invariant)."""
+    kap, S = rand_fields(dims, 3)
+    dirs = np.array([[1, 0.4, 0], [1, 0.5, 0], [0.37, 1, 0.81], [1, 1, 1], [0.5, 0.25, 1], [0, 0, -1],
+                     [0.3333, -1, 0.9], [-0.77, 0.12, -1], [1, 1, 0], [-1, -0.999999, 0.5]], dtype=np.float64)
+    r = orc.sweep(kap, S, dirs)
+    ncell = dims[0] * dims[1] * dims[2]
+    for i, n in enumerate(dirs):
+        L = orc.dir_record(n)["L"]
+        assert abs(r["min_den"][i] - L) < 1e-12 * L and abs(r["max_den"][i] - L) < 1e-12 * L
+        assert abs(r["sum_ds"][i] - ncell * L) < 1e-11 * ncell * L
+
+
+def test_p3_healpix_set_sum_ds(orc):
+    dims = (12, 10, 14)
+    kap, S = rand_fields(dims, 4)
+    dirs = orc.healpix_dirs(4)
+    r = orc.sweep(kap, S, dirs)
+    L = np.array([orc.dir_record(n)["L"] for n in dirs])
+    assert np.allclose(r["min_den"], L, rtol=1e-12) and np.allclose(r["max_den"], L, rtol=1e-12)
+
+
+def test_p4_segment_count_band(orc):
+    """Segments per direction = N_m (1 + m_b + m_c) for generic slopes (cost model PAPER.md:177)."""
+    dims = (32, 32, 32)
+    kap, S = rand_fields(dims, 6)
+    dirs = np.array([[1, 0.37, 0.81], [0.123, -1, 0.456]], dtype=np.float64)
+    for n in dirs:
+        r = orc.sweep(kap, S, n[None], want_counts=False)
+        rec = orc.dir_record(n)
+        pred = 32 ** 3 * (1 + rec["Mb"] / 2 ** 20 + rec["Mc"] / 2 ** 20)
+        assert abs(r["seg_total"] - pred) < 0.02 * pred
+    # rational-degenerate slopes from half-integer origins: every crossing lies on a slab plane
+    r = orc.sweep(kap, S, np.array([[1, 0.5, 0.25]]), want_counts=False)
+    assert r["seg_total"] == 32 ** 3
+
+
+# ---------------------------------------------------------------- P5: uniform medium closed form
+def test_p5_uniform_slab_closed_form(orc):
+    """Uniform kappa, S, zero inflow: exit intensity = S (1 - exp(-kappa * chord)) for every ray (eq. 7
+    is exact for piecewise-constant media), independent of the segmentation."""
+    dims = (10, 12, 8)
+    kap = np.full((1, 8, 12, 10), 0.3, dtype=np.float32)
+    S = np.full_like(kap, 1.7)
+    k64, s64 = float(kap.flat[0]), float(S.flat[0])
+    for n in ([1, 0.37, 0.81], [-0.2, 0.5, -1], [0, 1, 0], [1, 1, 1]):
+        t = orc.trace_direction(kap, S, n)
+        expect = s64 * (1 - np.exp(-k64 * t["chord"]))
+        assert np.allclose(t["exitI"][..., 0], expect, rtol=1e-13, atol=1e-15)
+        assert t["chord"].max() > 5.0
+    # with inflow I_bc: I = I_bc e^-tau + S (1 - e^-tau)
+    t = orc.trace_direction(kap, S, [1, 0.37, 0.81], Ibc=[0.9])
+    tau = k64 * t["chord"]
+    assert np.allclose(t["exitI"][..., 0], 0.9 * np.exp(-tau) + s64 * (1 - np.exp(-tau)), rtol=1e-13)
+
+
+def test_p5_chord_total_is_volume_over_cross_section(orc):
+    dims = (10, 12, 8)
+    kap, S = rand_fields(dims, 9)
+    n = [0.3, -0.8, 0.5]
+    t = orc.trace_direction(kap, S, n)
+    assert abs(t["chord"].sum() - 10 * 12 * 8 * orc.dir_record(n)["L"]) < 1e-9
+
+
+# ---------------------------------------------------------------- P8 / P6 / P11: rational brute force
+BF_DIMS = (6, 5, 4)
+BF_DIRS = [[0.37, 1, 0.81], [1, 0.5, 0.25], [-1, 1, 1], [0.2, -0.3, -1], [1, 0, 0.999999], [0, -1, 0]]
+
+
+def test_p8_bruteforce_geometry_and_J(orc):
+    """Independent algorithm (global event sort + midpoint classification, exact rationals): per-cell
+    counts bit-exact, per-cell sum ds, per-ray chord and exit intensity, and J_in to 1e-12."""
+    kap, S = rand_fields(BF_DIMS, 21)
+    dirs = np.array(BF_DIRS, dtype=np.float64)
+    ref = bf.sweep(kap[0], S[0], dirs, Ibc=0.25)
+    r = orc.sweep(kap, S, dirs, Ibc=[0.25], count_dirs=range(len(dirs)))
+    nx, ny, nz = BF_DIMS
+    for i, n in enumerate(dirs):
+        cnt = np.zeros((nz, ny, nx), dtype=np.uint32)
+        for (x, y, z), c in ref["per_dir"][i]["cnt"].items():
+            cnt[z, y, x] = c
+        assert np.array_equal(cnt, r["cnt_dirs"][i])
+        assert abs(sum(ref["per_dir"][i]["den"].values()) - r["sum_ds"][i]) < 1e-10
+        t = orc.trace_direction(kap, S, n, Ibc=[0.25])
+        for (p, q), (I, chord) in ref["per_dir"][i]["exits"].items():
+            assert abs(t["chord"][q - t["qmin"], p - t["pmin"]] - chord) < 1e-12
+            assert abs(t["exitI"][q - t["qmin"], p - t["pmin"], 0] - I) < 1e-12
+    Jin = np.zeros((nz, ny, nx))
+    for (x, y, z), v in ref["Jin"].items():
+        Jin[z, y, x] = v
+    assert np.allclose(r["Jin"][0], Jin, rtol=1e-12, atol=1e-15)
+    assert r["seg_total"] == sum(ref["cnt"].values())
+
+
+def test_p6_optically_thin_limit(orc):
+    """kappa -> 0 at fixed emissivity eps = kappa S: J_in -> path-length-weighted mean of the linear
+    emission integral (no exponentials), computed by the brute-force module with linear=True."""
+    kap, S = rand_fields(BF_DIMS, 22)
+    kap_thin = (kap.astype(np.float64) * 1e-8).astype(np.float32)
+    S_big = (S.astype(np.float64) * 1e8).astype(np.float32)
+    dirs = np.array(BF_DIRS[:4], dtype=np.float64)
+    ref = bf.sweep(kap_thin[0], S_big[0], dirs, linear=True)
+    r = orc.sweep(kap_thin, S_big, dirs)
+    nx, ny, nz = BF_DIMS
+    Jin = np.zeros((nz, ny, nx))
+    for (x, y, z), v in ref["Jin"].items():
+        Jin[z, y, x] = v
+    assert Jin.max() > 0.1
+    assert np.allclose(r["Jin"][0], Jin, rtol=1e-6, atol=1e-12)
+
+
+def test_p11_optically_thick_limit(orc):
+    """Uniform box with kappa dH = 60: every ray reaching an interior cell carries I_in = S, so
+    J_in = S (1/N_d) sum_i sum_j (ds_j / L_i) f(kappa ds_j) from the segment lengths alone
+    (checks the 1/N_d factor and the ds weighting of eqs. 10-13 together)."""
+    dims = (7, 7, 7)
+    kap = np.full((1, 7, 7, 7), 60.0, dtype=np.float32)
+    S = np.full_like(kap, 0.8)
+    dirs = np.array([[0.37, 1, 0.81], [1, 0.5, 0.25], [-1, 0.9, 0.3], [0.2, -0.3, -1]], dtype=np.float64)
+    r = orc.sweep(kap, S, dirs)
+    centre = (3, 3, 3)
+    expect = 0.0
+    for n in dirs:
+        for (p, q) in bf.lattice(dims, n):
+            iv, L = bf.ray_intervals(dims, n, p, q)
+            for cell, frac in iv:
+                if cell == centre:
+                    expect += float(frac) * bf.f_of(60.0 * float(frac) * L)
+    expect *= float(S.flat[0]) / len(dirs)
+    assert abs(r["Jin"][0, 3, 3, 3] - expect) < 1e-12 * expect
+
+
+# ---------------------------------------------------------------- P7: mirror / permutation symmetry
+def test_p7_mirror_and_permutation(orc):
+    dims = (6, 8, 10)
+    kap, S = rand_fields(dims, 31)
+    dirs = orc.healpix_dirs(2)[::3].copy()
+    base = orc.sweep(kap, S, dirs, count_dirs=range(len(dirs)))
+    for ax in range(3):                                   # numpy axis of [bin][z][y][x] for coordinate ax
+        npax = 3 - ax
+        d2 = dirs.copy()
+        d2[:, ax] *= -1
+        r2 = orc.sweep(np.flip(kap, npax), np.flip(S, npax), d2, count_dirs=range(len(dirs)))
+        assert np.array_equal(np.flip(r2["cnt_dirs"], npax), base["cnt_dirs"])
+        assert np.allclose(np.flip(r2["Jin"], npax), base["Jin"], rtol=1e-13, atol=1e-16)
+    # cyclic permutation x->y->z->x of fields and directions together
+    kp = np.ascontiguousarray(np.transpose(kap, (0, 2, 1, 3)))      # new [z'][y'][x'] = old [y][z][x]: swaps y,z
+    sp = np.ascontiguousarray(np.transpose(S, (0, 2, 1, 3)))
+    r3 = orc.sweep(kp, sp, dirs[:, [0, 2, 1]], count_dirs=range(len(dirs)))
+    assert np.array_equal(np.transpose(r3["cnt_sum"], (1, 0, 2)), base["cnt_sum"])
+    assert np.allclose(np.transpose(r3["Jin"], (0, 2, 1, 3)), base["Jin"], rtol=1e-12, atol=1e-16)
+
+
+# ---------------------------------------------------------------- P9: ray groups
+def test_p9_four_groups_never_share_a_cell(orc):
+    """rays of one of the 4 interleaved groups never traverse the same mesh grid."""
+    dims = (8, 6, 10)
+    kap, S = rand_fields(dims, 41)
+    for n in list(orc.healpix_dirs(2)) + [[1, 1, 1], [1, 0.5, 0.25], [0.999999, 1, 0.000001]]:
+        assert orc.trace_direction(kap, S, n, check_groups=True)["conflicts"] == 0
+
+
+# ---------------------------------------------------------------- P10: worked example
+def test_p10_worked_example_golden(orc):
+    gold = {}
+    for line in open(GOLD):
+        if line.strip() and not line.startswith("#"):
+            k, v = line.split()
+            gold[k] = float(v)
+    kap = np.zeros((1, 1, 2, 2), np.float32)
+    S = np.zeros_like(kap)
+    K = [[1.0, 0.5], [2.0, 0.25]]
+    Sv = [[1.0, 0.25], [0.5, 2.0]]
+    for k in range(2):
+        for j in range(2):
+            kap[0, 0, j, k] = K[k][j]
+            S[0, 0, j, k] = Sv[k][j]
+    n = np.array([[1.0, 0.375, 0.0]])
+    r = orc.sweep(kap, S, n, count_dirs=[0])
+    assert abs(orc.dir_record(n[0])["L"] - gold["L"]) < 1e-15
+    assert r["seg_total"] == gold["total_segments"]
+    assert abs(r["sum_ds"][0] - gold["sum_ds"]) < 1e-12
+    for k in range(2):
+        for j in range(2):
+            assert r["cnt_dirs"][0, 0, j, k] == gold["count_%d%d" % (k, j)]
+            assert abs(r["Jin"][0, 0, j, k] - gold["Jin_%d%d" % (k, j)]) < 1e-12
+            assert abs(r["J"][0, 0, j, k] - (gold["Jin_%d%d" % (k, j)] + float(np.float32(Sv[k][j])))) < 1e-12
+    t = orc.trace_direction(kap, S, n[0])
+    ex = t["exitI"][0 - t["qmin"], :, 0]
+    for name, p in (("pm1", -1), ("p0", 0), ("p1", 1)):
+        assert abs(ex[p - t["pmin"]] - gold["exit_" + name]) < 1e-12
+
+
+# ---------------------------------------------------------------- special cases and consistency
+def test_kappa_zero_is_well_defined(orc):
+    """A7: kappa = 0 cells: f(0) = 1, I unchanged; J_in stays finite."""
+    dims = (6, 6, 6)
+    kap, S = rand_fields(dims, 51)
+    kap[0, 2:4] = 0.0
+    r = orc.sweep(kap, S, orc.healpix_dirs(1))
+    assert np.all(np.isfinite(r["Jin"])) and r["Jin"].min() >= 0.0
+
+
+def test_multibin_bins_are_independent(orc):
+    """A15 / eq. 22: bins share geometry and do not couple."""
+    dims = (6, 5, 7)
+    k1, s1 = rand_fields(dims, 61)
+    k2, s2 = rand_fields(dims, 62)
+    dirs = orc.healpix_dirs(1)
+    both = orc.sweep(np.concatenate([k1, k2]), np.concatenate([s1, s2]), dirs, Ibc=[0.1, 0.7])
+    a = orc.sweep(k1, s1, dirs, Ibc=[0.1])
+    b = orc.sweep(k2, s2, dirs, Ibc=[0.7])
+    assert np.allclose(both["Jin"][0], a["Jin"][0], rtol=1e-13) and np.allclose(both["Jin"][1], b["Jin"][0], rtol=1e-13)
+    assert not np.allclose(both["Jin"][0], both["Jin"][1], rtol=1e-3)
+
+
+def test_sampled_cells_match_full_sweep(orc):
+    """orc_sweep_cells (used for parity at full benchmark sizes) traces only the rays through the
+    sampled cells with the same trace_ray: must reproduce the full sweep there."""
+    dims = (12, 10, 9)
+    kap, S = rand_fields(dims, 71)
+    dirs = orc.healpix_dirs(2)
+    full = orc.sweep(kap, S, dirs)
+    rng = np.random.default_rng(0)
+    cells = np.stack([rng.integers(0, dims[0], 20), rng.integers(0, dims[1], 20), rng.integers(0, dims[2], 20)], 1)
+    cells = np.unique(cells, axis=0)
+    cells = np.concatenate([cells, [[0, 0, 0], [11, 9, 8], [0, 9, 0]]])
+    part = orc.sweep_cells(kap, S, dirs, cells)
+    for s, (x, y, z) in enumerate(cells):
+        assert abs(part["Jin"][0, s] - full["Jin"][0, z, y, x]) <= 1e-13 * full["Jin"][0, z, y, x]
+        assert part["cnt"][s] == full["cnt_sum"][z, y, x]
+
+
+def test_cell_width_scales_optical_depth(orc):
+    """kappa is per unit length: (kappa, dH) and (kappa*dH, 1) give the same J_in."""
+    dims = (5, 6, 4)
+    kap, S = rand_fields(dims, 81)
+    dirs = orc.healpix_dirs(1)
+    a = orc.sweep(kap, S, dirs, cell_width=2.0)
+    b = orc.sweep((kap * np.float32(2.0)), S, dirs, cell_width=1.0)
+    assert np.allclose(a["Jin"], b["Jin"], rtol=1e-12)
