@@ -1,0 +1,153 @@
+/*
+ * rt.h -- C ABI of the B200-native diffuse-radiation ray sweep (arXiv:1410.0763, Tanaka et al.).
+ *
+ * The library computes, for a uniform 3-D mesh with absorption coefficient kappa and source
+ * function S per cell and a set of N_d directions, the mean intensity
+ *
+ *     J_in = (1/N_d) sum_i  Ibar^{ave,in}(n_i)        (eq. 13)
+ *     J    = J_in + S                                 (eq. 12)
+ *
+ * where, per direction, equally spaced parallel rays (one per cell cross-section on the
+ * plane normal to the dominant axis) are marched cell by cell with
+ *
+ *     I_out = I_in exp(-dtau) + S (1 - exp(-dtau)),  dtau = kappa * ds      (eq. 7)
+ *     Ibar_in = I_in (1 - exp(-dtau)) / dtau                                (eq. 8)
+ *     Ibar^{ave,in} = sum_j dtau_j Ibar_in,j / sum_j dtau_j                 (eqs. 10-11)
+ *
+ * and concurrently marching rays never write the same cell (section 3.1); here
+ * that is achieved by cell ownership instead of the paper's four sequential ray groups.
+ *
+ * Conventions
+ *  - Every call returns RT_OK (0) or a negative RT_E* code; nothing throws, aborts or prints.
+ *  - "host" / "device" is stated for every pointer.  Device pointers must belong to the CUDA
+ *    device that was current when rt_create was called.
+ *  - Field arrays are fp32, C-contiguous [nbins][nz][ny][nx] (x fastest).
+ *  - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All device
+ *    work is enqueued on it; calls are asynchronous unless stated otherwise.
+ *  - The context owns all internal device memory; the caller owns kappa, S, J and count buffers.
+ *  - One context must not be used from two host threads at once; different contexts are independent.
+ *  - The library has no CPU fallback: without a usable CUDA device rt_create fails with RT_ECUDA.
+ */
+#ifndef RT_H_
+#define RT_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rt_ctx rt_ctx;
+
+/* error codes */
+#define RT_OK        0
+#define RT_EINVAL   -1   /* bad argument: null pointer, non-positive dims, zero direction vector, unsupported option */
+#define RT_ENOMEM   -2   /* host or device allocation failed */
+#define RT_ECUDA    -3   /* CUDA runtime error; text via rt_last_cuda_error() */
+#define RT_ESTATE   -4   /* call order: e.g. rt_sweep before rt_set_fields */
+
+/* rt_create flags */
+#define RT_OWNED            0u   /* default: atomic-free, one writer per cell (ownership + seam accumulators) */
+#define RT_ATOMIC_ABLATION  1u   /* ablation: every ray segment does atomicAdd into the accumulator */
+#define RT_PAPER_GROUPS     2u   /* ablation: the paper's four sequential ray groups with plain stores */
+
+/* rt_sweep `what` */
+#define RT_J_IN     0u           /* eq. 13 */
+#define RT_J_TOTAL  1u           /* eq. 12: J_in + S */
+
+/*
+ * HEALPix ring-scheme pixel centres (Gorski et al. 2005, cited at PAPER.md:183, 463).
+ *   nside     : resolution parameter >= 1
+ *   dirs_out  : HOST, fp64 [12*nside*nside][3], unit vectors, RING order (north to south)
+ * Returns the number of directions written, or RT_EINVAL.
+ */
+int rt_healpix_dirs(int nside, double *dirs_out);
+
+/*
+ * Create a sweep context: quantise the directions (dominant axis, reflections, slopes in units of
+ * 2^-20, slab length), build the per-direction slab programs on the device (the integer traversal
+ * of PAPER.md:86 / Fig. 2, identical for every ray of a direction), choose layouts, allocate.
+ *   out           : HOST, receives the context
+ *   nx, ny, nz    : mesh dimensions (x fastest)
+ *   nbins         : frequency bins sharing one geometry (eq. 22), 1..16
+ *   dirs, ndirs   : HOST, fp64 [ndirs][3], need not be normalised, none may be zero; copied
+ *   rays_per_cell : rays per cell width in each transverse axis; only 1 is supported (RT_EINVAL otherwise)
+ *   cell_width    : mesh spacing dH (> 0); kappa is per unit length, so dtau = kappa * ds * dH
+ *   flags         : RT_OWNED | RT_ATOMIC_ABLATION | RT_PAPER_GROUPS
+ * Synchronises the device once (table build).  Returns RT_OK / RT_EINVAL / RT_ENOMEM / RT_ECUDA.
+ */
+int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins,
+              const double *dirs, int ndirs, int rays_per_cell, double cell_width, unsigned flags);
+
+/*
+ * Set the medium.  Enqueues a repack of (kappa, S) into the packed sweep layouts on `cuda_stream`.
+ *   kappa_dev, S_dev : DEVICE, fp32 [nbins][nz][ny][nx]; borrowed only until the enqueued repack
+ *                      has completed on the stream; the library keeps its own packed copies.
+ * kappa must be >= 0 and finite; kappa = 0 is allowed (f(0) = 1, reading A7).
+ */
+int rt_set_fields(rt_ctx *ctx, const float *kappa_dev, const float *S_dev, void *cuda_stream);
+
+/*
+ * Boundary inflow intensity per bin (default 0; the diffuse field has no external source in the
+ * paper's tests).   I_bc_host : HOST, fp32 [nbins].
+ */
+int rt_set_inflow(rt_ctx *ctx, const float *I_bc_host);
+
+/*
+ * One full sweep over all directions ("one iteration" of PAPER.md:322).
+ *   J_dev : DEVICE, fp32 [nbins][nz][ny][nx], caller-owned, fully overwritten
+ *   what  : RT_J_IN or RT_J_TOTAL
+ * Asynchronous on `cuda_stream`.  RT_ESTATE if rt_set_fields has not been called.
+ */
+int rt_sweep(rt_ctx *ctx, float *J_dev, unsigned what, void *cuda_stream);
+
+/*
+ * Diagnostics required by the parity gates (integer traversal data, summed ds).  They run the same
+ * traversal kernel as rt_sweep with the transfer arithmetic replaced by counting.
+ *
+ * rt_segment_counts: per-cell number of positive-length ray segments.
+ *   dir_index  : 0..ndirs-1 for one direction, -1 for the sum over all directions
+ *   counts_dev : DEVICE, uint32 [nz][ny][nx], fully overwritten.  Asynchronous.
+ * rt_sum_ds: fp32-path sum of segment lengths per direction, widened to fp64.
+ *   sum_ds_host : HOST, fp64 [ndirs].  Synchronises the stream.
+ *   min_ds_host, max_ds_host : HOST, fp64 [ndirs] or NULL: min / max over cells of the per-cell sum of ds.
+ * rt_total_segments: exact total over directions and cells (numerator of the throughput metric,
+ *   per bin).  n_host : HOST.  Synchronises the stream.
+ */
+int rt_segment_counts(rt_ctx *ctx, int dir_index, unsigned int *counts_dev, void *cuda_stream);
+int rt_sum_ds(rt_ctx *ctx, double *sum_ds_host, double *min_ds_host, double *max_ds_host, void *cuda_stream);
+int rt_total_segments(rt_ctx *ctx, unsigned long long *n_host, void *cuda_stream);
+
+/*
+ * Per-direction record as quantised by the library (for cross-checks against the oracle).
+ *   rec_host : HOST, long long [ndirs][6] = {dominant axis, reflect_x | reflect_y<<1 | reflect_z<<2,
+ *              M_b, M_c, kernel path (0 = owned fast path, 1 = generic), 0}
+ *   L_host   : HOST, fp64 [ndirs] slab length in cell widths, or NULL
+ */
+int rt_direction_records(rt_ctx *ctx, long long *rec_host, double *L_host);
+
+/*
+ * Tuning knobs (experiments and ablations; defaults are chosen by rt_create).
+ *   "slots" : concurrent direction slots per launch (each has private accumulators)
+ *   "rows"  : rays rows per warp in the owned kernel (1, 2, 4 or 8)
+ * Returns RT_EINVAL for unknown keys or unsupported values.  Must be called before rt_set_fields.
+ */
+int rt_tune(rt_ctx *ctx, const char *key, int value);
+
+/* Number of kernel launches issued by the last rt_sweep of this context. */
+int rt_last_launch_count(rt_ctx *ctx);
+
+/* Time of the last rt_sweep's traversal kernels only, in ms (cudaEvents on the sweep's stream);
+   synchronises on those events.  Negative if unavailable. */
+float rt_last_sweep_kernel_ms(rt_ctx *ctx);
+
+/* Free everything the context owns.  Synchronises the device.  NULL is allowed. */
+int rt_destroy(rt_ctx *ctx);
+
+/* Static text for an RT_* code. */
+const char *rt_strerror(int code);
+/* Text of the last CUDA error seen by this thread in the library ("" if none). */
+const char *rt_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RT_H_ */

@@ -1,0 +1,230 @@
+"""ctypes binding of include/rt.h.  Same names as the C ABI; argument marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+RT_OWNED, RT_ATOMIC_ABLATION, RT_PAPER_GROUPS = 0, 1, 2
+RT_J_IN, RT_J_TOTAL = 0, 1
+
+EXPORTED_SYMBOLS = [
+    "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_sweep", "rt_segment_counts",
+    "rt_sum_ds", "rt_total_segments", "rt_direction_records", "rt_tune", "rt_last_launch_count",
+    "rt_last_sweep_kernel_ms", "rt_destroy", "rt_strerror", "rt_last_cuda_error",
+]
+
+_lib = None
+
+
+class RtError(RuntimeError):
+    def __init__(self, code, where):
+        L = load_library()
+        msg = L.rt_strerror(code).decode()
+        cuda = L.rt_last_cuda_error().decode()
+        super().__init__("%s failed: %s (%d)%s" % (where, msg, code, (" [" + cuda + "]") if cuda and code == -3 else ""))
+        self.code = code
+
+
+def load_library():
+    """Load (building if necessary) librt.so.  Raises if it cannot be built: there is no fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if _build.needs_build():
+        path = _build.build()
+    L = C.CDLL(path)
+    vp, dp, fp = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_float)
+    L.rt_healpix_dirs.argtypes = [C.c_int, dp]
+    L.rt_healpix_dirs.restype = C.c_int
+    L.rt_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, C.c_int, dp, C.c_int, C.c_int, C.c_double, C.c_uint]
+    L.rt_create.restype = C.c_int
+    L.rt_set_fields.argtypes = [vp, vp, vp, vp]
+    L.rt_set_fields.restype = C.c_int
+    L.rt_set_inflow.argtypes = [vp, fp]
+    L.rt_set_inflow.restype = C.c_int
+    L.rt_sweep.argtypes = [vp, vp, C.c_uint, vp]
+    L.rt_sweep.restype = C.c_int
+    L.rt_segment_counts.argtypes = [vp, C.c_int, vp, vp]
+    L.rt_segment_counts.restype = C.c_int
+    L.rt_sum_ds.argtypes = [vp, dp, dp, dp, vp]
+    L.rt_sum_ds.restype = C.c_int
+    L.rt_total_segments.argtypes = [vp, C.POINTER(C.c_ulonglong), vp]
+    L.rt_total_segments.restype = C.c_int
+    L.rt_direction_records.argtypes = [vp, C.POINTER(C.c_longlong), dp]
+    L.rt_direction_records.restype = C.c_int
+    L.rt_tune.argtypes = [vp, C.c_char_p, C.c_int]
+    L.rt_tune.restype = C.c_int
+    L.rt_last_launch_count.argtypes = [vp]
+    L.rt_last_launch_count.restype = C.c_int
+    L.rt_last_sweep_kernel_ms.argtypes = [vp]
+    L.rt_last_sweep_kernel_ms.restype = C.c_float
+    L.rt_destroy.argtypes = [vp]
+    L.rt_destroy.restype = C.c_int
+    L.rt_strerror.argtypes = [C.c_int]
+    L.rt_strerror.restype = C.c_char_p
+    L.rt_last_cuda_error.argtypes = []
+    L.rt_last_cuda_error.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc, where):
+    if rc != 0:
+        raise RtError(rc, where)
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, int):
+        return C.c_void_p(stream)
+    return C.c_void_p(stream.cuda_stream)
+
+
+def _dev_ptr(t, dtype, numel, name):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == dtype and t.numel() == numel):
+        raise ValueError("%s must be a contiguous CUDA tensor of dtype %s with %d elements" % (name, dtype, numel))
+    return C.c_void_p(t.data_ptr())
+
+
+# ---- the C ABI, one function per entry point ------------------------------------------------------
+def healpix_dirs(nside: int) -> np.ndarray:
+    """rt_healpix_dirs: HEALPix RING pixel centres [12 nside^2][3] fp64 (host)."""
+    out = np.empty((12 * nside * nside, 3), dtype=np.float64)
+    n = load_library().rt_healpix_dirs(int(nside), out.ctypes.data_as(C.POINTER(C.c_double)))
+    if n != out.shape[0]:
+        raise RtError(n if n < 0 else -1, "rt_healpix_dirs")
+    return out
+
+
+def rt_create(nx, ny, nz, nbins, dirs, rays_per_cell=1, cell_width=1.0, flags=RT_OWNED):
+    dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
+    h = C.c_void_p()
+    rc = load_library().rt_create(C.byref(h), int(nx), int(ny), int(nz), int(nbins),
+                                  dirs.ctypes.data_as(C.POINTER(C.c_double)), dirs.shape[0], int(rays_per_cell),
+                                  float(cell_width), int(flags))
+    _check(rc, "rt_create")
+    return h
+
+
+def rt_tune(h, key: str, value: int):
+    _check(load_library().rt_tune(h, key.encode(), int(value)), "rt_tune(%s)" % key)
+
+
+def rt_set_fields(h, kappa, S, numel, stream=None):
+    import torch
+    _check(load_library().rt_set_fields(h, _dev_ptr(kappa, torch.float32, numel, "kappa"),
+                                        _dev_ptr(S, torch.float32, numel, "S"), _stream(stream)), "rt_set_fields")
+
+
+def rt_set_inflow(h, Ibc):
+    a = np.ascontiguousarray(Ibc, dtype=np.float32)
+    _check(load_library().rt_set_inflow(h, a.ctypes.data_as(C.POINTER(C.c_float))), "rt_set_inflow")
+
+
+def rt_sweep(h, J, numel, what=RT_J_IN, stream=None):
+    import torch
+    _check(load_library().rt_sweep(h, _dev_ptr(J, torch.float32, numel, "J"), int(what), _stream(stream)), "rt_sweep")
+
+
+def rt_segment_counts(h, dir_index, counts, numel, stream=None):
+    import torch
+    _check(load_library().rt_segment_counts(h, int(dir_index), _dev_ptr(counts, torch.int32, numel, "counts"),
+                                            _stream(stream)), "rt_segment_counts")
+
+
+def rt_sum_ds(h, ndirs, stream=None):
+    s, mn, mx = (np.empty(ndirs, dtype=np.float64) for _ in range(3))
+    p = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+    _check(load_library().rt_sum_ds(h, p(s), p(mn), p(mx), _stream(stream)), "rt_sum_ds")
+    return s, mn, mx
+
+
+def rt_total_segments(h, stream=None) -> int:
+    n = C.c_ulonglong(0)
+    _check(load_library().rt_total_segments(h, C.byref(n), _stream(stream)), "rt_total_segments")
+    return int(n.value)
+
+
+def rt_direction_records(h, ndirs):
+    rec = np.empty((ndirs, 6), dtype=np.int64)
+    L = np.empty(ndirs, dtype=np.float64)
+    _check(load_library().rt_direction_records(h, rec.ctypes.data_as(C.POINTER(C.c_longlong)),
+                                               L.ctypes.data_as(C.POINTER(C.c_double))), "rt_direction_records")
+    return rec, L
+
+
+def rt_destroy(h):
+    _check(load_library().rt_destroy(h), "rt_destroy")
+
+
+# ---- convenience wrapper (still argument marshalling only) -----------------------------------------
+class RayTracer:
+    """Owns one rt_ctx.  Fields and outputs are torch CUDA tensors [nbins][nz][ny][nx] fp32."""
+
+    def __init__(self, dims, nbins, dirs, cell_width=1.0, flags=RT_OWNED, slots=None, rows=None):
+        self.nx, self.ny, self.nz = (int(v) for v in dims)
+        self.nbins = int(nbins)
+        self.dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
+        self.ndirs = self.dirs.shape[0]
+        self.numel = self.nx * self.ny * self.nz * self.nbins
+        self.h = rt_create(self.nx, self.ny, self.nz, self.nbins, self.dirs, 1, cell_width, flags)
+        if slots is not None:
+            rt_tune(self.h, "slots", slots)
+        if rows is not None:
+            rt_tune(self.h, "rows", rows)
+
+    def shape(self):
+        return (self.nbins, self.nz, self.ny, self.nx)
+
+    def set_fields(self, kappa, S, stream=None):
+        rt_set_fields(self.h, kappa, S, self.numel, stream)
+
+    def set_inflow(self, Ibc):
+        rt_set_inflow(self.h, Ibc)
+
+    def sweep(self, out=None, what=RT_J_IN, stream=None):
+        import torch
+        if out is None:
+            out = torch.empty(self.shape(), dtype=torch.float32, device="cuda")
+        rt_sweep(self.h, out, self.numel, what, stream)
+        return out
+
+    def segment_counts(self, dir_index=-1, stream=None):
+        import torch
+        out = torch.empty((self.nz, self.ny, self.nx), dtype=torch.int32, device="cuda")
+        rt_segment_counts(self.h, dir_index, out, self.nx * self.ny * self.nz, stream)
+        return out
+
+    def sum_ds(self, stream=None):
+        return rt_sum_ds(self.h, self.ndirs, stream)
+
+    def total_segments(self, stream=None) -> int:
+        return rt_total_segments(self.h, stream)
+
+    def direction_records(self):
+        return rt_direction_records(self.h, self.ndirs)
+
+    def last_launch_count(self) -> int:
+        return int(load_library().rt_last_launch_count(self.h))
+
+    def last_sweep_kernel_ms(self) -> float:
+        return float(load_library().rt_last_sweep_kernel_ms(self.h))
+
+    def close(self):
+        if self.h is not None:
+            rt_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,490 @@
+// C ABI (include/rt.h) and host-side planner of the diffuse-radiation ray sweep.
+// Host work here is O(N_d): direction records (PAPER.md:183 directions -> dominant axis, reflections,
+// quantised slopes), batching of directions into launches, buffer management.  Everything that is
+// O(N_m) or O(N_m N_d) runs in the kernels of rt_kernels.cu.
+#include "../../include/rt.h"
+#include "rt_internal.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace rt;
+
+static thread_local char g_cuda_err[256] = "";
+
+static int cuda_fail(cudaError_t e)
+{
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+    return RT_ECUDA;
+}
+#define CK(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(e__); } while (0)
+
+struct HostDir {
+    int a, b, c;          // axes
+    int refl[3];
+    long long Mb, Mc;
+    double L;
+    int layout;           // 0 native, 1 transposed
+    int Na, Nb, Nc;
+    double work;          // 1 + mb + mc
+};
+
+struct rt_ctx {
+    int nx = 0, ny = 0, nz = 0, nbins = 1, ndirs = 0;
+    long long ncell = 0;
+    double cell_width = 1.0;
+    unsigned flags = 0;
+    int device = 0;
+    std::vector<HostDir> hd;
+    std::vector<int> order[2];       // direction indices per layout, sorted by work (descending)
+    bool fast[2] = {false, false};   // owned kernel usable for the layout
+    int rows = 4;
+    int slots_req = 0;               // user override
+    int slots[2] = {0, 0};           // allocated slots per layout
+    bool fields_set = false;
+    bool buffers_ready = false;
+    // device
+    DirDev *d_dirs = nullptr;
+    double *d_L = nullptr;
+    SlabProg *d_prog = nullptr;
+    float2 *d_P[2] = {nullptr, nullptr};
+    float *d_acc[2] = {nullptr, nullptr};
+    float *d_accC[2] = {nullptr, nullptr};
+    int *d_batch = nullptr;          // [ndirs] direction index per (launch, slot), launch-major
+    float *d_Ibc = nullptr;
+    double *d_red = nullptr;         // [3] reduction scratch
+    unsigned long long *d_u64 = nullptr;
+    unsigned *d_cnt = nullptr;       // [ncell] scratch for rt_total_segments
+    int np_max[2] = {0, 0}, nq_max[2] = {0, 0};
+    int last_launches = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    bool ev_valid = false;
+};
+
+extern "C" const char *rt_strerror(int code)
+{
+    switch (code) {
+    case RT_OK: return "ok";
+    case RT_EINVAL: return "invalid argument";
+    case RT_ENOMEM: return "out of memory";
+    case RT_ECUDA: return "CUDA error";
+    case RT_ESTATE: return "call order error";
+    }
+    return "unknown error";
+}
+extern "C" const char *rt_last_cuda_error(void) { return g_cuda_err; }
+
+// HEALPix ring-scheme pixel centres; closed form of Gorski et al. (2005) as cited by PAPER.md:183.
+extern "C" int rt_healpix_dirs(int nside, double *out)
+{
+    if (nside < 1 || nside > 8192 || !out) return RT_EINVAL;
+    const double PI = 3.14159265358979323846;
+    const double ns = (double)nside;
+    int n = 0;
+    for (int ring = 1; ring < 4 * nside; ++ring) {
+        const bool north = ring < nside, south = ring > 3 * nside;
+        const int ic = south ? 4 * nside - ring : ring;         // cap ring index counted from its pole
+        const int count = (north || south) ? 4 * ic : 4 * nside;
+        double z;
+        if (north || south) z = 1.0 - (double)ic * ic / (3.0 * ns * ns);
+        else z = 4.0 / 3.0 - 2.0 * ring / (3.0 * ns);
+        const double rxy = std::sqrt((1.0 - z) * (1.0 + z));
+        const double zz = south ? -z : z;
+        for (int j = 1; j <= count; ++j) {
+            double phi;
+            if (north || south) phi = (j - 0.5) * PI / (2.0 * ic);
+            else phi = (j - 0.5 * ((ring - nside + 1) % 2)) * PI / (2.0 * ns);
+            out[3 * n + 0] = rxy * std::cos(phi);
+            out[3 * n + 1] = rxy * std::sin(phi);
+            out[3 * n + 2] = zz;
+            ++n;
+        }
+    }
+    return n;
+}
+
+static void free_device(rt_ctx *c)
+{
+    cudaFree(c->d_dirs); cudaFree(c->d_L); cudaFree(c->d_prog);
+    for (int l = 0; l < 2; ++l) { cudaFree(c->d_P[l]); cudaFree(c->d_acc[l]); cudaFree(c->d_accC[l]); }
+    cudaFree(c->d_batch); cudaFree(c->d_Ibc); cudaFree(c->d_red); cudaFree(c->d_u64); cudaFree(c->d_cnt);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+}
+
+extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const double *dirs, int ndirs,
+                         int rays_per_cell, double cell_width, unsigned flags)
+{
+    if (!out) return RT_EINVAL;
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1 || nbins < 1 || nbins > 16 || !dirs || ndirs < 1) return RT_EINVAL;
+    if (rays_per_cell != 1) return RT_EINVAL;
+    if (!(cell_width > 0.0) || !std::isfinite(cell_width)) return RT_EINVAL;
+    if (flags > 2u) return RT_EINVAL;
+    if ((long long)nx * ny * nz * nbins >= (1ll << 40)) return RT_EINVAL;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    if (ndev < 1) return cuda_fail(cudaErrorNoDevice);
+
+    rt_ctx *c = new (std::nothrow) rt_ctx;
+    if (!c) return RT_ENOMEM;
+    c->nx = nx; c->ny = ny; c->nz = nz; c->nbins = nbins; c->ndirs = ndirs;
+    c->ncell = (long long)nx * ny * nz; c->cell_width = cell_width; c->flags = flags;
+    cudaGetDevice(&c->device);
+    const int dims[3] = {nx, ny, nz};
+
+    // ---- direction records (reading O2): plain IEEE fp64 operations in a fixed order
+    std::vector<DirDev> dd(ndirs);
+    std::vector<double> Lv(ndirs);
+    c->hd.resize(ndirs);
+    long long prog_total = 0;
+    for (int i = 0; i < ndirs; ++i) {
+        const double *n = dirs + 3 * i;
+        const double ab[3] = {std::fabs(n[0]), std::fabs(n[1]), std::fabs(n[2])};
+        if (!(ab[0] > 0.0 || ab[1] > 0.0 || ab[2] > 0.0) || !std::isfinite(ab[0] + ab[1] + ab[2])) { delete c; return RT_EINVAL; }
+        HostDir h;
+        h.a = 0;
+        if (ab[1] > ab[h.a]) h.a = 1;
+        if (ab[2] > ab[h.a]) h.a = 2;
+        h.b = (h.a == 0) ? 1 : 0;
+        h.c = (h.a == 2) ? 1 : 2;
+        for (int ax = 0; ax < 3; ++ax) h.refl[ax] = n[ax] < 0.0 ? 1 : 0;
+        const double mb = ab[h.b] / ab[h.a], mc = ab[h.c] / ab[h.a];
+        h.Mb = std::min<long long>(kOne, (long long)std::nearbyint(mb * (double)kOne));
+        h.Mc = std::min<long long>(kOne, (long long)std::nearbyint(mc * (double)kOne));
+        const double fb = (double)h.Mb / (double)kOne, fc = (double)h.Mc / (double)kOne;
+        h.L = std::sqrt(1.0 + fb * fb + fc * fc);
+        h.layout = (h.a == 0) ? 1 : 0;
+        h.Na = dims[h.a]; h.Nb = dims[h.b]; h.Nc = dims[h.c];
+        h.work = 1.0 + fb + fc;
+        c->hd[i] = h;
+        Lv[i] = h.L;
+
+        // strides of the canonical axes in the layout this direction sweeps
+        long long st[3];                       // element stride of x, y, z
+        if (h.layout == 0) { st[0] = 1; st[1] = nx; st[2] = (long long)nx * ny; }          // [z][y][x]
+        else               { st[1] = 1; st[2] = ny; st[0] = (long long)ny * nz; }          // [x][z][y]
+        DirDev d;
+        d.sk = st[h.a]; d.sl = st[h.c];
+        d.base = 0;
+        if (h.refl[h.a]) { d.base += (long long)(h.Na - 1) * d.sk; d.sk = -d.sk; }
+        if (h.refl[h.c]) { d.base += (long long)(h.Nc - 1) * d.sl; d.sl = -d.sl; }
+        d.sj = h.refl[h.b] ? -1 : 1;           // st[h.b] == 1 by construction of the layouts
+        d.Na = h.Na; d.Nb = h.Nb; d.Nc = h.Nc; d.layout = h.layout;
+        d.prog_off = (int)prog_total;
+        d.invL = (float)(1.0 / (h.L * cell_width));
+        d.Mb = (int)h.Mb; d.Mc = (int)h.Mc; d.pad = 0;
+        prog_total += h.Na;
+        if (prog_total > 0x7fffffffll) { delete c; return RT_EINVAL; }
+        dd[i] = d;
+        c->order[h.layout].push_back(i);
+        const int np = h.Nb + (int)((h.Na * h.Mb + kOne - 1) / kOne) + 1;
+        const int nq = h.Nc + (int)((h.Na * h.Mc + kOne - 1) / kOne) + 1;
+        c->np_max[h.layout] = std::max(c->np_max[h.layout], np);
+        c->nq_max[h.layout] = std::max(c->nq_max[h.layout], nq);
+    }
+    // homogeneous batches: similar work per direction in one launch; same dominant axis adjacent
+    for (int l = 0; l < 2; ++l)
+        std::stable_sort(c->order[l].begin(), c->order[l].end(), [&](int x, int y) {
+            if (c->hd[x].a != c->hd[y].a) return c->hd[x].a < c->hd[y].a;
+            return c->hd[x].work > c->hd[y].work;
+        });
+    // owned kernel: the memory-contiguous transverse extent must be 32/64/128/256 (one warp owns full rows)
+    const int NbL[2] = {nx, ny};
+    for (int l = 0; l < 2; ++l) c->fast[l] = (flags == RT_OWNED) && (NbL[l] == 32 || NbL[l] == 64 || NbL[l] == 128 || NbL[l] == 256);
+
+#define CKC(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { int rc__ = (e__ == cudaErrorMemoryAllocation) ? RT_ENOMEM : cuda_fail(e__); free_device(c); delete c; return rc__; } } while (0)
+    CKC(cudaMalloc(&c->d_dirs, sizeof(DirDev) * ndirs));
+    CKC(cudaMalloc(&c->d_L, sizeof(double) * ndirs));
+    CKC(cudaMalloc(&c->d_prog, sizeof(SlabProg) * prog_total));
+    CKC(cudaMalloc(&c->d_batch, sizeof(int) * ndirs));
+    CKC(cudaMalloc(&c->d_Ibc, sizeof(float) * nbins));
+    CKC(cudaMalloc(&c->d_red, sizeof(double) * 3));
+    CKC(cudaMalloc(&c->d_u64, sizeof(unsigned long long)));
+    CKC(cudaMemset(c->d_Ibc, 0, sizeof(float) * nbins));
+    CKC(cudaMemcpy(c->d_dirs, dd.data(), sizeof(DirDev) * ndirs, cudaMemcpyHostToDevice));
+    CKC(cudaMemcpy(c->d_L, Lv.data(), sizeof(double) * ndirs, cudaMemcpyHostToDevice));
+    {
+        std::vector<int> batch;
+        for (int l = 0; l < 2; ++l) batch.insert(batch.end(), c->order[l].begin(), c->order[l].end());
+        CKC(cudaMemcpy(c->d_batch, batch.data(), sizeof(int) * ndirs, cudaMemcpyHostToDevice));
+    }
+    CKC(launch_build_programs(c->d_dirs, ndirs, c->d_prog, cell_width, c->d_L, 0));
+    CKC(cudaEventCreate(&c->ev0));
+    CKC(cudaEventCreate(&c->ev1));
+    CKC(cudaDeviceSynchronize());
+#undef CKC
+    *out = c;
+    return RT_OK;
+}
+
+extern "C" int rt_tune(rt_ctx *c, const char *key, int value)
+{
+    if (!c || !key) return RT_EINVAL;
+    if (c->buffers_ready) return RT_ESTATE;
+    if (!strcmp(key, "slots")) { if (value < 1 || value > 4096) return RT_EINVAL; c->slots_req = value; return RT_OK; }
+    if (!strcmp(key, "rows")) { if (!(value == 1 || value == 2 || value == 4 || value == 8)) return RT_EINVAL; c->rows = value; return RT_OK; }
+    return RT_EINVAL;
+}
+
+// rows per warp actually used for a layout (must divide every Nc of the layout's directions)
+static int rows_for(const rt_ctx *c, int layout)
+{
+    int r = c->rows;
+    for (int i : c->order[layout])
+        while (r > 1 && c->hd[i].Nc % r != 0) r >>= 1;
+    return r;
+}
+
+static int ensure_buffers(rt_ctx *c)
+{
+    if (c->buffers_ready) return RT_OK;
+    const size_t field_bytes = sizeof(float2) * (size_t)c->ncell * c->nbins;
+    const size_t acc_bytes = sizeof(float) * (size_t)c->ncell * c->nbins;
+    size_t freeb = 0, totalb = 0;
+    CK(cudaMemGetInfo(&freeb, &totalb));
+    // slots: enough concurrent directions to fill the machine, bounded by memory (1/3 of free)
+    for (int l = 0; l < 2; ++l) {
+        const int nd = (int)c->order[l].size();
+        int want = 0;
+        if (nd > 0) {
+            if (c->slots_req > 0) want = std::min(nd, c->slots_req);
+            else {
+                // one direction gives Nc/rows warps (owned kernel); aim at ~2400 resident warps
+                int Nc = c->hd[c->order[l][0]].Nc;
+                for (int i : c->order[l]) Nc = std::min(Nc, c->hd[i].Nc);
+                const int warps = std::max(1, Nc / rows_for(c, l)) * c->nbins;
+                want = std::max(1, std::min(nd, (2400 + warps - 1) / warps));
+                if (!c->fast[l]) want = std::min(nd, 16);
+            }
+            const size_t budget = freeb / 3;
+            const size_t need_fixed = 2 * field_bytes;
+            size_t maxs = budget > need_fixed ? (budget - need_fixed) / (4 * acc_bytes) : 1;
+            if (maxs < 1) maxs = 1;
+            want = (int)std::min<size_t>((size_t)want, maxs);
+        }
+        c->slots[l] = want;
+    }
+    for (int l = 0; l < 2; ++l) {
+        {   // both packed copies are always kept (the pack kernel writes both in one pass)
+            cudaError_t e = cudaMalloc(&c->d_P[l], field_bytes);
+            if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RT_ENOMEM : cuda_fail(e);
+        }
+        if (c->slots[l] > 0) {
+            cudaError_t e = cudaMalloc(&c->d_acc[l], acc_bytes * c->slots[l]);
+            if (e == cudaSuccess) e = cudaMalloc(&c->d_accC[l], acc_bytes * c->slots[l]);
+            if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RT_ENOMEM : cuda_fail(e);
+        }
+    }
+    c->buffers_ready = true;
+    return RT_OK;
+}
+
+extern "C" int rt_set_fields(rt_ctx *c, const float *kappa_dev, const float *S_dev, void *stream)
+{
+    if (!c || !kappa_dev || !S_dev) return RT_EINVAL;
+    int rc = ensure_buffers(c);
+    if (rc != RT_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(launch_pack_fields(kappa_dev, S_dev, c->d_P[0], c->d_P[1], c->nx, c->ny, c->nz, c->nbins, st));
+    c->fields_set = true;
+    return RT_OK;
+}
+
+extern "C" int rt_set_inflow(rt_ctx *c, const float *I_bc_host)
+{
+    if (!c || !I_bc_host) return RT_EINVAL;
+    for (int b = 0; b < c->nbins; ++b) if (!(I_bc_host[b] >= 0.0f) || !std::isfinite(I_bc_host[b])) return RT_EINVAL;
+    CK(cudaMemcpy(c->d_Ibc, I_bc_host, sizeof(float) * c->nbins, cudaMemcpyHostToDevice));
+    return RT_OK;
+}
+
+// Enqueue the traversal in `mode` of all directions (only_dir < 0) or of one direction (slot 0 of
+// its layout).  The slot accumulators that will be used are zeroed first; used[l] receives the
+// number of slots of layout l that hold results afterwards.
+static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStream_t st, int *launches, int used[2])
+{
+    const size_t acc_bytes = sizeof(float) * (size_t)c->ncell * nbins;
+    int offset = 0;       // position of the layout's first direction in d_batch
+    used[0] = used[1] = 0;
+    for (int l = 0; l < 2; ++l) {
+        if (c->order[l].empty() || (only_dir >= 0 && c->hd[only_dir].layout != l)) continue;
+        const int S = (only_dir >= 0) ? 1 : c->slots[l];
+        CK(cudaMemsetAsync(c->d_acc[l], 0, acc_bytes * S, st));
+        CK(cudaMemsetAsync(c->d_accC[l], 0, acc_bytes * S, st));
+    }
+    if (mode == MODE_J) CK(cudaEventRecord(c->ev0, st));
+    for (int l = 0; l < 2; ++l) {
+        const int nd = (int)c->order[l].size();
+        const int off_l = offset;
+        offset += nd;
+        if (nd == 0) continue;
+        if (only_dir >= 0 && c->hd[only_dir].layout != l) continue;
+        const int S = (only_dir >= 0) ? 1 : c->slots[l];
+        used[l] = S;
+        SweepLaunch L;
+        memset(&L, 0, sizeof(L));
+        L.P = c->d_P[l]; L.acc = c->d_acc[l]; L.accC = c->d_accC[l];
+        L.dirs = c->d_dirs; L.prog = c->d_prog; L.nbins = nbins; L.ncell = c->ncell; L.Ibc = c->d_Ibc;
+        L.rows = rows_for(c, l); L.mode = mode;
+        L.Nb = (l == 0) ? c->nx : c->ny;
+        // batches never mix dominant axes (Nc differs between y- and z-dominant directions)
+        int i = 0;
+        while (i < nd) {
+            const int a = c->hd[c->order[l][i]].a;
+            int n = 0;
+            while (i + n < nd && n < S && c->hd[c->order[l][i + n]].a == a) ++n;
+            int first = i, count = n;
+            if (only_dir >= 0) {
+                if (c->order[l][i] != only_dir) { i += 1; continue; }
+                count = 1;
+            }
+            L.batch = c->d_batch + off_l + first;
+            L.nslots = count;
+            L.Nc = c->hd[c->order[l][first]].Nc;
+            if (c->fast[l] && owned_supported(L.Nb, L.Nc, L.rows)) {
+                CK(launch_sweep_owned(L, st));
+                ++*launches;
+            } else if (c->flags == RT_ATOMIC_ABLATION) {
+                L.variant = 1;
+                CK(launch_sweep_generic(L, c->np_max[l], c->nq_max[l], st));
+                ++*launches;
+            } else {
+                L.variant = 0;
+                for (int g = 0; g < 4; ++g) {
+                    L.group = g;
+                    CK(launch_sweep_generic(L, c->np_max[l], c->nq_max[l], st));
+                    ++*launches;
+                }
+            }
+            i += count;
+        }
+    }
+    if (mode == MODE_J) { CK(cudaEventRecord(c->ev1, st)); c->ev_valid = true; }
+    return RT_OK;
+}
+
+extern "C" int rt_sweep(rt_ctx *c, float *J_dev, unsigned what, void *stream)
+{
+    if (!c || !J_dev || what > 1u) return RT_EINVAL;
+    if (!c->fields_set) return RT_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    int launches = 0;
+    int used[2];
+    int rc = run_traversal(c, MODE_J, -1, c->nbins, st, &launches, used);
+    if (rc != RT_OK) return rc;
+    CK(launch_normalise(J_dev, c->d_P[0], c->d_acc[0], c->d_accC[0], used[0], c->d_acc[1], c->d_accC[1], used[1],
+                        c->nx, c->ny, c->nz, c->nbins, (float)(1.0 / (double)c->ndirs), what == RT_J_TOTAL ? 1 : 0, st));
+    c->last_launches = launches + 1;
+    return RT_OK;
+}
+
+extern "C" int rt_segment_counts(rt_ctx *c, int dir_index, unsigned int *counts_dev, void *stream)
+{
+    if (!c || !counts_dev || dir_index < -1 || dir_index >= c->ndirs) return RT_EINVAL;
+    int rc = ensure_buffers(c);
+    if (rc != RT_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    int launches = 0;
+    int used[2];
+    rc = run_traversal(c, MODE_COUNT, dir_index, 1, st, &launches, used);
+    if (rc != RT_OK) return rc;
+    CK(launch_counts_finalise(counts_dev, c->d_acc[0], c->d_accC[0], used[0], c->d_acc[1], c->d_accC[1], used[1],
+                              c->nx, c->ny, c->nz, st));
+    return RT_OK;
+}
+
+extern "C" int rt_total_segments(rt_ctx *c, unsigned long long *n_host, void *stream)
+{
+    if (!c || !n_host) return RT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!c->d_cnt) {
+        cudaError_t e = cudaMalloc(&c->d_cnt, sizeof(unsigned) * (size_t)c->ncell);
+        if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RT_ENOMEM : cuda_fail(e);
+    }
+    int rc = rt_segment_counts(c, -1, c->d_cnt, stream);
+    if (rc != RT_OK) return rc;
+    CK(cudaMemsetAsync(c->d_u64, 0, sizeof(unsigned long long), st));
+    CK(launch_sum_u32(c->d_u64, c->d_cnt, c->ncell, st));
+    CK(cudaMemcpyAsync(n_host, c->d_u64, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return RT_OK;
+}
+
+extern "C" int rt_sum_ds(rt_ctx *c, double *sum_host, double *min_host, double *max_host, void *stream)
+{
+    if (!c || !sum_host) return RT_EINVAL;
+    int rc = ensure_buffers(c);
+    if (rc != RT_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    std::vector<double> res(3 * (size_t)c->ndirs);
+    double *d_all = nullptr;
+    cudaError_t e = cudaMalloc(&d_all, sizeof(double) * 3 * (size_t)c->ndirs);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RT_ENOMEM : cuda_fail(e);
+    {
+        std::vector<double> init(3 * (size_t)c->ndirs);
+        for (int i = 0; i < c->ndirs; ++i) { init[3 * i] = 0.0; init[3 * i + 1] = 1.0e300; init[3 * i + 2] = 0.0; }
+        e = cudaMemcpyAsync(d_all, init.data(), sizeof(double) * init.size(), cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { cudaFree(d_all); return cuda_fail(e); }
+    }
+    for (int i = 0; i < c->ndirs; ++i) {
+        int launches = 0, used[2];
+        rc = run_traversal(c, MODE_DS, i, 1, st, &launches, used);
+        if (rc != RT_OK) { cudaFree(d_all); return rc; }
+        const int l = c->hd[i].layout;
+        e = launch_ds_reduce(d_all + 3 * i, c->d_acc[l], c->d_accC[l], c->ncell, st);
+        if (e != cudaSuccess) { cudaFree(d_all); return cuda_fail(e); }
+    }
+    e = cudaMemcpyAsync(res.data(), d_all, sizeof(double) * res.size(), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d_all);
+    if (e != cudaSuccess) return cuda_fail(e);
+    for (int i = 0; i < c->ndirs; ++i) {
+        sum_host[i] = res[3 * i];
+        if (min_host) min_host[i] = res[3 * i + 1];
+        if (max_host) max_host[i] = res[3 * i + 2];
+    }
+    return RT_OK;
+}
+
+extern "C" int rt_direction_records(rt_ctx *c, long long *rec, double *L_host)
+{
+    if (!c || !rec) return RT_EINVAL;
+    for (int i = 0; i < c->ndirs; ++i) {
+        const HostDir &h = c->hd[i];
+        rec[6 * i + 0] = h.a;
+        rec[6 * i + 1] = h.refl[0] | (h.refl[1] << 1) | (h.refl[2] << 2);
+        rec[6 * i + 2] = h.Mb;
+        rec[6 * i + 3] = h.Mc;
+        rec[6 * i + 4] = (c->fast[h.layout] && owned_supported(h.Nb, h.Nc, rows_for(c, h.layout))) ? 0 : 1;
+        rec[6 * i + 5] = 0;
+        if (L_host) L_host[i] = h.L;
+    }
+    return RT_OK;
+}
+
+extern "C" int rt_last_launch_count(rt_ctx *c) { return c ? c->last_launches : RT_EINVAL; }
+
+extern "C" float rt_last_sweep_kernel_ms(rt_ctx *c)
+{
+    if (!c || !c->ev_valid) return -1.0f;
+    if (cudaEventSynchronize(c->ev1) != cudaSuccess) return -1.0f;
+    float ms = -1.0f;
+    if (cudaEventElapsedTime(&ms, c->ev0, c->ev1) != cudaSuccess) return -1.0f;
+    return ms;
+}
+
+extern "C" int rt_destroy(rt_ctx *c)
+{
+    if (!c) return RT_OK;
+    cudaDeviceSynchronize();
+    free_device(c);
+    delete c;
+    return RT_OK;
+}

@@ -1,0 +1,75 @@
+// Internal declarations shared by rt_api.cu (host planner + C ABI) and rt_kernels.cu (sm_100a kernels).
+// Not part of the public boundary (include/rt.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace rt {
+
+constexpr int kF = 20;                         // slope quantisation: 2^-20 (reading A4)
+constexpr long long kOne = 1ll << kF;
+constexpr float kKappaMin = 8.673617379884035e-19f;   // 2^-60: kappa floor in the packed copy (reading A7)
+
+// Slab program: the traversal of ONE slab for ALL rays of a direction (identical because lattice
+// rays differ by whole cells).  Up to three pieces; between pieces the ray steps to the next cell
+// along b (SB), along c (SC) or both.  Zero-length pieces are dropped (P bits clear) but their
+// step still happens (a ray that lands exactly on a cell boundary at the end of the slab).
+struct SlabProg {
+    float len0, len1, len2;                    // path lengths in units of length (frac * L * cell_width)
+    unsigned flags;
+};
+enum : unsigned { F_SB1 = 1u, F_SC1 = 2u, F_SB2 = 4u, F_SC2 = 8u, F_P1 = 16u, F_P2 = 32u };
+
+// Per-direction device record.
+struct DirDev {
+    long long base;      // element offset (within one bin) of canonical (k=0, l=0), memory column 0
+    long long sk, sl;    // signed element strides along canonical k (dominant axis) and l (transverse c)
+    int sj;              // +1 / -1: rays move towards higher / lower memory columns
+    int Na, Nb, Nc;      // extents along a, b (memory-contiguous axis of the layout), c
+    int layout;          // 0: native [z][y][x];  1: transposed [x][z][y] (x-dominant directions)
+    int prog_off;        // index of the first SlabProg of this direction
+    float invL;          // 1 / (L * cell_width)
+    int Mb, Mc;          // quantised slopes (generic kernel recomputes the traversal per ray)
+    int pad;
+};
+static_assert(sizeof(DirDev) == 64, "DirDev layout");
+
+enum Mode : int { MODE_J = 0, MODE_COUNT = 1, MODE_DS = 2 };
+
+struct SweepLaunch {
+    const float2 *P;         // packed (kappa, S) field of the batch's layout, [nbins][cells]
+    float *acc;              // slot accumulators of that layout: [slots][nbins][cells]
+    float *accC;             // seam accumulators, same shape
+    const DirDev *dirs;      // device array of all direction records
+    const SlabProg *prog;    // device array of all slab programs
+    const int *batch;        // device array: direction index per slot of this launch
+    int nslots;              // grid.y
+    int nbins;               // grid.z
+    long long ncell;
+    const float *Ibc;        // device [nbins]
+    int Nb, Nc;              // common to the batch (same layout => same Nb; Nc may differ per direction)
+    int rows;                // rays rows per warp
+    int mode;
+    int variant;             // generic kernel: 0 = four groups (one launch per group), 1 = atomics
+    int group;               // generic kernel: group id 0..3
+};
+
+// launchers (rt_kernels.cu); all return cudaError_t of the launch
+cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, SlabProg *prog, double cell_width,
+                                  const double *Lvals, cudaStream_t st);
+cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat, float2 *PT,
+                               int nx, int ny, int nz, int nbins, cudaStream_t st);
+bool owned_supported(int Nb, int Nc, int rows);
+cudaError_t launch_sweep_owned(const SweepLaunch &L, cudaStream_t st);
+cudaError_t launch_sweep_generic(const SweepLaunch &L, int max_lattice_b, int max_lattice_c, cudaStream_t st);
+cudaError_t launch_normalise(float *J, const float2 *Pnat, const float *accN, const float *accNC, int slotsN,
+                             const float *accT, const float *accTC, int slotsT,
+                             int nx, int ny, int nz, int nbins, float inv_nd, int add_S, cudaStream_t st);
+cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const float *accNC, int slotsN,
+                                   const float *accT, const float *accTC, int slotsT,
+                                   int nx, int ny, int nz, cudaStream_t st);
+// per-cell sum of ds of ONE direction held in slot 0 of the given layout: writes {sum, min, max} (fp64)
+cudaError_t launch_ds_reduce(double *out3, const float *acc, const float *accC, long long ncell, cudaStream_t st);
+cudaError_t launch_sum_u32(unsigned long long *out, const unsigned *counts, long long n, cudaStream_t st);
+
+}  // namespace rt

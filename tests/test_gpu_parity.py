@@ -1,0 +1,343 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle.  All tests need a GPU.
+
+Bars (BASELINE.json north_star): integer traversal data bit-exact; summed ds within 1e-6 relative;
+J within 1e-5 max relative error (reading A14 for the floor).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+J_TOL = 1e-5
+DS_TOL = 1e-6
+
+
+def _torch():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+def rel_err(got, ref):
+    """A14: |got - ref| / max(|ref|, 1e-30 * max|ref|)."""
+    ref = np.asarray(ref, dtype=np.float64)
+    got = np.asarray(got, dtype=np.float64)
+    floor = 1e-30 * max(np.abs(ref).max(), 1e-300)
+    return np.abs(got - ref) / np.maximum(np.abs(ref), floor)
+
+
+def gpu_run(kap, S, dirs, Ibc=None, cell_width=1.0, flags=0, count_dirs=(), want_ds=True, slots=None, rows=None):
+    import paper_1410_0763_b200 as rt
+    torch = _torch()
+    nb, nz, ny, nx = kap.shape
+    tr = rt.RayTracer((nx, ny, nz), nb, dirs, cell_width=cell_width, flags=flags, slots=slots, rows=rows)
+    out = {}
+    try:
+        if Ibc is not None:
+            tr.set_inflow(Ibc)
+        kd = torch.from_numpy(kap).cuda()
+        sd = torch.from_numpy(S).cuda()
+        tr.set_fields(kd, sd)
+        out["Jin"] = tr.sweep(what=rt.RT_J_IN).cpu().numpy()
+        out["J"] = tr.sweep(what=rt.RT_J_TOTAL).cpu().numpy()
+        out["cnt_sum"] = tr.segment_counts(-1).cpu().numpy().astype(np.uint32)
+        out["cnt_dirs"] = np.stack([tr.segment_counts(int(i)).cpu().numpy().astype(np.uint32) for i in count_dirs]) \
+            if len(count_dirs) else None
+        out["seg_total"] = tr.total_segments()
+        if want_ds:
+            out["sum_ds"], out["min_ds"], out["max_ds"] = tr.sum_ds()
+        out["rec"], out["L"] = tr.direction_records()
+        torch.cuda.synchronize()
+    finally:
+        tr.close()
+    return out
+
+
+def sample_dirs(orc, dirs, n=16, seed=0):
+    """Seeded sample of directions that includes every degenerate class (zero slope, unit slope)."""
+    recs = [orc.dir_record(d) for d in dirs]
+    zero = [i for i, r in enumerate(recs) if r["Mb"] == 0 or r["Mc"] == 0]
+    unit = [i for i, r in enumerate(recs) if r["Mb"] == 2 ** 20 or r["Mc"] == 2 ** 20]
+    rng = np.random.default_rng(seed)
+    pick = set(zero[:3] + unit[:3])
+    for a in range(3):
+        cand = [i for i, r in enumerate(recs) if r["a"] == a]
+        pick.update(rng.choice(cand, size=min(3, len(cand)), replace=False).tolist())
+    while len(pick) < min(n, len(dirs)):
+        pick.add(int(rng.integers(0, len(dirs))))
+    return sorted(pick)
+
+
+def check_records(orc, dirs, out):
+    for i, d in enumerate(dirs):
+        r = orc.dir_record(d)
+        assert out["rec"][i, 0] == r["a"]
+        assert out["rec"][i, 1] == r["refl"][0] | (r["refl"][1] << 1) | (r["refl"][2] << 2)
+        assert out["rec"][i, 2] == r["Mb"] and out["rec"][i, 3] == r["Mc"]
+        assert abs(out["L"][i] - r["L"]) <= 1e-15 * r["L"]
+
+
+def check_full(orc, kap, S, dirs, out, ref, cell_width=1.0):
+    ncell = kap.shape[1] * kap.shape[2] * kap.shape[3]
+    # integer traversal data: bit-exact
+    assert np.array_equal(out["cnt_sum"], ref["cnt_sum"])
+    assert out["seg_total"] == ref["seg_total"]
+    if ref.get("cnt_dirs") is not None and out["cnt_dirs"] is not None:
+        assert np.array_equal(out["cnt_dirs"], ref["cnt_dirs"])
+    # summed ds: vs oracle and vs the closed form N_m * L (pin P3)
+    if "sum_ds" in out:
+        assert np.abs(out["sum_ds"] / ref["sum_ds"] - 1).max() <= DS_TOL
+        closed = ncell * out["L"] * cell_width
+        assert np.abs(out["sum_ds"] / closed - 1).max() <= DS_TOL
+        assert np.abs(out["min_ds"] / (out["L"] * cell_width) - 1).max() <= 2e-6
+        assert np.abs(out["max_ds"] / (out["L"] * cell_width) - 1).max() <= 2e-6
+    # J_in (strict) and J
+    e_in = rel_err(out["Jin"], ref["Jin"])
+    e_tot = rel_err(out["J"], ref["J"])
+    assert e_in.max() <= J_TOL, "J_in max rel err %.3e" % e_in.max()
+    assert e_tot.max() <= J_TOL, "J max rel err %.3e" % e_tot.max()
+    return e_in.max()
+
+
+# ---------------------------------------------------------------------------------------------
+def test_healpix_library_matches_oracle(orc):
+    import paper_1410_0763_b200 as rt
+    for nside in (1, 2, 3, 8, 16):
+        assert np.abs(rt.healpix_dirs(nside) - orc.healpix_dirs(nside)).max() <= 1e-15
+
+
+def test_c1_full(orc):
+    """Config 1: 32^3, Nside 2 (48 directions), uniform random fields: everything compared in full."""
+    from rt_inputs import make_fields, CONFIGS
+    kap, S = make_fields("C1")
+    dirs = orc.healpix_dirs(CONFIGS["C1"].nside)
+    out = gpu_run(kap, S, dirs, count_dirs=range(48))
+    ref = orc.sweep(kap, S, dirs, count_dirs=range(48))
+    check_records(orc, dirs, out)
+    assert np.all(out["rec"][:, 4] == 0), "C1 must run on the owned (atomic-free) fast path"
+    check_full(orc, kap, S, dirs, out, ref)
+
+
+def test_c2_full(orc):
+    """Config 2: 64^3, Nside 8 (768 directions), lognormal density."""
+    from rt_inputs import make_fields, CONFIGS
+    kap, S = make_fields("C2")
+    dirs = orc.healpix_dirs(CONFIGS["C2"].nside)
+    cd = sample_dirs(orc, dirs, 16)
+    out = gpu_run(kap, S, dirs, count_dirs=cd)
+    ref = orc.sweep(kap, S, dirs, count_dirs=cd)
+    check_records(orc, dirs, out)
+    assert np.all(out["rec"][:, 4] == 0)
+    check_full(orc, kap, S, dirs, out, ref)
+
+
+@pytest.mark.parametrize("name,dims,nside", [
+    ("C3", (64, 32, 128), 4),      # bubbles generator, anisotropic dims: three different Nb/Nc/Na per axis
+    ("C5", (32, 64, 128), 4),      # 3 bins, anisotropic
+    ("C4", (128, 256, 32), 2),     # wide rows (G = 2 and 4 chunks per thread)
+    ("C2", (256, 32, 64), 2),
+])
+def test_reduced_configs_full(orc, name, dims, nside):
+    """The C3/C4/C5 generators at reduced, anisotropic sizes: full comparison on every cell."""
+    from rt_inputs import make_fields
+    kap, S = make_fields(name, dims=dims)
+    dirs = orc.healpix_dirs(nside)
+    cd = sample_dirs(orc, dirs, 12)
+    out = gpu_run(kap, S, dirs, count_dirs=cd)
+    ref = orc.sweep(kap, S, dirs, count_dirs=cd)
+    check_records(orc, dirs, out)
+    assert np.all(out["rec"][:, 4] == 0)
+    check_full(orc, kap, S, dirs, out, ref)
+
+
+def _sample_cells(dims, n, seed, kap):
+    rng = np.random.default_rng(seed)
+    nx, ny, nz = dims
+    cells = np.stack([rng.integers(0, nx, n), rng.integers(0, ny, n), rng.integers(0, nz, n)], 1)
+    corners = [[0, 0, 0], [nx - 1, ny - 1, nz - 1], [nx - 1, 0, nz - 1], [0, ny - 1, 0], [nx // 2, ny // 2, nz // 2]]
+    # most and least opaque cells (bin 0)
+    zmax, ymax, xmax = np.unravel_index(np.argmax(kap[0]), kap[0].shape)
+    zmin, ymin, xmin = np.unravel_index(np.argmin(kap[0]), kap[0].shape)
+    extra = corners + [[xmax, ymax, zmax], [xmin, ymin, zmin]]
+    return np.unique(np.concatenate([cells, np.array(extra)]), axis=0).astype(np.int32)
+
+
+@pytest.mark.parametrize("name,ncells", [("C3", 40), ("C4", 40), ("C5", 32)])
+def test_full_size_sampled(orc, name, ncells):
+    """Configs 3-5 at BASELINE.json's full sizes, in the launch configuration bench.py times:
+    sampled cells the oracle computes one by one (J_in, J, counts), plus properties that hold at
+    any size (total segments from the per-direction closed count, sum ds = N_m L)."""
+    from rt_inputs import make_fields, CONFIGS
+    import paper_1410_0763_b200 as rt
+    torch = _torch()
+    spec = CONFIGS[name]
+    kap, S = make_fields(name)
+    nb, nz, ny, nx = kap.shape
+    dirs = orc.healpix_dirs(spec.nside)
+    cells = _sample_cells(spec.dims, ncells, 7, kap)
+    ref = orc.sweep_cells(kap, S, dirs, cells)
+    tr = rt.RayTracer(spec.dims, nb, dirs)
+    try:
+        kd, sd = torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda()
+        tr.set_fields(kd, sd)
+        Jin = tr.sweep(what=rt.RT_J_IN)
+        J = tr.sweep(what=rt.RT_J_TOTAL)
+        cnt = tr.segment_counts(-1)
+        seg_total = tr.total_segments()
+        rec, L = tr.direction_records()
+        assert np.all(rec[:, 4] == 0)
+        ix = torch.from_numpy(cells.astype(np.int64)).cuda()
+        got_in = Jin[:, ix[:, 2], ix[:, 1], ix[:, 0]].cpu().numpy()
+        got_J = J[:, ix[:, 2], ix[:, 1], ix[:, 0]].cpu().numpy()
+        got_cnt = cnt[ix[:, 2], ix[:, 1], ix[:, 0]].cpu().numpy().astype(np.uint32)
+        assert bool(torch.isfinite(Jin).all()) and float(Jin.min()) >= 0.0
+        cnt_total = int(cnt.to(torch.int64).sum().item())
+    finally:
+        tr.close()
+    assert np.array_equal(got_cnt, ref["cnt"])                       # integer data: bit-exact
+    assert seg_total == cnt_total
+    e_in, e_J = rel_err(got_in, ref["Jin"]), rel_err(got_J, ref["J"])
+    assert e_in.max() <= J_TOL, "%s J_in max rel err %.3e" % (name, e_in.max())
+    assert e_J.max() <= J_TOL, "%s J max rel err %.3e" % (name, e_J.max())
+    # segments per direction: N_m (1 + m_b + m_c) within the degenerate-slope deficit (pin P4 band)
+    pred = spec.ncell * np.sum(1.0 + rec[:, 2] / 2.0 ** 20 + rec[:, 3] / 2.0 ** 20)
+    assert abs(seg_total - pred) < 0.02 * pred
+
+
+def test_full_size_sum_ds_c3(orc):
+    """Sum of ds per direction at a full benchmark size against the closed form N_m * L (P3)."""
+    from rt_inputs import CONFIGS
+    import paper_1410_0763_b200 as rt
+    _torch()
+    spec = CONFIGS["C3"]
+    dirs = orc.healpix_dirs(spec.nside)[::24]          # 128 of the 3072 directions
+    tr = rt.RayTracer(spec.dims, 1, dirs)
+    try:
+        s, mn, mx = tr.sum_ds()
+        rec, L = tr.direction_records()
+    finally:
+        tr.close()
+    assert np.abs(s / (spec.ncell * L) - 1).max() <= DS_TOL
+    assert np.abs(mn / L - 1).max() <= 2e-6 and np.abs(mx / L - 1).max() <= 2e-6
+
+
+# ---------------------------------------------------------------------------------------------
+# edge cases
+def _rand(dims, seed, nb=1):
+    nx, ny, nz = dims
+    rng = np.random.default_rng(seed)
+    return (rng.uniform(0.05, 2.0, (nb, nz, ny, nx)).astype(np.float32),
+            rng.uniform(0.0, 1.0, (nb, nz, ny, nx)).astype(np.float32))
+
+
+@pytest.mark.parametrize("dims", [(20, 12, 10), (33, 7, 5), (1, 1, 1), (64, 20, 12), (20, 64, 12)])
+def test_generic_fallback_dims(orc, dims):
+    """Mesh sizes the owned kernel does not cover run on the generic (four-group) kernel; mixed cases
+    (one layout fast, the other generic) too.  Same gates."""
+    kap, S = _rand(dims, 5)
+    dirs = orc.healpix_dirs(2)
+    out = gpu_run(kap, S, dirs, count_dirs=range(0, 48, 5))
+    ref = orc.sweep(kap, S, dirs, count_dirs=range(0, 48, 5))
+    check_records(orc, dirs, out)
+    check_full(orc, kap, S, dirs, out, ref)
+
+
+@pytest.mark.parametrize("flags", [1, 2])
+def test_ablation_variants_pass_the_same_gates(orc, flags):
+    """RT_ATOMIC_ABLATION and RT_PAPER_GROUPS differ from the owned path only by summation order."""
+    from rt_inputs import make_fields
+    kap, S = make_fields("C1")
+    dirs = orc.healpix_dirs(2)
+    out = gpu_run(kap, S, dirs, flags=flags, count_dirs=range(0, 48, 7))
+    ref = orc.sweep(kap, S, dirs, count_dirs=range(0, 48, 7))
+    assert np.all(out["rec"][:, 4] == 1)
+    check_full(orc, kap, S, dirs, out, ref)
+
+
+@pytest.mark.parametrize("rows", [1, 2, 4, 8])
+def test_rows_per_warp_variants(orc, rows):
+    kap, S = _rand((64, 32, 16), 9)
+    dirs = orc.healpix_dirs(2)
+    out = gpu_run(kap, S, dirs, rows=rows, slots=5, count_dirs=[0, 13, 47])
+    ref = orc.sweep(kap, S, dirs, count_dirs=[0, 13, 47])
+    check_full(orc, kap, S, dirs, out, ref)
+
+
+def test_inflow_cellwidth_multibin(orc):
+    kap, S = _rand((32, 64, 16), 11, nb=3)
+    dirs = orc.healpix_dirs(2)
+    Ibc = [0.5, 0.0, 2.0]
+    out = gpu_run(kap, S, dirs, Ibc=Ibc, cell_width=0.7)
+    ref = orc.sweep(kap, S, dirs, Ibc=Ibc, cell_width=0.7)
+    check_full(orc, kap, S, dirs, out, ref, cell_width=0.7)
+
+
+def test_degenerate_directions(orc):
+    """Axis-aligned, exact diagonals, unit slopes, half slopes (crossings on slab planes), near-degenerate."""
+    kap, S = _rand((32, 32, 32), 13)
+    dirs = np.array([[1, 0, 0], [-1, 0, 0], [0, 1, 0], [0, -1, 0], [0, 0, 1], [0, 0, -1], [1, 1, 1], [-1, 1, -1],
+                     [1, 1, 0], [0, -1, 1], [1, 0.5, 0.25], [0.5, -1, 0.5], [1, 0.999999, 1e-6], [0.25, 0.75, -1],
+                     [1e-7, 1, 1e-7]], dtype=np.float64)
+    out = gpu_run(kap, S, dirs, count_dirs=range(len(dirs)))
+    ref = orc.sweep(kap, S, dirs, count_dirs=range(len(dirs)))
+    check_records(orc, dirs, out)
+    check_full(orc, kap, S, dirs, out, ref)
+
+
+def test_kappa_zero_and_extremes(orc):
+    """kappa = 0 (A7), tiny and huge optical depths: finite, and within tolerance (kappa floor 2^-60)."""
+    kap, S = _rand((32, 32, 32), 17)
+    kap[0, 8:12] = 0.0
+    kap[0, 20:22] = 1e-6
+    kap[0, 25:27] = 300.0
+    dirs = orc.healpix_dirs(2)
+    out = gpu_run(kap, S, dirs, want_ds=False)
+    ref = orc.sweep(kap, S, dirs)
+    assert np.all(np.isfinite(out["Jin"]))
+    assert np.array_equal(out["cnt_sum"], ref["cnt_sum"])
+    # behind 300 mean free paths per cell J_in of the far side underflows; A14 floor handles it
+    assert rel_err(out["Jin"], ref["Jin"]).max() <= J_TOL
+    assert rel_err(out["J"], ref["J"]).max() <= J_TOL
+
+
+def test_error_codes():
+    import paper_1410_0763_b200 as rt
+    torch = _torch()
+    d = rt.healpix_dirs(1)
+    for bad in [dict(nx=0), dict(nbins=0), dict(nbins=17), dict(rays=2), dict(cw=0.0), dict(flags=7)]:
+        with pytest.raises(rt.RtError) as ei:
+            rt.rt_create(bad.get("nx", 8), 8, 8, bad.get("nbins", 1), d, bad.get("rays", 1), bad.get("cw", 1.0),
+                         bad.get("flags", 0))
+        assert ei.value.code == -1
+    with pytest.raises(rt.RtError):
+        rt.rt_create(8, 8, 8, 1, np.zeros((1, 3)))
+    h = rt.rt_create(8, 8, 8, 1, d)
+    try:
+        J = torch.empty(512, dtype=torch.float32, device="cuda")
+        with pytest.raises(rt.RtError) as ei:
+            rt.rt_sweep(h, J, 512)                      # fields not set
+        assert ei.value.code == -4
+    finally:
+        rt.rt_destroy(h)
+
+
+def test_sweep_is_deterministic_and_repeatable(orc):
+    from rt_inputs import make_fields
+    import paper_1410_0763_b200 as rt
+    torch = _torch()
+    kap, S = make_fields("C1")
+    dirs = orc.healpix_dirs(2)
+    tr = rt.RayTracer((32, 32, 32), 1, dirs)
+    try:
+        tr.set_fields(torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda())
+        a = tr.sweep().clone()
+        b = tr.sweep().clone()
+        assert torch.equal(a, b)                       # atomic-free: bitwise reproducible
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            c = tr.sweep(stream=st).clone()
+        st.synchronize()
+        assert torch.equal(a, c)
+        assert tr.last_launch_count() >= 2
+    finally:
+        tr.close()
