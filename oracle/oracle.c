@@ -155,8 +155,7 @@ static inline void do_segment(orc_work_t *w, size_t cell, double ds, double *I)
         double dtau = (double)w->kappa[o] * ds;
         if (!w->slot || w->slot[cell] >= 0)
             w->num[o] += ds * I[bin] * f_of(dtau);                       /* eq. 8 weighted by ds (A7) */
-        double em1 = expm1(-dtau);                                        /* e^-dtau - 1 */
-        I[bin] = I[bin] * (1.0 + em1) + (double)w->S[o] * (-em1);        /* eq. 7 */
+        I[bin] = I[bin] * exp(-dtau) + (double)w->S[o] * (-expm1(-dtau));  /* eq. 7, term by term */
     }
 }
 

@@ -114,7 +114,7 @@ cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat,
 // ------------------------------------------------------------------------------------------------
 // Segment update (eq. 7, eq. 8), fp32
 //   A = 1 - exp(-kappa*len); contribution to the cell += I_in * A  (numerator of eq. 11 times kappa*L,
-//   see DESIGN.md "Arithmetic"); I_out = I_in + (S - I_in) * A.
+//   see DESIGN.md "Arithmetic"); I_out = I_in * e + S * A with e = exp(-kappa*len).
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ float ex2_approx(float x)
 {
@@ -123,24 +123,28 @@ __device__ __forceinline__ float ex2_approx(float x)
     return y;
 }
 
-__device__ __forceinline__ float one_minus_exp(float kap, float len, float ct)
+// e = exp(-kappa*len) and A = 1 - e, each with small RELATIVE error: e straight from ex2 (never as
+// 1 - A: behind an opaque cell the transmitted part I*e is all that is left), A from a polynomial
+// where 1 - e would cancel.
+__device__ __forceinline__ float one_minus_exp(float kap, float len, float ct, float &e)
 {
     const float x = kap * len;
-    const float big = 1.0f - ex2_approx(kap * ct);            // ct = -len*log2(e)
+    e = ex2_approx(kap * ct);                                  // ct = -len*log2(e)
     // small-x branch: x * (c0 + c1 x + c2 x^2 + c3 x^3), fitted on [0, 1/4]; rel. error 3.4e-7
     float p = fmaf(x, -0.0377338513f, 0.1660640817f);
     p = fmaf(x, p, -0.4999701648f);
     p = fmaf(x, p, 0.9999997683f);
-    return x < 0.25f ? x * p : big;
+    return x < 0.25f ? x * p : 1.0f - e;
 }
 
 template <int MODE>
 __device__ __forceinline__ void seg_update(float &I, float kap, float src, float len, float ct, float &part)
 {
     if (MODE == MODE_J) {
-        const float A = one_minus_exp(kap, len, ct);
+        float e;
+        const float A = one_minus_exp(kap, len, ct, e);
         part = fmaf(I, A, part);
-        I = fmaf(src - I, A, I);
+        I = fmaf(I, e, src * A);                               // eq. 7
     } else if (MODE == MODE_COUNT) {
         part += 1.0f;
     } else {
@@ -465,9 +469,10 @@ k_sweep_generic(const SweepLaunch L, int np_max, int nq_max)
             float v = 0.0f;
             if (MODE == MODE_J) {
                 const float2 ks = P[o];
-                const float A = one_minus_exp(ks.x, len, -len * 1.4426950408889634f);
+                float e;
+                const float A = one_minus_exp(ks.x, len, -len * 1.4426950408889634f, e);
                 v = I * A * invL;
-                I = fmaf(ks.y - I, A, I);
+                I = fmaf(I, e, ks.y * A);
             } else if (MODE == MODE_COUNT) {
                 v = 1.0f;
             } else {

@@ -22,7 +22,7 @@ def rel_err(got, ref):
     """A14: |got - ref| / max(|ref|, 1e-30 * max|ref|)."""
     ref = np.asarray(ref, dtype=np.float64)
     got = np.asarray(got, dtype=np.float64)
-    floor = 1e-30 * max(np.abs(ref).max(), 1e-300)
+    floor = max(1e-30 * np.abs(ref).max(), 1e-300)
     return np.abs(got - ref) / np.maximum(np.abs(ref), floor)
 
 
