@@ -55,7 +55,7 @@ def _gaussian_field(rng, dims):
     """Zero-mean unit-variance Gaussian random field with P(k) ~ k^-3, shape (nz, ny, nx)."""
     nx, ny, nz = dims
     white = rng.standard_normal((nz, ny, nx))
-    fk = np.fft.rfftn(white)
+    fk = np.fft.rfftn(white, axes=(0, 1, 2))
     kz = 2.0 * np.pi * np.fft.fftfreq(nz)[:, None, None]
     ky = 2.0 * np.pi * np.fft.fftfreq(ny)[None, :, None]
     kx = 2.0 * np.pi * np.fft.rfftfreq(nx)[None, None, :]
@@ -65,7 +65,7 @@ def _gaussian_field(rng, dims):
     amp[0, 0, 0] = 0.0
     fk *= amp
     del amp, k2
-    g = np.fft.irfftn(fk, s=(nz, ny, nx))
+    g = np.fft.irfftn(fk, s=(nz, ny, nx), axes=(0, 1, 2))
     del fk
     g -= g.mean()
     g /= g.std()

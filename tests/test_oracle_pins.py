@@ -176,6 +176,18 @@ def test_p5_uniform_slab_closed_form(orc):
     assert np.allclose(t["exitI"][..., 0], 0.9 * np.exp(-tau) + s64 * (1 - np.exp(-tau)), rtol=1e-13)
 
 
+def test_p5_pure_absorption_keeps_relative_accuracy(orc):
+    """S = 0, inflow I_bc: exit intensity = I_bc exp(-kappa * chord) down to 1e-49 with full relative
+    accuracy (eq. 7 evaluated term by term: the transmitted part must not be formed as 1 - (1 - e))."""
+    kap = np.full((1, 8, 12, 10), 8.0, dtype=np.float32)
+    S = np.zeros_like(kap)
+    t = orc.trace_direction(kap, S, [1, 0.37, 0.81], Ibc=[1.0])
+    expect = np.exp(-8.0 * t["chord"])
+    inside = t["chord"] > 0
+    assert expect[inside].min() < 1e-40
+    assert np.allclose(t["exitI"][..., 0][inside], expect[inside], rtol=1e-12, atol=0)
+
+
 def test_p5_chord_total_is_volume_over_cross_section(orc):
     dims = (10, 12, 8)
     kap, S = rand_fields(dims, 9)
