@@ -180,18 +180,131 @@ template <>
 __device__ __forceinline__ void unpack<1>(const float2 &v, float (&kap)[1], float (&src)[1])
 { kap[0] = v.x; src[0] = v.y; }
 
-__device__ __forceinline__ void acc_rmw(float2 *p, const float (&part)[2], float w)
-{
-    float2 o = *p;
-    o.x = fmaf(part[0], w, o.x); o.y = fmaf(part[1], w, o.y);
-    *p = o;
-}
-__device__ __forceinline__ void acc_rmw(float *p, const float (&part)[1], float w)
-{
-    *p = fmaf(part[0], w, *p);
-}
-
 constexpr int kWarpsPerCta = 4;
+
+__device__ __forceinline__ float  vfma(float part0, float w, float o)  { return fmaf(part0, w, o); }
+
+template <int CW>
+__device__ __forceinline__ typename VecT<CW>::A acc_new(const typename VecT<CW>::A &o, const float (&part)[CW], float w);
+template <>
+__device__ __forceinline__ float2 acc_new<2>(const float2 &o, const float (&part)[2], float w)
+{ return make_float2(fmaf(part[0], w, o.x), fmaf(part[1], w, o.y)); }
+template <>
+__device__ __forceinline__ float acc_new<1>(const float &o, const float (&part)[1], float w)
+{ return fmaf(part[0], w, o); }
+
+// The six slab patterns that occur away from exact boundary touches get straight-line code
+// (FLC = compile-time flags); anything else runs the same body with run-time flags (FLC < 0).
+constexpr int kPatNone = 0;
+constexpr int kPatB    = F_SB1 | F_P1;
+constexpr int kPatC    = F_SC1 | F_P1;
+constexpr int kPatBC   = F_SB1 | F_P1 | F_SC2 | F_P2;
+constexpr int kPatCB   = F_SC1 | F_P1 | F_SB2 | F_P2;
+constexpr int kPatD    = F_SB1 | F_SC1 | F_P1;
+
+// One slab for the R rays rows of a warp.  rowd[r] = packed data of memory row (lbase + r) of this
+// slab (r = R: the seam row, valid only if some piece steps along c); acco / accCo = old
+// accumulator values of the rows this warp owns / of the seam row.
+template <int CW, int G, int R, int MODE, int FLC>
+__device__ __forceinline__ void slab_rows(const unsigned fl_rt, float (&I)[R][G][CW],
+                                          const typename VecT<CW>::D (&rowd)[R + 1][G],
+                                          const typename VecT<CW>::A (&acco)[R][G],
+                                          const typename VecT<CW>::A (&accCo)[G],
+                                          const float len0, const float len1, const float len2,
+                                          const float Ibc, const float invL, const int lane, const bool rev,
+                                          const int lbase, const int Nc,
+                                          float *__restrict__ acc, float *__restrict__ accC,
+                                          const long long (&orow)[R + 1], const int (&col)[G])
+{
+    using AV = typename VecT<CW>::A;
+    constexpr unsigned FULL = 0xffffffffu;
+    constexpr float LOG2E = 1.4426950408889634f;
+    const unsigned fl = (FLC >= 0) ? (unsigned)FLC : fl_rt;
+    const float ct0 = -len0 * LOG2E, ct1 = -len1 * LOG2E, ct2 = -len2 * LOG2E;
+    const bool anySC = (fl & (F_SC1 | F_SC2)) != 0;
+
+    float part_cur[G][CW];
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int i = 0; i < CW; ++i) part_cur[g][i] = 0.0f;
+
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        int l_r = lbase + r; if (l_r >= Nc) l_r -= Nc;
+        const bool wrap_r = (l_r == Nc - 1);
+        float part_next[G][CW];
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int i = 0; i < CW; ++i) part_next[g][i] = 0.0f;
+
+        float carry = Ibc;            // intensity handed from chunk g-1 (a new ray for g = 0)
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            float kc[CW], sc[CW], kn[CW], sn[CW];
+            unpack<CW>(rowd[r][g], kc, sc);
+            unpack<CW>(rowd[r + 1][g], kn, sn);
+            float (&Iu)[CW] = I[r][g];
+#pragma unroll
+            for (int i = 0; i < CW; ++i) seg_update<MODE>(Iu[i], kc[i], sc[i], len0, ct0, part_cur[g][i]);
+            bool sel = false;
+#pragma unroll
+            for (int stage = 1; stage <= 2; ++stage) {
+                const unsigned fsb = (stage == 1) ? F_SB1 : F_SB2;
+                const unsigned fsc = (stage == 1) ? F_SC1 : F_SC2;
+                const unsigned fp = (stage == 1) ? F_P1 : F_P2;
+                const float len = (stage == 1) ? len1 : len2;
+                const float ct = (stage == 1) ? ct1 : ct2;
+                if (fl & (fsb | fsc)) {
+                    if (MODE == MODE_J) {
+                        if (fl & fsb) {       // step along b: hand every ray to the next column's owner
+                            const float out = rev ? Iu[0] : Iu[CW - 1];
+                            const float t = __shfl_sync(FULL, out, (lane + 31) & 31);
+                            const float in = (lane == 0) ? carry : t;
+                            carry = t;
+                            if (CW == 2) {
+                                const float keep = rev ? Iu[CW - 1] : Iu[0];
+                                Iu[0] = rev ? keep : in;
+                                Iu[CW - 1] = rev ? in : keep;
+                            } else {
+                                Iu[0] = in;
+                            }
+                        }
+                        if ((fl & fsc) && wrap_r) {   // step along c out of the box: new rays enter
+#pragma unroll
+                            for (int i = 0; i < CW; ++i) Iu[i] = Ibc;
+                        }
+                    }
+                    if (fl & fsc) sel = true;
+                }
+                if (fl & fp) {
+                    if (sel) {
+#pragma unroll
+                        for (int i = 0; i < CW; ++i) seg_update<MODE>(Iu[i], kn[i], sn[i], len, ct, part_next[g][i]);
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < CW; ++i) seg_update<MODE>(Iu[i], kc[i], sc[i], len, ct, part_cur[g][i]);
+                    }
+                }
+            }
+        }
+        // row r's partial is complete (own pieces + pieces of ray row r-1 that stepped along c)
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+            *reinterpret_cast<AV *>(acc + orow[r] + col[g]) = acc_new<CW>(acco[r][g], part_cur[g], invL);
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int i = 0; i < CW; ++i) part_cur[g][i] = part_next[g][i];
+    }
+    if (anySC) {
+        // seam: the partial of the memory row above the warp's last ray row has another owner
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+            *reinterpret_cast<AV *>(accC + orow[R] + col[g]) = acc_new<CW>(accCo[g], part_cur[g], invL);
+    }
+}
 
 template <int CW, int G, int R, int MODE>
 __global__ void __launch_bounds__(32 * kWarpsPerCta)
@@ -199,8 +312,6 @@ k_sweep_owned(const SweepLaunch L)
 {
     using DV = typename VecT<CW>::D;
     using AV = typename VecT<CW>::A;
-    constexpr unsigned FULL = 0xffffffffu;
-    constexpr float LOG2E = 1.4426950408889634f;
 
     const int lane = threadIdx.x & 31;
     const int slot = blockIdx.y, bin = blockIdx.z;
@@ -233,131 +344,55 @@ k_sweep_owned(const SweepLaunch L)
 #pragma unroll
             for (int i = 0; i < CW; ++i) I[r][g][i] = Ibc;
 
+    // inputs of the current slab, loaded one slab ahead (software prefetch in registers)
+    DV rowd[R + 1][G];
+    AV acco[R][G], accCo[G];
+    long long orow[R + 1];
     int lbase = q0;                       // memory row (canonical l) of ray row 0 in the current slab
     SlabProg pr = prog[0];
-    // data of ray row 0 of the current slab
-    DV cur[G];
-    {
-        const long long o = (long long)lbase * sl;
+
+    auto issue_loads = [&](int k, int lb, bool withSeam) {
+        const long long offk = (long long)k * sk;
 #pragma unroll
-        for (int g = 0; g < G; ++g) cur[g] = *reinterpret_cast<const DV *>(P + o + col[g]);
-    }
+        for (int r = 0; r <= R; ++r) {
+            int l = lb + r; if (l >= Nc) l -= Nc;
+            orow[r] = offk + (long long)l * sl;
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+                rowd[r][g] = *reinterpret_cast<const DV *>(P + orow[r] + col[g]);
+                acco[r][g] = *reinterpret_cast<const AV *>(acc + orow[r] + col[g]);
+            }
+        if (withSeam) {
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+                rowd[R][g] = *reinterpret_cast<const DV *>(P + orow[R] + col[g]);
+                accCo[g] = *reinterpret_cast<const AV *>(accC + orow[R] + col[g]);
+            }
+        }
+    };
+    issue_loads(0, lbase, (pr.flags & (F_SC1 | F_SC2)) != 0);
 
     for (int k = 0; k < Na; ++k) {
         const unsigned fl = pr.flags;
         const float len0 = pr.len0, len1 = pr.len1, len2 = pr.len2;
-        const float ct0 = -len0 * LOG2E, ct1 = -len1 * LOG2E, ct2 = -len2 * LOG2E;
-        const bool anySC = (fl & (F_SC1 | F_SC2)) != 0;
-        const long long offk = (long long)k * sk;
         if (k + 1 < Na) pr = prog[k + 1];
-        int lnext0 = lbase + (anySC ? 1 : 0);
-        if (lnext0 >= Nc) lnext0 -= Nc;
-
-        float part_cur[G][CW];
-#pragma unroll
-        for (int g = 0; g < G; ++g)
-#pragma unroll
-            for (int i = 0; i < CW; ++i) part_cur[g][i] = 0.0f;
-
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            int l_r = lbase + r;      if (l_r >= Nc) l_r -= Nc;
-            int l_n = l_r + 1;        if (l_n >= Nc) l_n -= Nc;
-            const bool wrap_r = (l_r == Nc - 1);
-            const long long orow = offk + (long long)l_r * sl;
-            const long long onext = offk + (long long)l_n * sl;
-            // data of the next memory row: it is ray row r+1's own row (always needed) or, for the
-            // last ray row, the seam row (needed only if some piece steps along c in this slab)
-            DV nxt[G];
-            if (r + 1 < R || anySC) {
-#pragma unroll
-                for (int g = 0; g < G; ++g) nxt[g] = *reinterpret_cast<const DV *>(P + onext + col[g]);
-            } else {
-#pragma unroll
-                for (int g = 0; g < G; ++g) nxt[g] = cur[g];
-            }
-            float part_next[G][CW];
-#pragma unroll
-            for (int g = 0; g < G; ++g)
-#pragma unroll
-                for (int i = 0; i < CW; ++i) part_next[g][i] = 0.0f;
-
-            float carry = Ibc;            // intensity handed from chunk g-1 (a new ray for g = 0)
-#pragma unroll
-            for (int g = 0; g < G; ++g) {
-                float kc[CW], sc[CW], kn[CW], sn[CW];
-                unpack<CW>(cur[g], kc, sc);
-                unpack<CW>(nxt[g], kn, sn);
-                float (&Iu)[CW] = I[r][g];
-                // piece 0: always in the entry cell
-#pragma unroll
-                for (int i = 0; i < CW; ++i) seg_update<MODE>(Iu[i], kc[i], sc[i], len0, ct0, part_cur[g][i]);
-                bool sel = false;
-#pragma unroll
-                for (int stage = 1; stage <= 2; ++stage) {
-                    const unsigned fsb = (stage == 1) ? F_SB1 : F_SB2;
-                    const unsigned fsc = (stage == 1) ? F_SC1 : F_SC2;
-                    const unsigned fp = (stage == 1) ? F_P1 : F_P2;
-                    const float len = (stage == 1) ? len1 : len2;
-                    const float ct = (stage == 1) ? ct1 : ct2;
-                    if (fl & (fsb | fsc)) {
-                        if (MODE == MODE_J) {
-                            if (fl & fsb) {       // step along b: hand every ray to the next column's owner
-                                const float out = rev ? Iu[0] : Iu[CW - 1];
-                                const float t = __shfl_sync(FULL, out, (lane + 31) & 31);
-                                const float in = (lane == 0) ? carry : t;
-                                carry = t;
-                                if (!rev) {
-#pragma unroll
-                                    for (int i = CW - 1; i > 0; --i) Iu[i] = Iu[i - 1];
-                                    Iu[0] = in;
-                                } else {
-#pragma unroll
-                                    for (int i = 0; i < CW - 1; ++i) Iu[i] = Iu[i + 1];
-                                    Iu[CW - 1] = in;
-                                }
-                            }
-                            if ((fl & fsc) && wrap_r) {   // step along c out of the box: new rays enter
-#pragma unroll
-                                for (int i = 0; i < CW; ++i) Iu[i] = Ibc;
-                            }
-                        }
-                        if (fl & fsc) sel = true;
-                    }
-                    if (fl & fp) {
-                        if (sel) {
-#pragma unroll
-                            for (int i = 0; i < CW; ++i) seg_update<MODE>(Iu[i], kn[i], sn[i], len, ct, part_next[g][i]);
-                        } else {
-#pragma unroll
-                            for (int i = 0; i < CW; ++i) seg_update<MODE>(Iu[i], kc[i], sc[i], len, ct, part_cur[g][i]);
-                        }
-                    }
-                }
-            }
-            // row r's partial is complete (own pieces + pieces of ray row r-1 that stepped along c)
-#pragma unroll
-            for (int g = 0; g < G; ++g)
-                acc_rmw(reinterpret_cast<AV *>(acc + orow + col[g]), part_cur[g], invL);
-#pragma unroll
-            for (int g = 0; g < G; ++g) {
-                cur[g] = nxt[g];
-#pragma unroll
-                for (int i = 0; i < CW; ++i) part_cur[g][i] = part_next[g][i];
-            }
-            if (r == R - 1 && anySC) {
-                // seam: the partial of the memory row above the warp's last ray row has another owner
-#pragma unroll
-                for (int g = 0; g < G; ++g)
-                    acc_rmw(reinterpret_cast<AV *>(accC + onext + col[g]), part_cur[g], invL);
-            }
+#define RT_BODY(FLC) slab_rows<CW, G, R, MODE, FLC>(fl, I, rowd, acco, accCo, len0, len1, len2, Ibc, invL, lane, rev, \
+                                                    lbase, Nc, acc, accC, orow, col)
+        switch (fl) {
+        case kPatNone: RT_BODY(kPatNone); break;
+        case kPatB:    RT_BODY(kPatB); break;
+        case kPatC:    RT_BODY(kPatC); break;
+        case kPatBC:   RT_BODY(kPatBC); break;
+        case kPatCB:   RT_BODY(kPatCB); break;
+        case kPatD:    RT_BODY(kPatD); break;
+        default:       RT_BODY(-1); break;
         }
-        lbase = lnext0;
-        if (k + 1 < Na) {
-            const long long o = (long long)(k + 1) * sk + (long long)lbase * sl;
-#pragma unroll
-            for (int g = 0; g < G; ++g) cur[g] = *reinterpret_cast<const DV *>(P + o + col[g]);
-        }
+#undef RT_BODY
+        if (fl & (F_SC1 | F_SC2)) { lbase += 1; if (lbase >= Nc) lbase -= Nc; }
+        if (k + 1 < Na) issue_loads(k + 1, lbase, (pr.flags & (F_SC1 | F_SC2)) != 0);
     }
 }
 
