@@ -141,6 +141,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--slots", type=int, default=None)
     ap.add_argument("--rows", type=int, default=None)
+    ap.add_argument("--stages", type=int, default=None)
     ap.add_argument("--flags", type=int, default=0, help="0 owned, 1 atomic ablation, 2 paper's four groups")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -163,7 +164,7 @@ def main():
     spec = CONFIGS[args.config]
     kap, S = make_fields(args.config)
     dirs = rt.healpix_dirs(spec.nside)
-    tr = rt.RayTracer(spec.dims, spec.nbins, dirs, flags=args.flags, slots=args.slots, rows=args.rows)
+    tr = rt.RayTracer(spec.dims, spec.nbins, dirs, flags=args.flags, slots=args.slots, rows=args.rows, stages=args.stages)
     stream = torch.cuda.current_stream()
     kap_h = torch.from_numpy(kap).pin_memory()
     S_h = torch.from_numpy(S).pin_memory()

@@ -39,10 +39,12 @@ struct rt_ctx {
     double cell_width = 1.0;
     unsigned flags = 0;
     int device = 0;
+    int sm_count = 148;
     std::vector<HostDir> hd;
     std::vector<int> order[2];       // direction indices per layout, sorted by work (descending)
     bool fast[2] = {false, false};   // owned kernel usable for the layout
-    int rows = 4;
+    int rows = 2;
+    int stages = 2;                  // depth of the owned kernel's TMA shared-memory ring (0 = register path)
     int slots_req = 0;               // user override
     int slots[2] = {0, 0};           // allocated slots per layout
     bool fields_set = false;
@@ -136,6 +138,7 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     c->nx = nx; c->ny = ny; c->nz = nz; c->nbins = nbins; c->ndirs = ndirs;
     c->ncell = (long long)nx * ny * nz; c->cell_width = cell_width; c->flags = flags;
     cudaGetDevice(&c->device);
+    cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device);
     const int dims[3] = {nx, ny, nz};
 
     // ---- direction records (reading O2): plain IEEE fp64 operations in a fixed order
@@ -228,7 +231,8 @@ extern "C" int rt_tune(rt_ctx *c, const char *key, int value)
     if (!c || !key) return RT_EINVAL;
     if (c->buffers_ready) return RT_ESTATE;
     if (!strcmp(key, "slots")) { if (value < 1 || value > 4096) return RT_EINVAL; c->slots_req = value; return RT_OK; }
-    if (!strcmp(key, "rows")) { if (!(value == 1 || value == 2 || value == 4 || value == 8)) return RT_EINVAL; c->rows = value; return RT_OK; }
+    if (!strcmp(key, "stages")) { if (!(value == 0 || (value >= 2 && value <= 4))) return RT_EINVAL; c->stages = value; return RT_OK; }
+    if (!strcmp(key, "rows")) { if (!(value == 1 || value == 2 || value == 4)) return RT_EINVAL; c->rows = value; return RT_OK; }
     return RT_EINVAL;
 }
 
@@ -255,11 +259,16 @@ static int ensure_buffers(rt_ctx *c)
         if (nd > 0) {
             if (c->slots_req > 0) want = std::min(nd, c->slots_req);
             else {
-                // one direction gives Nc/rows warps (owned kernel); aim at ~2400 resident warps
+                // one direction gives ceil(Nc/rows/4) CTAs per bin (owned kernel): fill the machine with
+                // exactly one wave of resident CTAs, no partial second wave
                 int Nc = c->hd[c->order[l][0]].Nc;
                 for (int i : c->order[l]) Nc = std::min(Nc, c->hd[i].Nc);
-                const int warps = std::max(1, Nc / rows_for(c, l)) * c->nbins;
-                want = std::max(1, std::min(nd, (2400 + warps - 1) / warps));
+                const int rows = rows_for(c, l);
+                const int ctas_dir = ((Nc / rows + kOwnedWarpsPerCta - 1) / kOwnedWarpsPerCta) * c->nbins;
+                int per_sm = c->fast[l] ? owned_ctas_per_sm(l == 0 ? c->nx : c->ny, rows, c->stages) : 0;
+                if (per_sm < 1) per_sm = 4;
+                const int resident = per_sm * c->sm_count;
+                want = std::max(1, std::min(nd, resident / std::max(1, ctas_dir)));
                 if (!c->fast[l]) want = std::min(nd, 16);
             }
             const size_t budget = freeb / 3;
@@ -331,7 +340,7 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
         memset(&L, 0, sizeof(L));
         L.P = c->d_P[l]; L.acc = c->d_acc[l]; L.accC = c->d_accC[l];
         L.dirs = c->d_dirs; L.prog = c->d_prog; L.nbins = nbins; L.ncell = c->ncell; L.Ibc = c->d_Ibc;
-        L.rows = rows_for(c, l); L.mode = mode;
+        L.rows = rows_for(c, l); L.mode = mode; L.stages = c->stages;
         L.Nb = (l == 0) ? c->nx : c->ny;
         // batches never mix dominant axes (Nc differs between y- and z-dominant directions)
         int i = 0;

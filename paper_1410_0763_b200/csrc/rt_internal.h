@@ -52,6 +52,7 @@ struct SweepLaunch {
     int mode;
     int variant;             // generic kernel: 0 = four groups (one launch per group), 1 = atomics
     int group;               // generic kernel: group id 0..3
+    int stages;              // owned kernel: 0 = inputs via registers; 2..4 = depth of the TMA shared-memory ring
 };
 
 // launchers (rt_kernels.cu); all return cudaError_t of the launch
@@ -60,6 +61,8 @@ cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, SlabProg *prog,
 cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat, float2 *PT,
                                int nx, int ny, int nz, int nbins, cudaStream_t st);
 bool owned_supported(int Nb, int Nc, int rows);
+int owned_ctas_per_sm(int Nb, int rows, int stages);
+constexpr int kOwnedWarpsPerCta = 4;
 cudaError_t launch_sweep_owned(const SweepLaunch &L, cudaStream_t st);
 cudaError_t launch_sweep_generic(const SweepLaunch &L, int max_lattice_b, int max_lattice_c, cudaStream_t st);
 cudaError_t launch_normalise(float *J, const float2 *Pnat, const float *accN, const float *accNC, int slotsN,

@@ -182,8 +182,6 @@ __device__ __forceinline__ void unpack<1>(const float2 &v, float (&kap)[1], floa
 
 constexpr int kWarpsPerCta = 4;
 
-__device__ __forceinline__ float  vfma(float part0, float w, float o)  { return fmaf(part0, w, o); }
-
 template <int CW>
 __device__ __forceinline__ typename VecT<CW>::A acc_new(const typename VecT<CW>::A &o, const float (&part)[CW], float w);
 template <>
@@ -202,14 +200,12 @@ constexpr int kPatBC   = F_SB1 | F_P1 | F_SC2 | F_P2;
 constexpr int kPatCB   = F_SC1 | F_P1 | F_SB2 | F_P2;
 constexpr int kPatD    = F_SB1 | F_SC1 | F_P1;
 
-// One slab for the R rays rows of a warp.  rowd[r] = packed data of memory row (lbase + r) of this
-// slab (r = R: the seam row, valid only if some piece steps along c); acco / accCo = old
-// accumulator values of the rows this warp owns / of the seam row.
-template <int CW, int G, int R, int MODE, int FLC>
-__device__ __forceinline__ void slab_rows(const unsigned fl_rt, float (&I)[R][G][CW],
-                                          const typename VecT<CW>::D (&rowd)[R + 1][G],
-                                          const typename VecT<CW>::A (&acco)[R][G],
-                                          const typename VecT<CW>::A (&accCo)[G],
+// One slab for the R rays rows of a warp.  `src` supplies the slab's inputs: data(r, g) = packed
+// (kappa, S) of chunk g of memory row (lbase + r) (r = R: the seam row, valid only if some piece
+// steps along c), acc(r, g) / accC(g) = old accumulator values of the rows this warp owns / of
+// the seam row.  New accumulator values go straight to global memory (one writer per cell).
+template <int CW, int G, int R, int MODE, int FLC, class Src>
+__device__ __forceinline__ void slab_rows(const unsigned fl_rt, float (&I)[R][G][CW], const Src &src,
                                           const float len0, const float len1, const float len2,
                                           const float Ibc, const float invL, const int lane, const bool rev,
                                           const int lbase, const int Nc,
@@ -243,8 +239,12 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, float (&I)[R][G]
 #pragma unroll
         for (int g = 0; g < G; ++g) {
             float kc[CW], sc[CW], kn[CW], sn[CW];
-            unpack<CW>(rowd[r][g], kc, sc);
-            unpack<CW>(rowd[r + 1][g], kn, sn);
+            unpack<CW>(src.data(r, g), kc, sc);
+            if (anySC) unpack<CW>(src.data(r + 1, g), kn, sn);
+            else { 
+#pragma unroll
+                for (int i = 0; i < CW; ++i) { kn[i] = kc[i]; sn[i] = sc[i]; }
+            }
             float (&Iu)[CW] = I[r][g];
 #pragma unroll
             for (int i = 0; i < CW; ++i) seg_update<MODE>(Iu[i], kc[i], sc[i], len0, ct0, part_cur[g][i]);
@@ -292,7 +292,7 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, float (&I)[R][G]
         // row r's partial is complete (own pieces + pieces of ray row r-1 that stepped along c)
 #pragma unroll
         for (int g = 0; g < G; ++g)
-            *reinterpret_cast<AV *>(acc + orow[r] + col[g]) = acc_new<CW>(acco[r][g], part_cur[g], invL);
+            *reinterpret_cast<AV *>(acc + orow[r] + col[g]) = acc_new<CW>(src.acc(r, g), part_cur[g], invL);
 #pragma unroll
         for (int g = 0; g < G; ++g)
 #pragma unroll
@@ -302,9 +302,35 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, float (&I)[R][G]
         // seam: the partial of the memory row above the warp's last ray row has another owner
 #pragma unroll
         for (int g = 0; g < G; ++g)
-            *reinterpret_cast<AV *>(accC + orow[R] + col[g]) = acc_new<CW>(accCo[g], part_cur[g], invL);
+            *reinterpret_cast<AV *>(accC + orow[R] + col[g]) = acc_new<CW>(src.accC(g), part_cur[g], invL);
     }
 }
+
+#define RT_DISPATCH_SLAB(fl, ...)                                                         \
+    switch (fl) {                                                                         \
+    case kPatNone: slab_rows<CW, G, R, MODE, kPatNone>(__VA_ARGS__); break;               \
+    case kPatB:    slab_rows<CW, G, R, MODE, kPatB>(__VA_ARGS__); break;                  \
+    case kPatC:    slab_rows<CW, G, R, MODE, kPatC>(__VA_ARGS__); break;                  \
+    case kPatBC:   slab_rows<CW, G, R, MODE, kPatBC>(__VA_ARGS__); break;                 \
+    case kPatCB:   slab_rows<CW, G, R, MODE, kPatCB>(__VA_ARGS__); break;                 \
+    case kPatD:    slab_rows<CW, G, R, MODE, kPatD>(__VA_ARGS__); break;                  \
+    default:       slab_rows<CW, G, R, MODE, -1>(__VA_ARGS__); break;                     \
+    }
+
+// row shift of slab k in closed form: floor(1/2 + k m_c), m_c in units of 2^-20
+__device__ __forceinline__ int row_shift(int k, int Mc) { return (int)(((kOne >> 1) + (long long)k * Mc) >> kF); }
+
+// ---- variant A: inputs loaded straight into registers at the top of each slab ----------------------
+template <int CW, int G, int R>
+struct RegSrc {
+    using DV = typename VecT<CW>::D;
+    using AV = typename VecT<CW>::A;
+    DV rowd[R + 1][G];
+    AV acco[R][G], accCo[G];
+    __device__ __forceinline__ const DV &data(int r, int g) const { return rowd[r][g]; }
+    __device__ __forceinline__ const AV &acc(int r, int g) const { return acco[r][g]; }
+    __device__ __forceinline__ const AV &accC(int g) const { return accCo[g]; }
+};
 
 template <int CW, int G, int R, int MODE>
 __global__ void __launch_bounds__(32 * kWarpsPerCta)
@@ -316,7 +342,7 @@ k_sweep_owned(const SweepLaunch L)
     const int lane = threadIdx.x & 31;
     const int slot = blockIdx.y, bin = blockIdx.z;
     const DirDev *__restrict__ Dp = L.dirs + L.batch[slot];
-    const int Nc = Dp->Nc, Na = Dp->Na;
+    const int Nc = Dp->Nc, Na = Dp->Na, Mc = Dp->Mc;
     const int q0 = (blockIdx.x * kWarpsPerCta + (threadIdx.x >> 5)) * R;
     if (q0 >= Nc) return;
     const long long sk = Dp->sk, sl = Dp->sl;
@@ -344,76 +370,268 @@ k_sweep_owned(const SweepLaunch L)
 #pragma unroll
             for (int i = 0; i < CW; ++i) I[r][g][i] = Ibc;
 
-    // inputs of the current slab, loaded one slab ahead (software prefetch in registers)
-    DV rowd[R + 1][G];
-    AV acco[R][G], accCo[G];
+    RegSrc<CW, G, R> src;
     long long orow[R + 1];
-    int lbase = q0;                       // memory row (canonical l) of ray row 0 in the current slab
     SlabProg pr = prog[0];
 
-    auto issue_loads = [&](int k, int lb, bool withSeam) {
+    for (int k = 0; k < Na; ++k) {
+        const unsigned fl = pr.flags;
+        const float len0 = pr.len0, len1 = pr.len1, len2 = pr.len2;
+        if (k + 1 < Na) pr = prog[k + 1];
+        const int lbase = (q0 + row_shift(k, Mc)) % Nc;
         const long long offk = (long long)k * sk;
 #pragma unroll
         for (int r = 0; r <= R; ++r) {
-            int l = lb + r; if (l >= Nc) l -= Nc;
+            int l = lbase + r; if (l >= Nc) l -= Nc;
             orow[r] = offk + (long long)l * sl;
         }
 #pragma unroll
         for (int r = 0; r < R; ++r)
 #pragma unroll
             for (int g = 0; g < G; ++g) {
-                rowd[r][g] = *reinterpret_cast<const DV *>(P + orow[r] + col[g]);
-                acco[r][g] = *reinterpret_cast<const AV *>(acc + orow[r] + col[g]);
+                src.rowd[r][g] = *reinterpret_cast<const DV *>(P + orow[r] + col[g]);
+                src.acco[r][g] = *reinterpret_cast<const AV *>(acc + orow[r] + col[g]);
             }
-        if (withSeam) {
+        if (fl & (F_SC1 | F_SC2)) {
 #pragma unroll
             for (int g = 0; g < G; ++g) {
-                rowd[R][g] = *reinterpret_cast<const DV *>(P + orow[R] + col[g]);
-                accCo[g] = *reinterpret_cast<const AV *>(accC + orow[R] + col[g]);
+                src.rowd[R][g] = *reinterpret_cast<const DV *>(P + orow[R] + col[g]);
+                src.accCo[g] = *reinterpret_cast<const AV *>(accC + orow[R] + col[g]);
             }
         }
-    };
-    issue_loads(0, lbase, (pr.flags & (F_SC1 | F_SC2)) != 0);
+        RT_DISPATCH_SLAB(fl, fl, I, src, len0, len1, len2, Ibc, invL, lane, rev, lbase, Nc, acc, accC, orow, col)
+    }
+}
 
+// ---- variant B: inputs staged in a warp-private shared-memory ring by the TMA engine ---------------
+// Each warp owns D stages; stage (k mod D) holds slab k's packed field rows and old accumulator
+// rows, copied by 1-D bulk async copies (cp.async.bulk, SASS UBLKCP) issued by lane 0 D slabs ahead
+// and tracked by one mbarrier per stage (transaction-byte count).  No registers are spent on data in
+// flight, so the prefetch depth is set by shared memory, not by the register file.
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
+{ asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
+{ asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory"); }
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@!p bra WAIT_%=;\n\t}"
+        :: "r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+template <int CW, int G, int R>
+struct SmemSrc {
+    using DV = typename VecT<CW>::D;
+    using AV = typename VecT<CW>::A;
+    static constexpr int kNb = 32 * CW * G;
+    static constexpr int kRowP = kNb * (int)sizeof(float2);
+    static constexpr int kRowA = kNb * (int)sizeof(float);
+    static constexpr int kStage = (R + 1) * (kRowP + kRowA);
+    const unsigned char *stage;      // generic pointer to the stage in shared memory
+    int colb;                        // byte offset of this lane's chunk 0 within a float2 row (fwd) ...
+    int cstep;                       // ... and signed chunk stride in float2 elements
+    int col0;                        // first column of chunk 0
+    __device__ __forceinline__ DV data(int r, int g) const
+    { return *reinterpret_cast<const DV *>(stage + r * kRowP + (col0 + g * cstep) * (int)sizeof(float2)); }
+    __device__ __forceinline__ AV acc(int r, int g) const
+    { return *reinterpret_cast<const AV *>(stage + (R + 1) * kRowP + r * kRowA + (col0 + g * cstep) * (int)sizeof(float)); }
+    __device__ __forceinline__ AV accC(int g) const { return acc(R, g); }
+};
+
+template <int CW, int G, int R, int MODE, int D>
+__global__ void __launch_bounds__(32 * kWarpsPerCta)
+k_sweep_tma(const SweepLaunch L)
+{
+    using Src = SmemSrc<CW, G, R>;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int kWarpBytes = D * Src::kStage + 128;
+
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int slot = blockIdx.y, bin = blockIdx.z;
+    const DirDev *__restrict__ Dp = L.dirs + L.batch[slot];
+    const int Nc = Dp->Nc, Na = Dp->Na, Mc = Dp->Mc;
+    const int q0 = (blockIdx.x * kWarpsPerCta + wid) * R;
+    if (q0 >= Nc) return;
+    const long long sk = Dp->sk, sl = Dp->sl;
+    const bool rev = Dp->sj < 0;
+    const float invL = (MODE == MODE_J) ? Dp->invL : 1.0f;
+    const float Ibc = L.Ibc[bin];
+    const SlabProg *__restrict__ prog = L.prog + Dp->prog_off;
+
+    const long long foff = (long long)bin * L.ncell + Dp->base;
+    const float2 *__restrict__ P = L.P + foff;
+    float *__restrict__ acc = L.acc + ((long long)slot * L.nbins) * L.ncell + foff;
+    float *__restrict__ accC = L.accC + ((long long)slot * L.nbins) * L.ncell + foff;
+
+    unsigned char *wbase = smem_raw + wid * kWarpBytes;
+    const unsigned wbase_s = smem_u32(wbase);
+    const unsigned bars = wbase_s + D * Src::kStage;
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < D; ++s) mbar_init(bars + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+
+    int col[G];
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+        col[g] = rev ? (32 * CW * G - CW * (32 * g + lane + 1)) : CW * (32 * g + lane);
+
+    // producer: lane 0 asks the TMA engine for slab kk's rows
+    auto produce = [&](int kk) {
+        if (lane != 0) return;
+        const int s = kk % D;
+        const unsigned st = wbase_s + s * Src::kStage, bar = bars + 8 * s;
+        const int s0 = row_shift(kk, Mc), s1 = row_shift(kk + 1, Mc);
+        const bool seam = (s1 != s0);
+        const int lb = (q0 + s0) % Nc;
+        const long long offk = (long long)kk * sk;
+        const int nrows = R + (seam ? 1 : 0);
+        mbar_expect_tx(bar, (unsigned)(nrows * ((MODE == MODE_J ? Src::kRowP : 0) + Src::kRowA)));
+#pragma unroll
+        for (int r = 0; r <= R; ++r) {
+            if (r == R && !seam) break;
+            int l = lb + r; if (l >= Nc) l -= Nc;
+            const long long o = offk + (long long)l * sl;
+            if (MODE == MODE_J) bulk_g2s(st + r * Src::kRowP, P + o, Src::kRowP, bar);
+            bulk_g2s(st + (R + 1) * Src::kRowP + r * Src::kRowA, (r < R ? acc : accC) + o, Src::kRowA, bar);
+        }
+    };
+#pragma unroll 1
+    for (int kk = 0; kk < D && kk < Na; ++kk) produce(kk);
+
+    float I[R][G][CW];
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int i = 0; i < CW; ++i) I[r][g][i] = Ibc;
+
+    Src src;
+    src.col0 = col[0];
+    src.cstep = rev ? -32 * CW : 32 * CW;
+    src.colb = 0;
+    long long orow[R + 1];
+    SlabProg pr = prog[0];
+
+#pragma unroll 1
     for (int k = 0; k < Na; ++k) {
         const unsigned fl = pr.flags;
         const float len0 = pr.len0, len1 = pr.len1, len2 = pr.len2;
         if (k + 1 < Na) pr = prog[k + 1];
-#define RT_BODY(FLC) slab_rows<CW, G, R, MODE, FLC>(fl, I, rowd, acco, accCo, len0, len1, len2, Ibc, invL, lane, rev, \
-                                                    lbase, Nc, acc, accC, orow, col)
-        switch (fl) {
-        case kPatNone: RT_BODY(kPatNone); break;
-        case kPatB:    RT_BODY(kPatB); break;
-        case kPatC:    RT_BODY(kPatC); break;
-        case kPatBC:   RT_BODY(kPatBC); break;
-        case kPatCB:   RT_BODY(kPatCB); break;
-        case kPatD:    RT_BODY(kPatD); break;
-        default:       RT_BODY(-1); break;
+        const int lbase = (q0 + row_shift(k, Mc)) % Nc;
+        const long long offk = (long long)k * sk;
+#pragma unroll
+        for (int r = 0; r <= R; ++r) {
+            int l = lbase + r; if (l >= Nc) l -= Nc;
+            orow[r] = offk + (long long)l * sl;
         }
-#undef RT_BODY
-        if (fl & (F_SC1 | F_SC2)) { lbase += 1; if (lbase >= Nc) lbase -= Nc; }
-        if (k + 1 < Na) issue_loads(k + 1, lbase, (pr.flags & (F_SC1 | F_SC2)) != 0);
+        const int s = k % D;
+        src.stage = wbase + s * Src::kStage;
+        mbar_wait(bars + 8 * s, (unsigned)((k / D) & 1));
+        RT_DISPATCH_SLAB(fl, fl, I, src, len0, len1, len2, Ibc, invL, lane, rev, lbase, Nc, acc, accC, orow, col)
+        __syncwarp();                     // every lane is done reading stage s
+        if (k + D < Na) produce(k + D);
     }
 }
 
 bool owned_supported(int Nb, int Nc, int rows)
 {
     if (!(Nb == 32 || Nb == 64 || Nb == 128 || Nb == 256)) return false;
-    if (!(rows == 1 || rows == 2 || rows == 4 || rows == 8)) return false;
+    if (!(rows == 1 || rows == 2 || rows == 4)) return false;
     return Nc % rows == 0;
+}
+
+template <int CW, int G, int R, int MODE>
+static cudaError_t launch_owned_one(const SweepLaunch &L, cudaStream_t st)
+{
+    const int tiles = L.Nc / R;
+    dim3 grid((tiles + kWarpsPerCta - 1) / kWarpsPerCta, L.nslots, L.nbins), block(32 * kWarpsPerCta);
+    if (L.stages >= 2) {
+        using Src = SmemSrc<CW, G, R>;
+        auto go = [&](auto kern, int D) -> cudaError_t {
+            const int smem = kWarpsPerCta * (D * Src::kStage + 128);
+            if (smem > 227 * 1024) return cudaErrorInvalidValue;
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            if (e != cudaSuccess) return e;
+            kern<<<grid, block, smem, st>>>(L);
+            return cudaGetLastError();
+        };
+        switch (L.stages) {
+        case 2: return go(k_sweep_tma<CW, G, R, MODE, 2>, 2);
+        case 3: return go(k_sweep_tma<CW, G, R, MODE, 3>, 3);
+        default: return go(k_sweep_tma<CW, G, R, MODE, 4>, 4);
+        }
+    }
+    k_sweep_owned<CW, G, R, MODE><<<grid, block, 0, st>>>(L);
+    return cudaGetLastError();
+}
+
+template <int CW, int G, int R>
+static int owned_ctas_per_sm_impl(int stages)
+{
+    int n = 0;
+    cudaError_t e;
+    if (stages >= 2) {
+        using Src = SmemSrc<CW, G, R>;
+        const int D = stages > 4 ? 4 : stages;
+        const int smem = kWarpsPerCta * (D * Src::kStage + 128);
+        if (smem > 227 * 1024) return 0;
+        auto q = [&](auto kern) {
+            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, 32 * kWarpsPerCta, smem);
+        };
+        if (D == 2) e = q(k_sweep_tma<CW, G, R, MODE_J, 2>);
+        else if (D == 3) e = q(k_sweep_tma<CW, G, R, MODE_J, 3>);
+        else e = q(k_sweep_tma<CW, G, R, MODE_J, 4>);
+    } else {
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_sweep_owned<CW, G, R, MODE_J>, 32 * kWarpsPerCta, 0);
+    }
+    return e == cudaSuccess ? n : 0;
+}
+
+template <int CW, int G>
+static int owned_ctas_per_sm_rows(int rows, int stages)
+{
+    switch (rows) {
+    case 1: return owned_ctas_per_sm_impl<CW, G, 1>(stages);
+    case 2: return owned_ctas_per_sm_impl<CW, G, 2>(stages);
+    case 4: return owned_ctas_per_sm_impl<CW, G, 4>(stages);
+    }
+    return 0;
+}
+
+// resident CTAs (of kWarpsPerCta warps) per SM of the J-mode owned kernel; 0 if the configuration cannot launch
+int owned_ctas_per_sm(int Nb, int rows, int stages)
+{
+    switch (Nb) {
+    case 32:  return owned_ctas_per_sm_rows<1, 1>(rows, stages);
+    case 64:  return owned_ctas_per_sm_rows<2, 1>(rows, stages);
+    case 128: return owned_ctas_per_sm_rows<2, 2>(rows, stages);
+    case 256: return owned_ctas_per_sm_rows<2, 4>(rows, stages);
+    }
+    return 0;
 }
 
 template <int CW, int G, int R>
 static cudaError_t launch_owned_mode(const SweepLaunch &L, cudaStream_t st)
 {
-    const int tiles = L.Nc / R;
-    dim3 grid((tiles + kWarpsPerCta - 1) / kWarpsPerCta, L.nslots, L.nbins), block(32 * kWarpsPerCta);
     switch (L.mode) {
-    case MODE_J:     k_sweep_owned<CW, G, R, MODE_J><<<grid, block, 0, st>>>(L); break;
-    case MODE_COUNT: k_sweep_owned<CW, G, R, MODE_COUNT><<<grid, block, 0, st>>>(L); break;
-    default:         k_sweep_owned<CW, G, R, MODE_DS><<<grid, block, 0, st>>>(L); break;
+    case MODE_J:     return launch_owned_one<CW, G, R, MODE_J>(L, st);
+    case MODE_COUNT: return launch_owned_one<CW, G, R, MODE_COUNT>(L, st);
+    default:         return launch_owned_one<CW, G, R, MODE_DS>(L, st);
     }
-    return cudaGetLastError();
 }
 
 template <int CW, int G>
@@ -423,7 +641,6 @@ static cudaError_t launch_owned_rows(const SweepLaunch &L, cudaStream_t st)
     case 1: return launch_owned_mode<CW, G, 1>(L, st);
     case 2: return launch_owned_mode<CW, G, 2>(L, st);
     case 4: return launch_owned_mode<CW, G, 4>(L, st);
-    case 8: return launch_owned_mode<CW, G, 8>(L, st);
     }
     return cudaErrorInvalidValue;
 }
