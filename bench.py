@@ -27,6 +27,9 @@ if ROOT not in sys.path:
 METRIC = "ray_segment_updates_per_sec"
 UNIT = "updates/s"
 ALGO_BYTES_PER_CELL_DIR_BIN = 16.0     # read kappa,S (8 B) + read-modify-write J accumulator (8 B), SURVEY 8(d)
+# dram__bytes_read.sum + dram__bytes_write.sum per cell-direction-bin of the hot kernel, from the ncu --set full
+# capture named beside it (profiles/); multiplied by the cell-direction-bins of one launch to give `traffic`.
+NCU_DRAM_BYTES_PER_CELL_DIR_BIN = {"C4": (2.77e9 / (13 * 256 ** 3), "profiles/r1a_sweep_tma_full_c4.md")}
 
 
 def measured_peaks():
@@ -238,8 +241,12 @@ def main():
     avg_launch_ms = kernel_ms[0] / n_sweep_launches
     bytes_per_launch = ALGO_BYTES_PER_CELL_DIR_BIN * cell_dir_bins / n_sweep_launches
     achieved = bytes_per_launch / (avg_launch_ms * 1e-3) / 1e9
+    traffic, traffic_src = None, None
+    if args.config in NCU_DRAM_BYTES_PER_CELL_DIR_BIN and args.flags == 0:
+        per, traffic_src = NCU_DRAM_BYTES_PER_CELL_DIR_BIN[args.config]
+        traffic = per * cell_dir_bins / n_sweep_launches
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_kind": peak_kind, "kernel": "k_sweep_owned",
+                "traffic": traffic, "traffic_source": traffic_src, "peak_kind": peak_kind, "kernel": "k_sweep_tma",
                 "launches_per_step": n_sweep_launches, "avg_launch_ms": avg_launch_ms,
                 "algorithmic_bytes_per_launch": bytes_per_launch,
                 "kernel_share_of_step": kernel_ms[0] / (ms / args.steps)}
