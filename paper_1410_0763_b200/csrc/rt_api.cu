@@ -8,7 +8,9 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <map>
 #include <new>
+#include <tuple>
 #include <string>
 #include <vector>
 
@@ -41,7 +43,13 @@ struct rt_ctx {
     int device = 0;
     int sm_count = 148;
     std::vector<HostDir> hd;
-    std::vector<int> order[2];       // direction indices per layout, sorted by work (descending)
+    std::vector<int> order[2];       // direction indices per layout, sorted by (dominant axis, march sense, work)
+    // J sweep: directions that differ only by the sign of their b component are carried by one warp
+    // ("mirror pairs", rt_kernels.cu); pairs[l] holds the member with a non-negative b component,
+    // singles[l] everything that has no partner (zero b slope, or an unsymmetric user set)
+    std::vector<int> pairs[2], singles[2];
+    bool pair_enable = true;
+    int slots_pair[2] = {0, 0}, slots_single[2] = {0, 0};
     bool fast[2] = {false, false};   // owned kernel usable for the layout
     int rows = 2;
     int stages = 2;                  // depth of the owned kernel's TMA shared-memory ring (0 = register path)
@@ -56,7 +64,7 @@ struct rt_ctx {
     float2 *d_P[2] = {nullptr, nullptr};
     float *d_acc[2] = {nullptr, nullptr};
     float *d_accC[2] = {nullptr, nullptr};
-    int *d_batch = nullptr;          // [ndirs] direction index per (launch, slot), launch-major
+    int *d_batch = nullptr;          // [2*ndirs]: order[0], order[1], then pairs[0], singles[0], pairs[1], singles[1]
     float *d_Ibc = nullptr;
     double *d_red = nullptr;         // [3] reduction scratch
     unsigned long long *d_u64 = nullptr;
@@ -191,12 +199,40 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
         c->np_max[h.layout] = std::max(c->np_max[h.layout], np);
         c->nq_max[h.layout] = std::max(c->nq_max[h.layout], nq);
     }
-    // homogeneous batches: similar work per direction in one launch; same dominant axis adjacent
-    for (int l = 0; l < 2; ++l)
-        std::stable_sort(c->order[l].begin(), c->order[l].end(), [&](int x, int y) {
-            if (c->hd[x].a != c->hd[y].a) return c->hd[x].a < c->hd[y].a;
-            return c->hd[x].work > c->hd[y].work;
-        });
+    // homogeneous batches: the directions of one launch share the dominant axis and the sense of the
+    // march along it, so that concurrently resident CTAs read the same field slab at about the same
+    // time (the second reader finds it in L2), and have similar work per slab
+    auto by_class = [&](int x, int y) {
+        if (c->hd[x].a != c->hd[y].a) return c->hd[x].a < c->hd[y].a;
+        if (c->hd[x].refl[c->hd[x].a] != c->hd[y].refl[c->hd[y].a]) return c->hd[x].refl[c->hd[x].a] < c->hd[y].refl[c->hd[y].a];
+        return c->hd[x].work > c->hd[y].work;
+    };
+    for (int l = 0; l < 2; ++l) std::stable_sort(c->order[l].begin(), c->order[l].end(), by_class);
+    // mirror pairs: same dominant axis, same reflections of a and c, same quantised slopes, opposite b
+    {
+        typedef std::tuple<int, int, int, long long, long long> Key;
+        std::map<Key, std::vector<int>> pos, neg;
+        for (int i = 0; i < ndirs; ++i) {
+            const HostDir &h = c->hd[i];
+            if (h.Mb == 0) continue;
+            Key k(h.a, h.refl[h.a], h.refl[h.c], h.Mb, h.Mc);
+            (h.refl[h.b] ? neg : pos)[k].push_back(i);
+        }
+        std::vector<char> paired(ndirs, 0);
+        for (auto &kv : pos) {
+            auto it = neg.find(kv.first);
+            if (it == neg.end()) continue;
+            const size_t n = std::min(kv.second.size(), it->second.size());
+            for (size_t j = 0; j < n; ++j) {
+                paired[kv.second[j]] = 1; paired[it->second[j]] = 2;
+            }
+        }
+        for (int l = 0; l < 2; ++l)
+            for (int i : c->order[l]) {
+                if (paired[i] == 1) c->pairs[l].push_back(i);
+                else if (paired[i] == 0) c->singles[l].push_back(i);
+            }
+    }
     // owned kernel: the memory-contiguous transverse extent must be 32/64/128/256 (one warp owns full rows)
     const int NbL[2] = {nx, ny};
     for (int l = 0; l < 2; ++l) c->fast[l] = (flags == RT_OWNED) && (NbL[l] == 32 || NbL[l] == 64 || NbL[l] == 128 || NbL[l] == 256);
@@ -205,7 +241,7 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     CKC(cudaMalloc(&c->d_dirs, sizeof(DirDev) * ndirs));
     CKC(cudaMalloc(&c->d_L, sizeof(double) * ndirs));
     CKC(cudaMalloc(&c->d_prog, sizeof(SlabProg) * prog_total));
-    CKC(cudaMalloc(&c->d_batch, sizeof(int) * ndirs));
+    CKC(cudaMalloc(&c->d_batch, sizeof(int) * 2 * ndirs));
     CKC(cudaMalloc(&c->d_Ibc, sizeof(float) * nbins));
     CKC(cudaMalloc(&c->d_red, sizeof(double) * 3));
     CKC(cudaMalloc(&c->d_u64, sizeof(unsigned long long)));
@@ -215,7 +251,11 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     {
         std::vector<int> batch;
         for (int l = 0; l < 2; ++l) batch.insert(batch.end(), c->order[l].begin(), c->order[l].end());
-        CKC(cudaMemcpy(c->d_batch, batch.data(), sizeof(int) * ndirs, cudaMemcpyHostToDevice));
+        for (int l = 0; l < 2; ++l) {
+            batch.insert(batch.end(), c->pairs[l].begin(), c->pairs[l].end());
+            batch.insert(batch.end(), c->singles[l].begin(), c->singles[l].end());
+        }
+        CKC(cudaMemcpy(c->d_batch, batch.data(), sizeof(int) * batch.size(), cudaMemcpyHostToDevice));
     }
     CKC(launch_build_programs(c->d_dirs, ndirs, c->d_prog, cell_width, c->d_L, 0));
     CKC(cudaEventCreate(&c->ev0));
@@ -232,6 +272,7 @@ extern "C" int rt_tune(rt_ctx *c, const char *key, int value)
     if (c->buffers_ready) return RT_ESTATE;
     if (!strcmp(key, "slots")) { if (value < 1 || value > 4096) return RT_EINVAL; c->slots_req = value; return RT_OK; }
     if (!strcmp(key, "stages")) { if (!(value == 0 || (value >= 2 && value <= 4))) return RT_EINVAL; c->stages = value; return RT_OK; }
+    if (!strcmp(key, "pair")) { if (value != 0 && value != 1) return RT_EINVAL; c->pair_enable = value != 0; return RT_OK; }
     if (!strcmp(key, "rows")) { if (!(value == 1 || value == 2 || value == 4)) return RT_EINVAL; c->rows = value; return RT_OK; }
     return RT_EINVAL;
 }
@@ -265,10 +306,15 @@ static int ensure_buffers(rt_ctx *c)
                 for (int i : c->order[l]) Nc = std::min(Nc, c->hd[i].Nc);
                 const int rows = rows_for(c, l);
                 const int ctas_dir = ((Nc / rows + kOwnedWarpsPerCta - 1) / kOwnedWarpsPerCta) * c->nbins;
-                int per_sm = c->fast[l] ? owned_ctas_per_sm(l == 0 ? c->nx : c->ny, rows, c->stages) : 0;
-                if (per_sm < 1) per_sm = 4;
-                const int resident = per_sm * c->sm_count;
-                want = std::max(1, std::min(nd, resident / std::max(1, ctas_dir)));
+                auto wave = [&](bool pair) {
+                    int per_sm = c->fast[l] ? owned_ctas_per_sm(l == 0 ? c->nx : c->ny, rows, c->stages, pair) : 0;
+                    if (per_sm < 1) per_sm = 4;
+                    const int resident = per_sm * c->sm_count;
+                    return std::max(1, std::min(nd, resident / std::max(1, ctas_dir)));
+                };
+                c->slots_single[l] = wave(false);
+                c->slots_pair[l] = (c->fast[l] && c->stages >= 2) ? wave(true) : 0;
+                want = std::max(c->slots_single[l], c->slots_pair[l]);
                 if (!c->fast[l]) want = std::min(nd, 16);
             }
             const size_t budget = freeb / 3;
@@ -278,6 +324,8 @@ static int ensure_buffers(rt_ctx *c)
             want = (int)std::min<size_t>((size_t)want, maxs);
         }
         c->slots[l] = want;
+        c->slots_single[l] = (c->slots_req > 0 || !c->fast[l]) ? want : std::min(want, c->slots_single[l]);
+        c->slots_pair[l] = (c->slots_req > 0) ? want : std::min(want, c->slots_pair[l]);
     }
     for (int l = 0; l < 2; ++l) {
         {   // both packed copies are always kept (the pack kernel writes both in one pass)
@@ -319,7 +367,6 @@ extern "C" int rt_set_inflow(rt_ctx *c, const float *I_bc_host)
 static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStream_t st, int *launches, int used[2])
 {
     const size_t acc_bytes = sizeof(float) * (size_t)c->ncell * nbins;
-    int offset = 0;       // position of the layout's first direction in d_batch
     used[0] = used[1] = 0;
     for (int l = 0; l < 2; ++l) {
         if (c->order[l].empty() || (only_dir >= 0 && c->hd[only_dir].layout != l)) continue;
@@ -328,50 +375,70 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
         CK(cudaMemsetAsync(c->d_accC[l], 0, acc_bytes * S, st));
     }
     if (mode == MODE_J) CK(cudaEventRecord(c->ev0, st));
+    int off_all = 0;                 // position of the layout's list in d_batch: order[] region ...
+    int off_j = c->ndirs;            // ... and pairs[]/singles[] region
     for (int l = 0; l < 2; ++l) {
         const int nd = (int)c->order[l].size();
-        const int off_l = offset;
-        offset += nd;
+        const int my_all = off_all, my_j = off_j;
+        off_all += nd;
+        off_j += (int)(c->pairs[l].size() + c->singles[l].size());
         if (nd == 0) continue;
         if (only_dir >= 0 && c->hd[only_dir].layout != l) continue;
-        const int S = (only_dir >= 0) ? 1 : c->slots[l];
-        used[l] = S;
         SweepLaunch L;
         memset(&L, 0, sizeof(L));
         L.P = c->d_P[l]; L.acc = c->d_acc[l]; L.accC = c->d_accC[l];
         L.dirs = c->d_dirs; L.prog = c->d_prog; L.nbins = nbins; L.ncell = c->ncell; L.Ibc = c->d_Ibc;
         L.rows = rows_for(c, l); L.mode = mode; L.stages = c->stages;
         L.Nb = (l == 0) ? c->nx : c->ny;
-        // batches never mix dominant axes (Nc differs between y- and z-dominant directions)
-        int i = 0;
-        while (i < nd) {
-            const int a = c->hd[c->order[l][i]].a;
-            int n = 0;
-            while (i + n < nd && n < S && c->hd[c->order[l][i + n]].a == a) ++n;
-            int first = i, count = n;
-            if (only_dir >= 0) {
-                if (c->order[l][i] != only_dir) { i += 1; continue; }
-                count = 1;
-            }
-            L.batch = c->d_batch + off_l + first;
-            L.nslots = count;
-            L.Nc = c->hd[c->order[l][first]].Nc;
-            if (c->fast[l] && owned_supported(L.Nb, L.Nc, L.rows)) {
-                CK(launch_sweep_owned(L, st));
-                ++*launches;
-            } else if (c->flags == RT_ATOMIC_ABLATION) {
-                L.variant = 1;
-                CK(launch_sweep_generic(L, c->np_max[l], c->nq_max[l], st));
-                ++*launches;
-            } else {
-                L.variant = 0;
-                for (int g = 0; g < 4; ++g) {
-                    L.group = g;
+        const bool owned_l = c->fast[l];
+        // the lists this traversal walks: (direction list, position in d_batch, slots per launch, paired)
+        struct Pass { const std::vector<int> *list; int off; int S; int pair; };
+        Pass passes[2];
+        int npass = 0;
+        const bool use_pairs = (mode == MODE_J) && only_dir < 0 && c->pair_enable && owned_l && c->stages >= 2 &&
+                               !c->pairs[l].empty();
+        if (use_pairs) {
+            passes[npass++] = Pass{&c->pairs[l], my_j, c->slots_pair[l], 1};
+            passes[npass++] = Pass{&c->singles[l], my_j + (int)c->pairs[l].size(), c->slots_single[l], 0};
+        } else {
+            passes[npass++] = Pass{&c->order[l], my_all, (only_dir >= 0) ? 1 : c->slots_single[l], 0};
+        }
+        for (int ps = 0; ps < npass; ++ps) {
+            const std::vector<int> &list = *passes[ps].list;
+            const int nl = (int)list.size(), S = std::max(1, passes[ps].S);
+            L.pair = passes[ps].pair;
+            // batches never mix dominant axes (Nc differs between y- and z-dominant directions)
+            int i = 0;
+            while (i < nl) {
+                const int a = c->hd[list[i]].a;
+                int n = 0;
+                while (i + n < nl && n < S && c->hd[list[i + n]].a == a) ++n;
+                int first = i, count = n;
+                if (only_dir >= 0) {
+                    if (list[i] != only_dir) { i += 1; continue; }
+                    count = 1;
+                }
+                used[l] = std::max(used[l], count);
+                L.batch = c->d_batch + passes[ps].off + first;
+                L.nslots = count;
+                L.Nc = c->hd[list[first]].Nc;
+                if (owned_l && owned_supported(L.Nb, L.Nc, L.rows)) {
+                    CK(launch_sweep_owned(L, st));
+                    ++*launches;
+                } else if (c->flags == RT_ATOMIC_ABLATION) {
+                    L.variant = 1;
                     CK(launch_sweep_generic(L, c->np_max[l], c->nq_max[l], st));
                     ++*launches;
+                } else {
+                    L.variant = 0;
+                    for (int g = 0; g < 4; ++g) {
+                        L.group = g;
+                        CK(launch_sweep_generic(L, c->np_max[l], c->nq_max[l], st));
+                        ++*launches;
+                    }
                 }
+                i += count;
             }
-            i += count;
         }
     }
     if (mode == MODE_J) { CK(cudaEventRecord(c->ev1, st)); c->ev_valid = true; }

@@ -53,6 +53,7 @@ struct SweepLaunch {
     int variant;             // generic kernel: 0 = four groups (one launch per group), 1 = atomics
     int group;               // generic kernel: group id 0..3
     int stages;              // owned kernel: 0 = inputs via registers; 2..4 = depth of the TMA shared-memory ring
+    int pair;                // owned TMA kernel, MODE_J: every slot carries a direction and its b-mirror (rt_kernels.cu "mirror pairs")
 };
 
 // launchers (rt_kernels.cu); all return cudaError_t of the launch
@@ -61,7 +62,7 @@ cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, SlabProg *prog,
 cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat, float2 *PT,
                                int nx, int ny, int nz, int nbins, cudaStream_t st);
 bool owned_supported(int Nb, int Nc, int rows);
-int owned_ctas_per_sm(int Nb, int rows, int stages);
+int owned_ctas_per_sm(int Nb, int rows, int stages, bool pair);
 constexpr int kOwnedWarpsPerCta = 4;
 cudaError_t launch_sweep_owned(const SweepLaunch &L, cudaStream_t st);
 cudaError_t launch_sweep_generic(const SweepLaunch &L, int max_lattice_b, int max_lattice_c, cudaStream_t st);

@@ -306,6 +306,153 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, float (&I)[R][G]
     }
 }
 
+// ---- mirror pairs ---------------------------------------------------------------------------------
+// Two directions that differ only by the sign of their component along the memory-contiguous
+// transverse axis b (HEALPix sets are symmetric under x -> -x and y -> -y) have the
+// same slab programs, the same row drift along c and the same dominant-axis march: at every slab a
+// warp that carries both touches the SAME cells with the SAME piece lengths.  So the packed field
+// rows and the accumulator rows are moved once for the two directions, and e = exp(-kappa ds),
+// A = 1 - e and S*A are evaluated once per (cell, piece) and applied to both intensities.  Only
+// the b-step differs: rays of direction 0 are handed to the next higher column, rays of direction
+// 1 to the next lower one.  Stage-major order (all chunks do piece 0, then the step, ...) because
+// the two directions need their chunk-to-chunk carries in opposite chunk order.
+template <int MODE>
+__device__ __forceinline__ void seg_update2(float &I0, float &I1, float kap, float src, float len, float ct, float &part)
+{
+    if (MODE == MODE_J) {
+        float e;
+        const float A = one_minus_exp(kap, len, ct, e);
+        const float SA = src * A;
+        part = fmaf(I0 + I1, A, part);
+        I0 = fmaf(I0, e, SA);                                  // eq. 7, direction 0
+        I1 = fmaf(I1, e, SA);                                  // eq. 7, mirrored direction
+    } else if (MODE == MODE_COUNT) {
+        part += 2.0f;
+    } else {
+        part += 2.0f * len;
+    }
+}
+
+template <int CW, int G, int R, int MODE, int FLC, class Src>
+__device__ __forceinline__ void slab_rows_pair(const unsigned fl_rt, float (&I)[2][R][G][CW], const Src &src,
+                                               const float len0, const float len1, const float len2,
+                                               const float Ibc, const float invL, const int lane,
+                                               const int lbase, const int Nc,
+                                               float *__restrict__ acc, float *__restrict__ accC,
+                                               const long long (&orow)[R + 1], const int (&col)[G])
+{
+    using AV = typename VecT<CW>::A;
+    constexpr unsigned FULL = 0xffffffffu;
+    constexpr float LOG2E = 1.4426950408889634f;
+    const unsigned fl = (FLC >= 0) ? (unsigned)FLC : fl_rt;
+    const float ct0 = -len0 * LOG2E, ct1 = -len1 * LOG2E, ct2 = -len2 * LOG2E;
+    const bool anySC = (fl & (F_SC1 | F_SC2)) != 0;
+
+    float part_cur[G][CW];
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int i = 0; i < CW; ++i) part_cur[g][i] = 0.0f;
+
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        int l_r = lbase + r; if (l_r >= Nc) l_r -= Nc;
+        const bool wrap_r = (l_r == Nc - 1);
+        float part_next[G][CW];
+        float kc[G][CW], sc[G][CW], kn[G][CW], sn[G][CW];
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            unpack<CW>(src.data(r, g), kc[g], sc[g]);
+            if (anySC) unpack<CW>(src.data(r + 1, g), kn[g], sn[g]);
+#pragma unroll
+            for (int i = 0; i < CW; ++i) {
+                part_next[g][i] = 0.0f;
+                if (!anySC) { kn[g][i] = kc[g][i]; sn[g][i] = sc[g][i]; }
+            }
+        }
+        float (&I0)[G][CW] = I[0][r];
+        float (&I1)[G][CW] = I[1][r];
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int i = 0; i < CW; ++i) seg_update2<MODE>(I0[g][i], I1[g][i], kc[g][i], sc[g][i], len0, ct0, part_cur[g][i]);
+        bool sel = false;
+#pragma unroll
+        for (int stage = 1; stage <= 2; ++stage) {
+            const unsigned fsb = (stage == 1) ? F_SB1 : F_SB2;
+            const unsigned fsc = (stage == 1) ? F_SC1 : F_SC2;
+            const unsigned fp = (stage == 1) ? F_P1 : F_P2;
+            const float len = (stage == 1) ? len1 : len2;
+            const float ct = (stage == 1) ? ct1 : ct2;
+            if (fl & (fsb | fsc)) {
+                if (MODE == MODE_J) {
+                    if (fl & fsb) {
+                        // direction 0: every ray to the next higher column; a new ray enters column 0
+                        float carry = Ibc;
+#pragma unroll
+                        for (int g = 0; g < G; ++g) {
+                            const float t = __shfl_sync(FULL, I0[g][CW - 1], (lane + 31) & 31);
+                            const float in = (lane == 0) ? carry : t;
+                            carry = t;
+                            if (CW == 2) I0[g][CW - 1] = I0[g][0];
+                            I0[g][0] = in;
+                        }
+                        // direction 1: every ray to the next lower column; a new ray enters the last column
+                        carry = Ibc;
+#pragma unroll
+                        for (int g = G - 1; g >= 0; --g) {
+                            const float t = __shfl_sync(FULL, I1[g][0], (lane + 1) & 31);
+                            const float in = (lane == 31) ? carry : t;
+                            carry = t;
+                            if (CW == 2) I1[g][0] = I1[g][CW - 1];
+                            I1[g][CW - 1] = in;
+                        }
+                    }
+                    if ((fl & fsc) && wrap_r) {   // step along c out of the box: new rays enter
+#pragma unroll
+                        for (int g = 0; g < G; ++g)
+#pragma unroll
+                            for (int i = 0; i < CW; ++i) { I0[g][i] = Ibc; I1[g][i] = Ibc; }
+                    }
+                }
+                if (fl & fsc) sel = true;
+            }
+            if (fl & fp) {
+#pragma unroll
+                for (int g = 0; g < G; ++g)
+#pragma unroll
+                    for (int i = 0; i < CW; ++i) {
+                        if (sel) seg_update2<MODE>(I0[g][i], I1[g][i], kn[g][i], sn[g][i], len, ct, part_next[g][i]);
+                        else     seg_update2<MODE>(I0[g][i], I1[g][i], kc[g][i], sc[g][i], len, ct, part_cur[g][i]);
+                    }
+            }
+        }
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+            *reinterpret_cast<AV *>(acc + orow[r] + col[g]) = acc_new<CW>(src.acc(r, g), part_cur[g], invL);
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int i = 0; i < CW; ++i) part_cur[g][i] = part_next[g][i];
+    }
+    if (anySC) {
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+            *reinterpret_cast<AV *>(accC + orow[R] + col[g]) = acc_new<CW>(src.accC(g), part_cur[g], invL);
+    }
+}
+
+#define RT_DISPATCH_SLAB_PAIR(fl, ...)                                                    \
+    switch (fl) {                                                                         \
+    case kPatNone: slab_rows_pair<CW, G, R, MODE, kPatNone>(__VA_ARGS__); break;          \
+    case kPatB:    slab_rows_pair<CW, G, R, MODE, kPatB>(__VA_ARGS__); break;             \
+    case kPatC:    slab_rows_pair<CW, G, R, MODE, kPatC>(__VA_ARGS__); break;             \
+    case kPatBC:   slab_rows_pair<CW, G, R, MODE, kPatBC>(__VA_ARGS__); break;            \
+    case kPatCB:   slab_rows_pair<CW, G, R, MODE, kPatCB>(__VA_ARGS__); break;            \
+    case kPatD:    slab_rows_pair<CW, G, R, MODE, kPatD>(__VA_ARGS__); break;             \
+    default:       slab_rows_pair<CW, G, R, MODE, -1>(__VA_ARGS__); break;                \
+    }
+
 #define RT_DISPATCH_SLAB(fl, ...)                                                         \
     switch (fl) {                                                                         \
     case kPatNone: slab_rows<CW, G, R, MODE, kPatNone>(__VA_ARGS__); break;               \
@@ -447,7 +594,7 @@ struct SmemSrc {
     __device__ __forceinline__ AV accC(int g) const { return acc(R, g); }
 };
 
-template <int CW, int G, int R, int MODE, int D>
+template <int CW, int G, int R, int MODE, int D, int ND>
 __global__ void __launch_bounds__(32 * kWarpsPerCta)
 k_sweep_tma(const SweepLaunch L)
 {
@@ -510,13 +657,15 @@ k_sweep_tma(const SweepLaunch L)
 #pragma unroll 1
     for (int kk = 0; kk < D && kk < Na; ++kk) produce(kk);
 
-    float I[R][G][CW];
+    float I[ND][R][G][CW];
 #pragma unroll
-    for (int r = 0; r < R; ++r)
+    for (int d = 0; d < ND; ++d)
 #pragma unroll
-        for (int g = 0; g < G; ++g)
+        for (int r = 0; r < R; ++r)
 #pragma unroll
-            for (int i = 0; i < CW; ++i) I[r][g][i] = Ibc;
+            for (int g = 0; g < G; ++g)
+#pragma unroll
+                for (int i = 0; i < CW; ++i) I[d][r][g][i] = Ibc;
 
     Src src;
     src.col0 = col[0];
@@ -540,7 +689,11 @@ k_sweep_tma(const SweepLaunch L)
         const int s = k % D;
         src.stage = wbase + s * Src::kStage;
         mbar_wait(bars + 8 * s, (unsigned)((k / D) & 1));
-        RT_DISPATCH_SLAB(fl, fl, I, src, len0, len1, len2, Ibc, invL, lane, rev, lbase, Nc, acc, accC, orow, col)
+        if constexpr (ND == 2) {
+            RT_DISPATCH_SLAB_PAIR(fl, fl, I, src, len0, len1, len2, Ibc, invL, lane, lbase, Nc, acc, accC, orow, col)
+        } else {
+            RT_DISPATCH_SLAB(fl, fl, I[0], src, len0, len1, len2, Ibc, invL, lane, rev, lbase, Nc, acc, accC, orow, col)
+        }
         __syncwarp();                     // every lane is done reading stage s
         if (k + D < Na) produce(k + D);
     }
@@ -568,18 +721,28 @@ static cudaError_t launch_owned_one(const SweepLaunch &L, cudaStream_t st)
             kern<<<grid, block, smem, st>>>(L);
             return cudaGetLastError();
         };
+        if constexpr (MODE == MODE_J) {
+            if (L.pair) {
+                switch (L.stages) {
+                case 2: return go(k_sweep_tma<CW, G, R, MODE, 2, 2>, 2);
+                case 3: return go(k_sweep_tma<CW, G, R, MODE, 3, 2>, 3);
+                default: return go(k_sweep_tma<CW, G, R, MODE, 4, 2>, 4);
+                }
+            }
+        }
         switch (L.stages) {
-        case 2: return go(k_sweep_tma<CW, G, R, MODE, 2>, 2);
-        case 3: return go(k_sweep_tma<CW, G, R, MODE, 3>, 3);
-        default: return go(k_sweep_tma<CW, G, R, MODE, 4>, 4);
+        case 2: return go(k_sweep_tma<CW, G, R, MODE, 2, 1>, 2);
+        case 3: return go(k_sweep_tma<CW, G, R, MODE, 3, 1>, 3);
+        default: return go(k_sweep_tma<CW, G, R, MODE, 4, 1>, 4);
         }
     }
+    if (L.pair) return cudaErrorInvalidValue;
     k_sweep_owned<CW, G, R, MODE><<<grid, block, 0, st>>>(L);
     return cudaGetLastError();
 }
 
 template <int CW, int G, int R>
-static int owned_ctas_per_sm_impl(int stages)
+static int owned_ctas_per_sm_impl(int stages, bool pair)
 {
     int n = 0;
     cudaError_t e;
@@ -592,9 +755,15 @@ static int owned_ctas_per_sm_impl(int stages)
             cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
             return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, 32 * kWarpsPerCta, smem);
         };
-        if (D == 2) e = q(k_sweep_tma<CW, G, R, MODE_J, 2>);
-        else if (D == 3) e = q(k_sweep_tma<CW, G, R, MODE_J, 3>);
-        else e = q(k_sweep_tma<CW, G, R, MODE_J, 4>);
+        if (pair) {
+            if (D == 2) e = q(k_sweep_tma<CW, G, R, MODE_J, 2, 2>);
+            else if (D == 3) e = q(k_sweep_tma<CW, G, R, MODE_J, 3, 2>);
+            else e = q(k_sweep_tma<CW, G, R, MODE_J, 4, 2>);
+        } else {
+            if (D == 2) e = q(k_sweep_tma<CW, G, R, MODE_J, 2, 1>);
+            else if (D == 3) e = q(k_sweep_tma<CW, G, R, MODE_J, 3, 1>);
+            else e = q(k_sweep_tma<CW, G, R, MODE_J, 4, 1>);
+        }
     } else {
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_sweep_owned<CW, G, R, MODE_J>, 32 * kWarpsPerCta, 0);
     }
@@ -602,24 +771,25 @@ static int owned_ctas_per_sm_impl(int stages)
 }
 
 template <int CW, int G>
-static int owned_ctas_per_sm_rows(int rows, int stages)
+static int owned_ctas_per_sm_rows(int rows, int stages, bool pair)
 {
     switch (rows) {
-    case 1: return owned_ctas_per_sm_impl<CW, G, 1>(stages);
-    case 2: return owned_ctas_per_sm_impl<CW, G, 2>(stages);
-    case 4: return owned_ctas_per_sm_impl<CW, G, 4>(stages);
+    case 1: return owned_ctas_per_sm_impl<CW, G, 1>(stages, pair);
+    case 2: return owned_ctas_per_sm_impl<CW, G, 2>(stages, pair);
+    case 4: return owned_ctas_per_sm_impl<CW, G, 4>(stages, pair);
     }
     return 0;
 }
 
 // resident CTAs (of kWarpsPerCta warps) per SM of the J-mode owned kernel; 0 if the configuration cannot launch
-int owned_ctas_per_sm(int Nb, int rows, int stages)
+int owned_ctas_per_sm(int Nb, int rows, int stages, bool pair)
 {
+    if (pair && stages < 2) return 0;
     switch (Nb) {
-    case 32:  return owned_ctas_per_sm_rows<1, 1>(rows, stages);
-    case 64:  return owned_ctas_per_sm_rows<2, 1>(rows, stages);
-    case 128: return owned_ctas_per_sm_rows<2, 2>(rows, stages);
-    case 256: return owned_ctas_per_sm_rows<2, 4>(rows, stages);
+    case 32:  return owned_ctas_per_sm_rows<1, 1>(rows, stages, pair);
+    case 64:  return owned_ctas_per_sm_rows<2, 1>(rows, stages, pair);
+    case 128: return owned_ctas_per_sm_rows<2, 2>(rows, stages, pair);
+    case 256: return owned_ctas_per_sm_rows<2, 4>(rows, stages, pair);
     }
     return 0;
 }
