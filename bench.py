@@ -145,6 +145,8 @@ def main():
     ap.add_argument("--slots", type=int, default=None)
     ap.add_argument("--rows", type=int, default=None)
     ap.add_argument("--stages", type=int, default=None)
+    ap.add_argument("--pair", type=int, default=None, help="0: switch the mirror-pair schedule off (ablation)")
+    ap.add_argument("--tune", action="append", default=[], help="key=value passed to rt_tune (experiments)")
     ap.add_argument("--flags", type=int, default=0, help="0 owned, 1 atomic ablation, 2 paper's four groups")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -167,7 +169,8 @@ def main():
     spec = CONFIGS[args.config]
     kap, S = make_fields(args.config)
     dirs = rt.healpix_dirs(spec.nside)
-    tr = rt.RayTracer(spec.dims, spec.nbins, dirs, flags=args.flags, slots=args.slots, rows=args.rows, stages=args.stages)
+    tr = rt.RayTracer(spec.dims, spec.nbins, dirs, flags=args.flags, slots=args.slots, rows=args.rows, stages=args.stages, pair=args.pair,
+                      tune=dict((kv.split('=')[0], int(kv.split('=')[1])) for kv in args.tune))
     stream = torch.cuda.current_stream()
     kap_h = torch.from_numpy(kap).pin_memory()
     S_h = torch.from_numpy(S).pin_memory()

@@ -169,7 +169,7 @@ def rt_destroy(h):
 class RayTracer:
     """Owns one rt_ctx.  Fields and outputs are torch CUDA tensors [nbins][nz][ny][nx] fp32."""
 
-    def __init__(self, dims, nbins, dirs, cell_width=1.0, flags=RT_OWNED, slots=None, rows=None, stages=None):
+    def __init__(self, dims, nbins, dirs, cell_width=1.0, flags=RT_OWNED, slots=None, rows=None, stages=None, pair=None, tune=None):
         self.nx, self.ny, self.nz = (int(v) for v in dims)
         self.nbins = int(nbins)
         self.dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
@@ -182,6 +182,10 @@ class RayTracer:
             rt_tune(self.h, "rows", rows)
         if stages is not None:
             rt_tune(self.h, "stages", stages)
+        if pair is not None:
+            rt_tune(self.h, "pair", int(pair))
+        for k, v in (tune or {}).items():
+            rt_tune(self.h, k, int(v))
 
     def shape(self):
         return (self.nbins, self.nz, self.ny, self.nx)

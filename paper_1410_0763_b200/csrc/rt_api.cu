@@ -49,6 +49,7 @@ struct rt_ctx {
     // singles[l] everything that has no partner (zero b slope, or an unsymmetric user set)
     std::vector<int> pairs[2], singles[2];
     bool pair_enable = true;
+    int hint = 0;
     int slots_pair[2] = {0, 0}, slots_single[2] = {0, 0};
     bool fast[2] = {false, false};   // owned kernel usable for the layout
     int rows = 2;
@@ -135,7 +136,7 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     if (rays_per_cell != 1) return RT_EINVAL;
     if (!(cell_width > 0.0) || !std::isfinite(cell_width)) return RT_EINVAL;
     if (flags > 2u) return RT_EINVAL;
-    if ((long long)nx * ny * nz * nbins >= (1ll << 40)) return RT_EINVAL;
+    if ((long long)nx * ny * nz >= (1ll << 31) || (long long)nx * ny * nz * nbins >= (1ll << 40)) return RT_EINVAL;
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
     if (e != cudaSuccess) return cuda_fail(e);
@@ -205,6 +206,7 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     auto by_class = [&](int x, int y) {
         if (c->hd[x].a != c->hd[y].a) return c->hd[x].a < c->hd[y].a;
         if (c->hd[x].refl[c->hd[x].a] != c->hd[y].refl[c->hd[y].a]) return c->hd[x].refl[c->hd[x].a] < c->hd[y].refl[c->hd[y].a];
+        if (c->hd[x].refl[c->hd[x].b] != c->hd[y].refl[c->hd[y].b]) return c->hd[x].refl[c->hd[x].b] < c->hd[y].refl[c->hd[y].b];
         return c->hd[x].work > c->hd[y].work;
     };
     for (int l = 0; l < 2; ++l) std::stable_sort(c->order[l].begin(), c->order[l].end(), by_class);
@@ -271,7 +273,8 @@ extern "C" int rt_tune(rt_ctx *c, const char *key, int value)
     if (!c || !key) return RT_EINVAL;
     if (c->buffers_ready) return RT_ESTATE;
     if (!strcmp(key, "slots")) { if (value < 1 || value > 4096) return RT_EINVAL; c->slots_req = value; return RT_OK; }
-    if (!strcmp(key, "stages")) { if (!(value == 0 || (value >= 2 && value <= 4))) return RT_EINVAL; c->stages = value; return RT_OK; }
+    if (!strcmp(key, "stages")) { if (!(value >= 2 && value <= 4)) return RT_EINVAL; c->stages = value; return RT_OK; }
+    if (!strcmp(key, "l2hint")) { if (value < 0 || value > 3) return RT_EINVAL; c->hint = value; return RT_OK; }
     if (!strcmp(key, "pair")) { if (value != 0 && value != 1) return RT_EINVAL; c->pair_enable = value != 0; return RT_OK; }
     if (!strcmp(key, "rows")) { if (!(value == 1 || value == 2 || value == 4)) return RT_EINVAL; c->rows = value; return RT_OK; }
     return RT_EINVAL;
@@ -313,7 +316,7 @@ static int ensure_buffers(rt_ctx *c)
                     return std::max(1, std::min(nd, resident / std::max(1, ctas_dir)));
                 };
                 c->slots_single[l] = wave(false);
-                c->slots_pair[l] = (c->fast[l] && c->stages >= 2) ? wave(true) : 0;
+                c->slots_pair[l] = c->fast[l] ? wave(true) : 0;
                 want = std::max(c->slots_single[l], c->slots_pair[l]);
                 if (!c->fast[l]) want = std::min(nd, 16);
             }
@@ -388,14 +391,14 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
         memset(&L, 0, sizeof(L));
         L.P = c->d_P[l]; L.acc = c->d_acc[l]; L.accC = c->d_accC[l];
         L.dirs = c->d_dirs; L.prog = c->d_prog; L.nbins = nbins; L.ncell = c->ncell; L.Ibc = c->d_Ibc;
-        L.rows = rows_for(c, l); L.mode = mode; L.stages = c->stages;
+        L.rows = rows_for(c, l); L.mode = mode; L.stages = c->stages; L.hint = c->hint;
         L.Nb = (l == 0) ? c->nx : c->ny;
         const bool owned_l = c->fast[l];
         // the lists this traversal walks: (direction list, position in d_batch, slots per launch, paired)
         struct Pass { const std::vector<int> *list; int off; int S; int pair; };
         Pass passes[2];
         int npass = 0;
-        const bool use_pairs = (mode == MODE_J) && only_dir < 0 && c->pair_enable && owned_l && c->stages >= 2 &&
+        const bool use_pairs = (mode == MODE_J) && only_dir < 0 && c->pair_enable && owned_l &&
                                !c->pairs[l].empty();
         if (use_pairs) {
             passes[npass++] = Pass{&c->pairs[l], my_j, c->slots_pair[l], 1};
@@ -411,8 +414,10 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
             int i = 0;
             while (i < nl) {
                 const int a = c->hd[list[i]].a;
+                const int rev = c->hd[list[i]].refl[c->hd[list[i]].b];
                 int n = 0;
-                while (i + n < nl && n < S && c->hd[list[i + n]].a == a) ++n;
+                while (i + n < nl && n < S && c->hd[list[i + n]].a == a &&
+                       c->hd[list[i + n]].refl[c->hd[list[i + n]].b] == rev) ++n;
                 int first = i, count = n;
                 if (only_dir >= 0) {
                     if (list[i] != only_dir) { i += 1; continue; }
@@ -421,6 +426,7 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
                 used[l] = std::max(used[l], count);
                 L.batch = c->d_batch + passes[ps].off + first;
                 L.nslots = count;
+                L.rev = rev;
                 L.Nc = c->hd[list[first]].Nc;
                 if (owned_l && owned_supported(L.Nb, L.Nc, L.rows)) {
                     CK(launch_sweep_owned(L, st));

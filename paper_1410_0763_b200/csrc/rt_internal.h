@@ -52,7 +52,9 @@ struct SweepLaunch {
     int mode;
     int variant;             // generic kernel: 0 = four groups (one launch per group), 1 = atomics
     int group;               // generic kernel: group id 0..3
-    int stages;              // owned kernel: 0 = inputs via registers; 2..4 = depth of the TMA shared-memory ring
+    int stages;              // owned kernel: depth of the TMA shared-memory ring (2..4)
+    int hint;                // owned TMA kernel: bit 0 = field rows evict_last in L2, bit 1 = accumulator rows evict_first
+    int rev;                 // owned kernel, single directions: all slots have a reflected b component (sj < 0)
     int pair;                // owned TMA kernel, MODE_J: every slot carries a direction and its b-mirror (rt_kernels.cu "mirror pairs")
 };
 

@@ -1,0 +1,502 @@
+// The owned sweep kernel (k_sweep_tma) of the diffuse-radiation ray sweep, as templates.  Included by
+// rt_sweep_nb*.cu, one translation unit per supported width of the memory-contiguous transverse axis
+// (so that nvcc compiles them in parallel).
+//
+// Ownership scheme (replaces the paper's four sequential ray groups):
+// one warp owns R consecutive ray rows (transverse axis c) over the full cyclic extent of the
+// memory-contiguous transverse axis b: Nb = 32*CW*G columns, each thread owning G chunks of CW
+// adjacent columns (aligned vector loads).  Along b the thread owns CELLS: a ray that crosses a
+// b-boundary is handed to the owner of the next column (register move / one rotate shuffle per
+// chunk; a chunk-to-chunk carry; leaving the last column = leaving the box, and a new ray with the
+// inflow intensity enters the first column).  Along c the warp owns RAYS: the memory row of ray
+// row r is (q0 + r + shift_k) mod Nc, pure address arithmetic; pieces that fall into the next
+// memory row use the next row's data and add to the next row's partial, both held by the same
+// thread.  Only the partial of the row above the warp's last ray row has another owner; it goes
+// to the seam accumulator accC with plain stores.  Every cell therefore has exactly one writer
+// per accumulator array and launch: no atomics, deterministic sums.
+//
+// Variants (template parameter V):
+//   V = 0  one direction per warp, rays move towards higher memory columns
+//   V = 1  one direction per warp, rays move towards lower memory columns (b component reflected):
+//          canonical lane / chunk order is the reverse of the memory order
+//   V = 2  mirror pair: a direction and its b-mirror share every load, store and exponential
+#pragma once
+#include "rt_internal.h"
+
+namespace rt {
+
+// ------------------------------------------------------------------------------------------------
+// Segment update (eq. 7, eq. 8), fp32
+//   A = 1 - exp(-kappa*len); contribution to the cell += I_in * A  (numerator of eq. 11 times kappa*L,
+//   see DESIGN.md "Arithmetic"); I_out = I_in * e + S * A with e = exp(-kappa*len).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// e = exp(-kappa*len) and A = 1 - e, each with small RELATIVE error: e straight from ex2 (never as
+// 1 - A: behind an opaque cell the transmitted part I*e is all that is left), A from a polynomial
+// where 1 - e would cancel.
+__device__ __forceinline__ float one_minus_exp(float kap, float len, float ct, float &e)
+{
+    const float x = kap * len;
+    e = ex2_approx(kap * ct);                                  // ct = -len*log2(e)
+    // small-x branch: x * (c0 + c1 x + c2 x^2 + c3 x^3), fitted on [0, 1/4]; rel. error 3.4e-7
+    float p = fmaf(x, -0.0377338513f, 0.1660640817f);
+    p = fmaf(x, p, -0.4999701648f);
+    p = fmaf(x, p, 0.9999997683f);
+    return x < 0.25f ? x * p : 1.0f - e;
+}
+
+// ND intensities (1, or 2 for a mirror pair) cross the same cell piece: e, A and S*A are shared.
+template <int MODE, int ND>
+__device__ __forceinline__ void seg_update(float (&I)[ND], float kap, float src, float len, float ct, float &part)
+{
+    if (MODE == MODE_J) {
+        float e;
+        const float A = one_minus_exp(kap, len, ct, e);
+        const float SA = src * A;
+        if (ND == 2) part = fmaf(I[0] + I[ND - 1], A, part);
+        else         part = fmaf(I[0], A, part);
+#pragma unroll
+        for (int d = 0; d < ND; ++d) I[d] = fmaf(I[d], e, SA);   // eq. 7
+    } else if (MODE == MODE_COUNT) {
+        part += (float)ND;
+    } else {
+        part += (float)ND * len;
+    }
+}
+
+template <int CW> struct VecT;
+template <> struct VecT<2> { using D = float4; using A = float2; };
+template <> struct VecT<1> { using D = float2; using A = float;  };
+
+template <int CW>
+__device__ __forceinline__ void unpack(const typename VecT<CW>::D &v, float (&kap)[CW], float (&src)[CW]);
+template <>
+__device__ __forceinline__ void unpack<2>(const float4 &v, float (&kap)[2], float (&src)[2])
+{ kap[0] = v.x; src[0] = v.y; kap[1] = v.z; src[1] = v.w; }
+template <>
+__device__ __forceinline__ void unpack<1>(const float2 &v, float (&kap)[1], float (&src)[1])
+{ kap[0] = v.x; src[0] = v.y; }
+
+template <int CW>
+__device__ __forceinline__ typename VecT<CW>::A acc_new(const typename VecT<CW>::A &o, const float (&part)[CW], float w);
+template <>
+__device__ __forceinline__ float2 acc_new<2>(const float2 &o, const float (&part)[2], float w)
+{ return make_float2(fmaf(part[0], w, o.x), fmaf(part[1], w, o.y)); }
+template <>
+__device__ __forceinline__ float acc_new<1>(const float &o, const float (&part)[1], float w)
+{ return fmaf(part[0], w, o); }
+
+constexpr int kWarpsPerCta = kOwnedWarpsPerCta;
+
+// The six slab patterns that occur away from exact boundary touches get straight-line code
+// (FLC = compile-time flags); anything else runs the same body with run-time flags (FLC < 0).
+constexpr int kPatNone = 0;
+constexpr int kPatB    = F_SB1 | F_P1;
+constexpr int kPatC    = F_SC1 | F_P1;
+constexpr int kPatBC   = F_SB1 | F_P1 | F_SC2 | F_P2;
+constexpr int kPatCB   = F_SC1 | F_P1 | F_SB2 | F_P2;
+constexpr int kPatD    = F_SB1 | F_SC1 | F_P1;
+
+// ------------------------------------------------------------------------------------------------
+// One slab for the R ray rows of a warp, stage-major: every chunk does piece 0, then the step, then
+// piece 1, ... (a mirror pair needs its chunk-to-chunk carries in both chunk orders).
+//   sp / sa : this lane's position in row 0 of the stage's packed-field rows / accumulator rows
+//             (shared memory); row r is at + r * kRowP / kRowA, canonical chunk g at a compile-time
+//             offset.  Row R is the seam row (valid only if some piece steps along c).
+//   rowp[r] : this lane's position in the global accumulator row of ray row r (r = R: seam
+//             accumulator).  New accumulator values go straight to global memory (one writer per cell).
+//   I[r][g][i][d] : intensity of the ray currently in column i of chunk g of ray row r, direction d;
+//             i is in MEMORY order.
+// ------------------------------------------------------------------------------------------------
+template <int CW, int G, int R, int MODE, int FLC, int V>
+__device__ __forceinline__ void slab_rows(const unsigned fl_rt, float (&I)[R][G][CW][(V == 2) ? 2 : 1],
+                                          const unsigned char *__restrict__ sp, const unsigned char *__restrict__ sa,
+                                          const float len0, const float len1, const float len2,
+                                          const float Ibc, const float invL, const int lane, const int lwrap,
+                                          float *const (&rowp)[R + 1])
+{
+    using DV = typename VecT<CW>::D;
+    using AV = typename VecT<CW>::A;
+    constexpr int ND = (V == 2) ? 2 : 1;
+    constexpr bool REV = (V == 1);
+    constexpr int kRowP = 32 * CW * G * (int)sizeof(float2), kRowA = 32 * CW * G * (int)sizeof(float);
+    constexpr unsigned FULL = 0xffffffffu;
+    constexpr float LOG2E = 1.4426950408889634f;
+    const unsigned fl = (FLC >= 0) ? (unsigned)FLC : fl_rt;
+    const float ct0 = -len0 * LOG2E, ct1 = -len1 * LOG2E, ct2 = -len2 * LOG2E;
+    const bool anySC = (fl & (F_SC1 | F_SC2)) != 0;
+    // memory chunk of canonical chunk g, as element offsets within a row
+#define RT_MG(g) ((REV ? (G - 1 - (g)) : (g)) * 32 * CW)
+
+    float part_cur[G][CW];
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int i = 0; i < CW; ++i) part_cur[g][i] = 0.0f;
+
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const bool wrap_r = (r == lwrap);
+        float part_next[G][CW];
+        float kc[G][CW], sc[G][CW], kn[G][CW], sn[G][CW];
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            unpack<CW>(*reinterpret_cast<const DV *>(sp + r * kRowP + RT_MG(g) * (int)sizeof(float2)), kc[g], sc[g]);
+            if (anySC)
+                unpack<CW>(*reinterpret_cast<const DV *>(sp + (r + 1) * kRowP + RT_MG(g) * (int)sizeof(float2)), kn[g], sn[g]);
+#pragma unroll
+            for (int i = 0; i < CW; ++i) {
+                part_next[g][i] = 0.0f;
+                if (!anySC) { kn[g][i] = kc[g][i]; sn[g][i] = sc[g][i]; }
+            }
+        }
+        float (&Ir)[G][CW][ND] = I[r];
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int i = 0; i < CW; ++i) seg_update<MODE, ND>(Ir[g][i], kc[g][i], sc[g][i], len0, ct0, part_cur[g][i]);
+        bool sel = false;
+#pragma unroll
+        for (int stage = 1; stage <= 2; ++stage) {
+            const unsigned fsb = (stage == 1) ? F_SB1 : F_SB2;
+            const unsigned fsc = (stage == 1) ? F_SC1 : F_SC2;
+            const unsigned fp = (stage == 1) ? F_P1 : F_P2;
+            const float len = (stage == 1) ? len1 : len2;
+            const float ct = (stage == 1) ? ct1 : ct2;
+            if (fl & (fsb | fsc)) {
+                if (MODE == MODE_J) {
+                    if (fl & fsb) {
+                        // direction 0: hand every ray to the owner of the next column in canonical order
+                        // (canonical lane + 1 is always the physical lane + 1); a new ray enters at
+                        // canonical column 0.  Within a chunk, memory element 0 is upstream unless REV.
+                        float carry = Ibc;
+#pragma unroll
+                        for (int g = 0; g < G; ++g) {
+                            const float out = REV ? Ir[g][0][0] : Ir[g][CW - 1][0];
+                            const float t = __shfl_sync(FULL, out, (lane + 31) & 31);
+                            const float in = (lane == 0) ? carry : t;
+                            carry = t;
+                            if (REV) { if (CW == 2) Ir[g][0][0] = Ir[g][CW - 1][0]; Ir[g][CW - 1][0] = in; }
+                            else     { if (CW == 2) Ir[g][CW - 1][0] = Ir[g][0][0]; Ir[g][0][0] = in; }
+                        }
+                        if (ND == 2) {
+                            // mirrored direction: towards lower columns; a new ray enters the last column
+                            carry = Ibc;
+#pragma unroll
+                            for (int g = G - 1; g >= 0; --g) {
+                                const float t = __shfl_sync(FULL, Ir[g][0][ND - 1], (lane + 1) & 31);
+                                const float in = (lane == 31) ? carry : t;
+                                carry = t;
+                                if (CW == 2) Ir[g][0][ND - 1] = Ir[g][CW - 1][ND - 1];
+                                Ir[g][CW - 1][ND - 1] = in;
+                            }
+                        }
+                    }
+                    if ((fl & fsc) && wrap_r) {   // step along c out of the box: new rays enter
+#pragma unroll
+                        for (int g = 0; g < G; ++g)
+#pragma unroll
+                            for (int i = 0; i < CW; ++i)
+#pragma unroll
+                                for (int d = 0; d < ND; ++d) Ir[g][i][d] = Ibc;
+                    }
+                }
+                if (fl & fsc) sel = true;
+            }
+            if (fl & fp) {
+#pragma unroll
+                for (int g = 0; g < G; ++g)
+#pragma unroll
+                    for (int i = 0; i < CW; ++i) {
+                        if (sel) seg_update<MODE, ND>(Ir[g][i], kn[g][i], sn[g][i], len, ct, part_next[g][i]);
+                        else     seg_update<MODE, ND>(Ir[g][i], kc[g][i], sc[g][i], len, ct, part_cur[g][i]);
+                    }
+            }
+        }
+        // row r's partial is complete (own pieces + pieces of ray row r-1 that stepped along c)
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+            *reinterpret_cast<AV *>(rowp[r] + RT_MG(g)) =
+                acc_new<CW>(*reinterpret_cast<const AV *>(sa + r * kRowA + RT_MG(g) * (int)sizeof(float)), part_cur[g], invL);
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int i = 0; i < CW; ++i) part_cur[g][i] = part_next[g][i];
+    }
+    if (anySC) {
+        // seam: the partial of the memory row above the warp's last ray row has another owner
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+            *reinterpret_cast<AV *>(rowp[R] + RT_MG(g)) =
+                acc_new<CW>(*reinterpret_cast<const AV *>(sa + R * kRowA + RT_MG(g) * (int)sizeof(float)), part_cur[g], invL);
+    }
+#undef RT_MG
+}
+
+#define RT_DISPATCH_SLAB(fl, ...)                                                         \
+    switch (fl) {                                                                         \
+    case kPatNone: slab_rows<CW, G, R, MODE, kPatNone, V>(__VA_ARGS__); break;            \
+    case kPatB:    slab_rows<CW, G, R, MODE, kPatB, V>(__VA_ARGS__); break;               \
+    case kPatC:    slab_rows<CW, G, R, MODE, kPatC, V>(__VA_ARGS__); break;               \
+    case kPatBC:   slab_rows<CW, G, R, MODE, kPatBC, V>(__VA_ARGS__); break;              \
+    case kPatCB:   slab_rows<CW, G, R, MODE, kPatCB, V>(__VA_ARGS__); break;              \
+    case kPatD:    slab_rows<CW, G, R, MODE, kPatD, V>(__VA_ARGS__); break;               \
+    default:       slab_rows<CW, G, R, MODE, -1, V>(__VA_ARGS__); break;                  \
+    }
+
+// ------------------------------------------------------------------------------------------------
+// TMA / mbarrier helpers (1-D bulk async copies: a mesh row is one contiguous run, so the 1-D bulk
+// form of TMA is used rather than tensor maps)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
+{ asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
+{ asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory"); }
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@!p bra WAIT_%=;\n\t}"
+        :: "r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+// Row bookkeeping of one march, advanced slab by slab with adds only:
+//   frac = fractional part of 1/2 + k*m_c in units of 2^-20 (m_c = Mc / 2^20 <= 1)
+//   lb   = (q0 + floor(1/2 + k*m_c)) mod Nc : memory row of the warp's first ray row at slab k
+//   offk = k * sk                            : element offset of slab k
+struct RowState {
+    int lb, offk;
+    unsigned frac;
+    __device__ __forceinline__ void init(int q0) { lb = q0; offk = 0; frac = (unsigned)(kOne >> 1); }
+    // true iff the rays step along c inside the current slab (cross or exact touch)
+    __device__ __forceinline__ bool steps(int Mc) const { return frac + (unsigned)Mc >= (unsigned)kOne; }
+    __device__ __forceinline__ void advance(int Mc, int Nc, int sk)
+    {
+        frac += (unsigned)Mc;
+        if (frac >= (unsigned)kOne) { frac -= (unsigned)kOne; lb = (lb + 1 == Nc) ? 0 : lb + 1; }
+        offk += sk;
+    }
+};
+
+template <int CW, int G, int R>
+struct StageGeom {
+    static constexpr int kNb = 32 * CW * G;
+    static constexpr int kRowP = kNb * (int)sizeof(float2);
+    static constexpr int kRowA = kNb * (int)sizeof(float);
+    static constexpr int kStage = (R + 1) * (kRowP + kRowA);
+};
+
+// Each warp owns D stages; stage (k mod D) holds slab k's packed field rows and old accumulator
+// rows, copied by bulk async copies (SASS UBLKCP) issued by lane 0 D slabs ahead and tracked by one
+// mbarrier per stage (transaction-byte count).  No registers are spent on data in flight, so the
+// prefetch depth is set by shared memory, not by the register file.
+template <int CW, int G, int R, int MODE, int D, int V>
+__global__ void __launch_bounds__(32 * kWarpsPerCta)
+k_sweep_tma(const SweepLaunch L)
+{
+    using SG = StageGeom<CW, G, R>;
+    constexpr int ND = (V == 2) ? 2 : 1;
+    constexpr bool REV = (V == 1);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int kWarpBytes = D * SG::kStage + 128;
+
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int slot = blockIdx.y, bin = blockIdx.z;
+    const DirDev *__restrict__ Dp = L.dirs + L.batch[slot];
+    const int Nc = Dp->Nc, Na = Dp->Na, Mc = Dp->Mc;
+    const int q0 = (blockIdx.x * kWarpsPerCta + wid) * R;
+    if (q0 >= Nc) return;
+    const int sk = (int)Dp->sk, sl = (int)Dp->sl;        // |offsets| < 2^31: checked by rt_create
+    const float invL = (MODE == MODE_J) ? Dp->invL : 1.0f;
+    const float Ibc = L.Ibc[bin];
+    const SlabProg *__restrict__ prog = L.prog + Dp->prog_off;
+
+    const long long foff = (long long)bin * L.ncell + Dp->base;
+    const float2 *__restrict__ P = L.P + foff;
+    float *__restrict__ acc = L.acc + ((long long)slot * L.nbins) * L.ncell + foff;
+    float *__restrict__ accC = L.accC + ((long long)slot * L.nbins) * L.ncell + foff;
+
+    unsigned char *wbase = smem_raw + wid * kWarpBytes;
+    const unsigned wbase_s = smem_u32(wbase);
+    const unsigned bars = wbase_s + D * SG::kStage;
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < D; ++s) mbar_init(bars + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+
+    // producer (lane 0): ask the TMA engine for the rows of the slab described by `ps` into stage s
+    RowState ps;
+    ps.init(q0);
+    auto produce = [&](int s) {
+        if (lane == 0) {
+            const unsigned st = wbase_s + s * SG::kStage, bar = bars + 8 * s;
+            const bool seam = ps.steps(Mc);
+            const int nrows = R + (seam ? 1 : 0);
+            mbar_expect_tx(bar, (unsigned)(nrows * ((MODE == MODE_J ? SG::kRowP : 0) + SG::kRowA)));
+#pragma unroll
+            for (int r = 0; r <= R; ++r) {
+                if (r == R && !seam) break;
+                int l = ps.lb + r; if (l >= Nc) l -= Nc;
+                const int o = ps.offk + l * sl;
+                if (MODE == MODE_J) bulk_g2s(st + r * SG::kRowP, P + o, SG::kRowP, bar);
+                bulk_g2s(st + (R + 1) * SG::kRowP + r * SG::kRowA, (r < R ? acc : accC) + o, SG::kRowA, bar);
+            }
+        }
+        ps.advance(Mc, Nc, sk);
+    };
+#pragma unroll 1
+    for (int kk = 0; kk < D && kk < Na; ++kk) produce(kk);
+
+    float I[R][G][CW][ND];
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+#pragma unroll
+            for (int i = 0; i < CW; ++i)
+#pragma unroll
+                for (int d = 0; d < ND; ++d) I[r][g][i][d] = Ibc;
+
+    // this lane's first memory column (canonical chunk 0 is memory chunk G-1 when REV)
+    const int lcol = CW * (REV ? 31 - lane : lane);
+    const unsigned char *lane_p = wbase + lcol * (int)sizeof(float2);
+    const unsigned char *lane_a = wbase + (R + 1) * SG::kRowP + lcol * (int)sizeof(float);
+    float *const acc_l = acc + lcol;
+    float *const accC_l = accC + lcol;
+
+    RowState cs;
+    cs.init(q0);
+    SlabProg pr = prog[0];
+    int s = 0;
+    unsigned phase = 0;
+
+#pragma unroll 1
+    for (int k = 0; k < Na; ++k) {
+        const unsigned fl = pr.flags;
+        const float len0 = pr.len0, len1 = pr.len1, len2 = pr.len2;
+        if (k + 1 < Na) pr = prog[k + 1];
+        float *rowp[R + 1];
+#pragma unroll
+        for (int r = 0; r <= R; ++r) {
+            int l = cs.lb + r; if (l >= Nc) l -= Nc;
+            rowp[r] = (r < R ? acc_l : accC_l) + (cs.offk + l * sl);
+        }
+        const int lwrap = Nc - 1 - cs.lb;
+        const unsigned char *sp = lane_p + s * SG::kStage;
+        const unsigned char *sa = lane_a + s * SG::kStage;
+        mbar_wait(bars + 8 * s, phase);
+        RT_DISPATCH_SLAB(fl, fl, I, sp, sa, len0, len1, len2, Ibc, invL, lane, lwrap, rowp)
+        __syncwarp();                     // every lane is done reading stage s
+        if (k + D < Na) produce(s);
+        cs.advance(Mc, Nc, sk);
+        if (++s == D) { s = 0; phase ^= 1u; }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Launchers for one width Nb = 32*CW*G (instantiated in rt_sweep_nb*.cu)
+// ------------------------------------------------------------------------------------------------
+template <int CW, int G, int R, int D>
+constexpr int sweep_smem_bytes() { return kWarpsPerCta * (D * StageGeom<CW, G, R>::kStage + 128); }
+
+template <int CW, int G, int R, int MODE, int D, int V>
+static cudaError_t launch_tma(const SweepLaunch &L, dim3 grid, cudaStream_t st)
+{
+    constexpr int smem = sweep_smem_bytes<CW, G, R, D>();
+    if (smem > 227 * 1024) return cudaErrorInvalidValue;
+    auto kern = k_sweep_tma<CW, G, R, MODE, D, V>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, dim3(32 * kWarpsPerCta), smem, st>>>(L);
+    return cudaGetLastError();
+}
+
+template <int CW, int G, int R, int MODE, int D>
+static cudaError_t launch_variant(const SweepLaunch &L, dim3 grid, cudaStream_t st)
+{
+    if constexpr (MODE == MODE_J) {
+        if (L.pair) return launch_tma<CW, G, R, MODE, D, 2>(L, grid, st);
+    } else {
+        if (L.pair) return cudaErrorInvalidValue;
+    }
+    return L.rev ? launch_tma<CW, G, R, MODE, D, 1>(L, grid, st) : launch_tma<CW, G, R, MODE, D, 0>(L, grid, st);
+}
+
+template <int CW, int G, int R>
+static cudaError_t launch_rows(const SweepLaunch &L, cudaStream_t st)
+{
+    const int tiles = L.Nc / R;
+    const dim3 grid((tiles + kWarpsPerCta - 1) / kWarpsPerCta, L.nslots, L.nbins);
+    if (L.mode == MODE_COUNT) return launch_variant<CW, G, R, MODE_COUNT, 2>(L, grid, st);   // diagnostics: depth 2
+    if (L.mode == MODE_DS)    return launch_variant<CW, G, R, MODE_DS, 2>(L, grid, st);
+    switch (L.stages) {
+    case 2:  return launch_variant<CW, G, R, MODE_J, 2>(L, grid, st);
+    case 3:  return launch_variant<CW, G, R, MODE_J, 3>(L, grid, st);
+    default: return launch_variant<CW, G, R, MODE_J, 4>(L, grid, st);
+    }
+}
+
+template <int CW, int G>
+cudaError_t launch_sweep_nb(const SweepLaunch &L, cudaStream_t st)
+{
+    switch (L.rows) {
+    case 1: return launch_rows<CW, G, 1>(L, st);
+    case 2: return launch_rows<CW, G, 2>(L, st);
+    case 4: return launch_rows<CW, G, 4>(L, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+template <int CW, int G, int R, int D>
+static int ctas_per_sm_one(bool pair)
+{
+    constexpr int smem = sweep_smem_bytes<CW, G, R, D>();
+    if (smem > 227 * 1024) return 0;
+    int n = 0;
+    auto q = [&](auto kern) {
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, 32 * kWarpsPerCta, smem);
+    };
+    const cudaError_t e = pair ? q(k_sweep_tma<CW, G, R, MODE_J, D, 2>) : q(k_sweep_tma<CW, G, R, MODE_J, D, 0>);
+    return e == cudaSuccess ? n : 0;
+}
+
+template <int CW, int G, int R>
+static int ctas_per_sm_rows(int stages, bool pair)
+{
+    switch (stages) {
+    case 2:  return ctas_per_sm_one<CW, G, R, 2>(pair);
+    case 3:  return ctas_per_sm_one<CW, G, R, 3>(pair);
+    default: return ctas_per_sm_one<CW, G, R, 4>(pair);
+    }
+}
+
+// resident CTAs (of kWarpsPerCta warps) per SM of the J-mode kernel; 0 if the configuration cannot launch
+template <int CW, int G>
+int ctas_per_sm_nb(int rows, int stages, bool pair)
+{
+    switch (rows) {
+    case 1: return ctas_per_sm_rows<CW, G, 1>(stages, pair);
+    case 2: return ctas_per_sm_rows<CW, G, 2>(stages, pair);
+    case 4: return ctas_per_sm_rows<CW, G, 4>(stages, pair);
+    }
+    return 0;
+}
+
+}  // namespace rt

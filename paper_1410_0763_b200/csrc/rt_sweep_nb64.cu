@@ -1,0 +1,8 @@
+// k_sweep_tma for meshes whose memory-contiguous transverse extent is 64 cells (CW = 2 columns per
+// chunk, G = 1 chunks per thread).  One translation unit per width so that they compile in parallel.
+#include "rt_sweep.cuh"
+
+namespace rt {
+cudaError_t launch_sweep_nb64(const SweepLaunch &L, cudaStream_t st) { return launch_sweep_nb<2, 1>(L, st); }
+int ctas_per_sm_nb64(int rows, int stages, bool pair) { return ctas_per_sm_nb<2, 1>(rows, stages, pair); }
+}  // namespace rt

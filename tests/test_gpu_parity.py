@@ -27,11 +27,11 @@ def rel_err(got, ref):
 
 
 def gpu_run(kap, S, dirs, Ibc=None, cell_width=1.0, flags=0, count_dirs=(), want_ds=True, slots=None, rows=None,
-            stages=None):
+            stages=None, pair=None):
     import paper_1410_0763_b200 as rt
     torch = _torch()
     nb, nz, ny, nx = kap.shape
-    tr = rt.RayTracer((nx, ny, nz), nb, dirs, cell_width=cell_width, flags=flags, slots=slots, rows=rows, stages=stages)
+    tr = rt.RayTracer((nx, ny, nz), nb, dirs, cell_width=cell_width, flags=flags, slots=slots, rows=rows, stages=stages, pair=pair)
     out = {}
     try:
         if Ibc is not None:
@@ -255,11 +255,11 @@ def test_ablation_variants_pass_the_same_gates(orc, flags):
     check_full(orc, kap, S, dirs, out, ref)
 
 
-@pytest.mark.parametrize("rows,stages", [(1, 0), (2, 0), (4, 0), (1, 2), (2, 3), (4, 4), (1, 4)])
-def test_rows_per_warp_variants(orc, rows, stages):
+@pytest.mark.parametrize("rows,stages,pair", [(1, 2, 1), (2, 2, 0), (4, 2, 1), (1, 3, 0), (2, 3, 1), (4, 4, 0), (1, 4, 1)])
+def test_rows_per_warp_variants(orc, rows, stages, pair):
     kap, S = _rand((64, 32, 16), 9)
     dirs = orc.healpix_dirs(2)
-    out = gpu_run(kap, S, dirs, rows=rows, stages=stages, slots=5, count_dirs=[0, 13, 47])
+    out = gpu_run(kap, S, dirs, rows=rows, stages=stages, pair=pair, slots=5, count_dirs=[0, 13, 47])
     ref = orc.sweep(kap, S, dirs, count_dirs=[0, 13, 47])
     check_full(orc, kap, S, dirs, out, ref)
 
