@@ -52,6 +52,7 @@ struct rt_ctx {
     int hint = 0;
     int slots_pair[2] = {0, 0}, slots_single[2] = {0, 0};
     bool fast[2] = {false, false};   // owned kernel usable for the layout
+    int pp[2] = {0, 0};              // packed field of the layout is pair-packed (rt_internal.h)
     int rows = 2;
     int stages = 2;                  // depth of the owned kernel's TMA shared-memory ring (0 = register path)
     int slots_req = 0;               // user override
@@ -237,7 +238,10 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     }
     // owned kernel: the memory-contiguous transverse extent must be 32/64/128/256 (one warp owns full rows)
     const int NbL[2] = {nx, ny};
-    for (int l = 0; l < 2; ++l) c->fast[l] = (flags == RT_OWNED) && (NbL[l] == 32 || NbL[l] == 64 || NbL[l] == 128 || NbL[l] == 256);
+    for (int l = 0; l < 2; ++l) {
+        c->fast[l] = (flags == RT_OWNED) && (NbL[l] == 32 || NbL[l] == 64 || NbL[l] == 128 || NbL[l] == 256);
+        c->pp[l] = (c->fast[l] && NbL[l] >= 64) ? 1 : 0;      // two columns per chunk
+    }
 
 #define CKC(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { int rc__ = (e__ == cudaErrorMemoryAllocation) ? RT_ENOMEM : cuda_fail(e__); free_device(c); delete c; return rc__; } } while (0)
     CKC(cudaMalloc(&c->d_dirs, sizeof(DirDev) * ndirs));
@@ -351,7 +355,7 @@ extern "C" int rt_set_fields(rt_ctx *c, const float *kappa_dev, const float *S_d
     int rc = ensure_buffers(c);
     if (rc != RT_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    CK(launch_pack_fields(kappa_dev, S_dev, c->d_P[0], c->d_P[1], c->nx, c->ny, c->nz, c->nbins, st));
+    CK(launch_pack_fields(kappa_dev, S_dev, c->d_P[0], c->d_P[1], c->pp[0], c->pp[1], c->nx, c->ny, c->nz, c->nbins, st));
     c->fields_set = true;
     return RT_OK;
 }
@@ -392,7 +396,7 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
         L.P = c->d_P[l]; L.acc = c->d_acc[l]; L.accC = c->d_accC[l];
         L.dirs = c->d_dirs; L.prog = c->d_prog; L.nbins = nbins; L.ncell = c->ncell; L.Ibc = c->d_Ibc;
         L.rows = rows_for(c, l); L.mode = mode; L.stages = c->stages; L.hint = c->hint;
-        L.Nb = (l == 0) ? c->nx : c->ny;
+        L.Nb = (l == 0) ? c->nx : c->ny; L.pp = c->pp[l];
         const bool owned_l = c->fast[l];
         // the lists this traversal walks: (direction list, position in d_batch, slots per launch, paired)
         struct Pass { const std::vector<int> *list; int off; int S; int pair; };
@@ -460,7 +464,7 @@ extern "C" int rt_sweep(rt_ctx *c, float *J_dev, unsigned what, void *stream)
     int used[2];
     int rc = run_traversal(c, MODE_J, -1, c->nbins, st, &launches, used);
     if (rc != RT_OK) return rc;
-    CK(launch_normalise(J_dev, c->d_P[0], c->d_acc[0], c->d_accC[0], used[0], c->d_acc[1], c->d_accC[1], used[1],
+    CK(launch_normalise(J_dev, c->d_P[0], c->pp[0], c->d_acc[0], c->d_accC[0], used[0], c->d_acc[1], c->d_accC[1], used[1],
                         c->nx, c->ny, c->nz, c->nbins, (float)(1.0 / (double)c->ndirs), what == RT_J_TOTAL ? 1 : 0, st));
     c->last_launches = launches + 1;
     return RT_OK;

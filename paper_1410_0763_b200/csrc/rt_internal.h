@@ -56,19 +56,28 @@ struct SweepLaunch {
     int hint;                // owned TMA kernel: bit 0 = field rows evict_last in L2, bit 1 = accumulator rows evict_first
     int rev;                 // owned kernel, single directions: all slots have a reflected b component (sj < 0)
     int pair;                // owned TMA kernel, MODE_J: every slot carries a direction and its b-mirror (rt_kernels.cu "mirror pairs")
+    int pp;                  // P is pair-packed (below)
 };
+
+// Packed-field layouts.  Interleaved: float2 (kappa, S) per cell.  Pair-packed (layouts swept by the
+// owned kernel with two columns per chunk): every two adjacent cells of a row are one float4
+// (kappa0, kappa1, S0, S1), so that a 16-byte shared-memory load delivers the operands of the packed
+// fp32x2 instructions as aligned register pairs.  Index of kappa of cell o in the float view; S is
+// at + 1 (interleaved) or + 2 (pair-packed).
+__host__ __device__ __forceinline__ size_t field_index(size_t o, int pp) { return pp ? 4 * (o >> 1) + (o & 1) : 2 * o; }
+__host__ __device__ __forceinline__ int field_s_offset(int pp) { return pp ? 2 : 1; }
 
 // launchers (rt_kernels.cu); all return cudaError_t of the launch
 cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, SlabProg *prog, double cell_width,
                                   const double *Lvals, cudaStream_t st);
-cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat, float2 *PT,
+cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat, float2 *PT, int ppN, int ppT,
                                int nx, int ny, int nz, int nbins, cudaStream_t st);
 bool owned_supported(int Nb, int Nc, int rows);
 int owned_ctas_per_sm(int Nb, int rows, int stages, bool pair);
 constexpr int kOwnedWarpsPerCta = 4;
 cudaError_t launch_sweep_owned(const SweepLaunch &L, cudaStream_t st);
 cudaError_t launch_sweep_generic(const SweepLaunch &L, int max_lattice_b, int max_lattice_c, cudaStream_t st);
-cudaError_t launch_normalise(float *J, const float2 *Pnat, const float *accN, const float *accNC, int slotsN,
+cudaError_t launch_normalise(float *J, const float2 *Pnat, int ppN, const float *accN, const float *accNC, int slotsN,
                              const float *accT, const float *accTC, int slotsT,
                              int nx, int ny, int nz, int nbins, float inv_nd, int add_S, cudaStream_t st);
 cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const float *accNC, int slotsN,

@@ -78,8 +78,10 @@ cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, SlabProg *prog,
 // Field packing: native copy and (x,y)-transposed copy, kappa floored at kKappaMin
 // ------------------------------------------------------------------------------------------------
 __global__ void k_pack_fields(const float *__restrict__ kappa, const float *__restrict__ S,
-                              float2 *__restrict__ Pnat, float2 *__restrict__ PT, int nx, int ny, int nz)
+                              float2 *__restrict__ Pnat, float2 *__restrict__ PT, int ppN, int ppT, int nx, int ny, int nz)
 {
+    float *__restrict__ fN = reinterpret_cast<float *>(Pnat);
+    float *__restrict__ fT = reinterpret_cast<float *>(PT);
     __shared__ float2 tile[32][33];
     const int bin = blockIdx.z / nz, z = blockIdx.z % nz;
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
@@ -90,23 +92,27 @@ __global__ void k_pack_fields(const float *__restrict__ kappa, const float *__re
         if (x < nx && y < ny) {
             size_t i = boff + ((size_t)z * ny + y) * nx + x;
             float2 v = make_float2(fmaxf(kappa[i], kKappaMin), S[i]);
-            Pnat[i] = v;
+            const size_t o = field_index(i, ppN);
+            fN[o] = v.x; fN[o + field_s_offset(ppN)] = v.y;
             tile[dy][threadIdx.x] = v;
         }
     }
     __syncthreads();
     for (int dx = threadIdx.y; dx < 32; dx += blockDim.y) {
         int x = x0 + dx, y = y0 + threadIdx.x;
-        if (x < nx && y < ny)
-            PT[boff + ((size_t)x * nz + z) * ny + y] = tile[threadIdx.x][dx];
+        if (x < nx && y < ny) {
+            const float2 v = tile[threadIdx.x][dx];
+            const size_t o = field_index(boff + ((size_t)x * nz + z) * ny + y, ppT);
+            fT[o] = v.x; fT[o + field_s_offset(ppT)] = v.y;
+        }
     }
 }
 
-cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat, float2 *PT,
+cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat, float2 *PT, int ppN, int ppT,
                                int nx, int ny, int nz, int nbins, cudaStream_t st)
 {
     dim3 grid((nx + 31) / 32, (ny + 31) / 32, nz * nbins), block(32, 8);
-    k_pack_fields<<<grid, block, 0, st>>>(kappa, S, Pnat, PT, nx, ny, nz);
+    k_pack_fields<<<grid, block, 0, st>>>(kappa, S, Pnat, PT, ppN, ppT, nx, ny, nz);
     return cudaGetLastError();
 }
 
@@ -195,7 +201,7 @@ k_sweep_generic(const SweepLaunch L, int np_max, int nq_max)
         if (g != L.group) return;
     }
     const long long foff = (long long)bin * L.ncell + D.base;
-    const float2 *__restrict__ P = L.P + foff;
+    const float *__restrict__ Pf = reinterpret_cast<const float *>(L.P);
     float *acc = L.acc + ((long long)slot * L.nbins) * L.ncell + foff;
     const float invL = (MODE == MODE_J) ? D.invL : 1.0f;
     const float Lw = 1.0f / D.invL;
@@ -233,7 +239,8 @@ k_sweep_generic(const SweepLaunch L, int np_max, int nq_max)
             const long long o = (long long)k * D.sk + ll * D.sl + (rev ? (D.Nb - 1 - jj) : jj);
             float v = 0.0f;
             if (MODE == MODE_J) {
-                const float2 ks = P[o];
+                const size_t fo = field_index((size_t)(foff + o), L.pp);
+                const float2 ks = make_float2(Pf[fo], Pf[fo + field_s_offset(L.pp)]);
                 float e;
                 const float A = one_minus_exp(ks.x, len, -len * 1.4426950408889634f, e);
                 v = I * A * invL;
@@ -267,7 +274,7 @@ cudaError_t launch_sweep_generic(const SweepLaunch &L, int np_max, int nq_max, c
 // transpose, of the transposed layout.
 // ------------------------------------------------------------------------------------------------
 template <bool COUNTS>
-__global__ void k_finalise(float *__restrict__ J, unsigned *__restrict__ counts, const float2 *__restrict__ Pnat,
+__global__ void k_finalise(float *__restrict__ J, unsigned *__restrict__ counts, const float2 *__restrict__ Pnat, int ppN,
                            const float *__restrict__ accN, const float *__restrict__ accNC, int slotsN,
                            const float *__restrict__ accT, const float *__restrict__ accTC, int slotsT,
                            int nx, int ny, int nz, int nbins, float inv_nd, int add_S)
@@ -297,7 +304,9 @@ __global__ void k_finalise(float *__restrict__ J, unsigned *__restrict__ counts,
             if (COUNTS) {
                 counts[i] = (unsigned)__float2uint_rn(s);
             } else {
-                const float2 ks = Pnat[i];
+                const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
+                const size_t o = field_index(i, ppN);
+                const float2 ks = make_float2(fN[o], fN[o + field_s_offset(ppN)]);
                 const float jin = s * inv_nd / ks.x;
                 J[i] = add_S ? jin + ks.y : jin;
             }
@@ -305,12 +314,12 @@ __global__ void k_finalise(float *__restrict__ J, unsigned *__restrict__ counts,
     }
 }
 
-cudaError_t launch_normalise(float *J, const float2 *Pnat, const float *accN, const float *accNC, int slotsN,
+cudaError_t launch_normalise(float *J, const float2 *Pnat, int ppN, const float *accN, const float *accNC, int slotsN,
                              const float *accT, const float *accTC, int slotsT,
                              int nx, int ny, int nz, int nbins, float inv_nd, int add_S, cudaStream_t st)
 {
     dim3 grid((nx + 31) / 32, (ny + 31) / 32, nz * nbins), block(32, 8);
-    k_finalise<false><<<grid, block, 0, st>>>(J, nullptr, Pnat, accN, accNC, slotsN, accT, accTC, slotsT,
+    k_finalise<false><<<grid, block, 0, st>>>(J, nullptr, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT,
                                               nx, ny, nz, nbins, inv_nd, add_S);
     return cudaGetLastError();
 }
@@ -320,7 +329,7 @@ cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const fl
                                    int nx, int ny, int nz, cudaStream_t st)
 {
     dim3 grid((nx + 31) / 32, (ny + 31) / 32, nz), block(32, 8);
-    k_finalise<true><<<grid, block, 0, st>>>(nullptr, counts, nullptr, accN, accNC, slotsN, accT, accTC, slotsT,
+    k_finalise<true><<<grid, block, 0, st>>>(nullptr, counts, nullptr, 0, accN, accNC, slotsN, accT, accTC, slotsT,
                                              nx, ny, nz, 1, 1.0f, 0);
     return cudaGetLastError();
 }

@@ -26,71 +26,94 @@
 namespace rt {
 
 // ------------------------------------------------------------------------------------------------
-// Segment update (eq. 7, eq. 8; PAPER.md:88-97), fp32
-//   A = 1 - exp(-kappa*len); contribution to the cell += I_in * A  (numerator of eq. 11 times kappa*L,
-//   see DESIGN.md "Arithmetic"); I_out = I_in * e + S * A with e = exp(-kappa*len).
+// Chunk vectors: the CW adjacent cells a lane owns in one chunk are one value of type VT<CW>::T, and
+// every arithmetic step of the segment update acts on the whole chunk.  For CW = 2 these are the
+// packed fp32x2 instructions of sm_100a (SASS FFMA2 / FMUL2 / FADD2: two IEEE fp32 results per
+// lane and issue slot, each rounded exactly like the scalar instruction).
 // ------------------------------------------------------------------------------------------------
+template <int CW> struct VT;
+template <> struct VT<1> { using T = float;  using D = float2; };    // T: chunk of values / accumulators, D: packed (kappa, S)
+template <> struct VT<2> { using T = float2; using D = float4; };
+
+__device__ __forceinline__ float  vmul(float a, float b) { return a * b; }
+__device__ __forceinline__ float2 vmul(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float  vadd(float a, float b) { return a + b; }
+__device__ __forceinline__ float2 vadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float  vfma(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ float2 vfma(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+template <class T> __device__ __forceinline__ T vsplat(float s);
+template <> __device__ __forceinline__ float  vsplat<float>(float s) { return s; }
+template <> __device__ __forceinline__ float2 vsplat<float2>(float s) { return make_float2(s, s); }
+
 __device__ __forceinline__ float ex2_approx(float x)
 {
     float y;
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+__device__ __forceinline__ float  vex2(float t) { return ex2_approx(t); }
+__device__ __forceinline__ float2 vex2(float2 t) { return make_float2(ex2_approx(t.x), ex2_approx(t.y)); }
+// per element: t > thr ? a : b
+__device__ __forceinline__ float  vsel_gt(float t, float thr, float a, float b) { return t > thr ? a : b; }
+__device__ __forceinline__ float2 vsel_gt(float2 t, float thr, float2 a, float2 b)
+{ return make_float2(t.x > thr ? a.x : b.x, t.y > thr ? a.y : b.y); }
 
-// e = exp(-kappa*len) and A = 1 - e, each with small RELATIVE error: e straight from ex2 (never as
-// 1 - A: behind an opaque cell the transmitted part I*e is all that is left), A from a polynomial
-// where 1 - e would cancel.
-__device__ __forceinline__ float one_minus_exp(float kap, float len, float ct, float &e)
+// element of a chunk at memory column 0 / CW-1, and the two ways a b-step moves a chunk's rays:
+// towards higher memory columns (a new ray enters column 0) or towards lower ones (enters column CW-1)
+__device__ __forceinline__ float vfirst(float v) { return v; }
+__device__ __forceinline__ float vfirst(float2 v) { return v.x; }
+__device__ __forceinline__ float vlast(float v) { return v; }
+__device__ __forceinline__ float vlast(float2 v) { return v.y; }
+__device__ __forceinline__ void vshift_up(float &v, float in) { v = in; }
+__device__ __forceinline__ void vshift_up(float2 &v, float in) { v.y = v.x; v.x = in; }
+__device__ __forceinline__ void vshift_down(float &v, float in) { v = in; }
+__device__ __forceinline__ void vshift_down(float2 &v, float in) { v.x = v.y; v.y = in; }
+
+__device__ __forceinline__ void unpack(const float2 &v, float &kap, float &src) { kap = v.x; src = v.y; }
+__device__ __forceinline__ void unpack(const float4 &v, float2 &kap, float2 &src)
+{ kap = make_float2(v.x, v.y); src = make_float2(v.z, v.w); }     // pair-packed layout (rt_internal.h)
+
+// ------------------------------------------------------------------------------------------------
+// Segment update (eq. 7, eq. 8; PAPER.md:88-97), fp32
+//   A = 1 - exp(-kappa*len); contribution to the cell += I_in * A  (numerator of eq. 11 times kappa*L,
+//   see DESIGN.md "Arithmetic"); I_out = I_in * e + S * A with e = exp(-kappa*len).
+// e and A each keep a small RELATIVE error: e straight from ex2 (never as 1 - A: behind an opaque
+// cell the transmitted part I*e is all that is left), A from a polynomial where 1 - e would cancel.
+// With t = kappa * ct, ct = -len*log2(e):  e = 2^t,  x = kappa*len = -t*ln2, and for x < 1/4
+//   A = x (c0 + c1 x + c2 x^2 + c3 x^3)  (fitted on [0, 1/4], rel. error 3.4e-7)
+//     = t (d0 + d1 t + d2 t^2 + d3 t^3),  d_k = c_k (-ln 2)^(k+1).
+// ------------------------------------------------------------------------------------------------
+template <class T>
+__device__ __forceinline__ T one_minus_exp(T kap, T ctv, T &e)
 {
-    const float x = kap * len;
-    e = ex2_approx(kap * ct);                                  // ct = -len*log2(e)
-    // small-x branch: x * (c0 + c1 x + c2 x^2 + c3 x^3), fitted on [0, 1/4]; rel. error 3.4e-7
-    float p = fmaf(x, -0.0377338513f, 0.1660640817f);
-    p = fmaf(x, p, -0.4999701648f);
-    p = fmaf(x, p, 0.9999997683f);
-    return x < 0.25f ? x * p : 1.0f - e;
+    const T t = vmul(kap, ctv);
+    e = vex2(t);
+    T p = vfma(t, vsplat<T>(-0.00871029682457447f), vsplat<T>(-0.055303432047367096f));
+    p = vfma(t, p, vsplat<T>(-0.24021217226982117f));
+    p = vfma(t, p, vsplat<T>(-0.6931470036506653f));
+    const T As = vmul(t, p);
+    const T Ab = vfma(e, vsplat<T>(-1.0f), vsplat<T>(1.0f));       // 1 - e, one rounding
+    return vsel_gt(t, -0.36067376022224085f, As, Ab);              // x < 1/4
 }
 
 // ND intensities (1, or 2 for a mirror pair) cross the same cell piece: e, A and S*A are shared.
-template <int MODE, int ND>
-__device__ __forceinline__ void seg_update(float (&I)[ND], float kap, float src, float len, float ct, float &part)
+template <int MODE, int ND, class T>
+__device__ __forceinline__ void seg_update(T (&I)[ND], T kap, T src, float len, T ctv, T &part)
 {
     if (MODE == MODE_J) {
-        float e;
-        const float A = one_minus_exp(kap, len, ct, e);
-        const float SA = src * A;
-        if (ND == 2) part = fmaf(I[0] + I[ND - 1], A, part);
-        else         part = fmaf(I[0], A, part);
+        T e;
+        const T A = one_minus_exp<T>(kap, ctv, e);
+        const T SA = vmul(src, A);
+        if (ND == 2) part = vfma(vadd(I[0], I[ND - 1]), A, part);
+        else         part = vfma(I[0], A, part);
 #pragma unroll
-        for (int d = 0; d < ND; ++d) I[d] = fmaf(I[d], e, SA);   // eq. 7
+        for (int d = 0; d < ND; ++d) I[d] = vfma(I[d], e, SA);   // eq. 7
     } else if (MODE == MODE_COUNT) {
-        part += (float)ND;
+        part = vadd(part, vsplat<T>((float)ND));
     } else {
-        part += (float)ND * len;
+        part = vadd(part, vsplat<T>((float)ND * len));
     }
 }
-
-template <int CW> struct VecT;
-template <> struct VecT<2> { using D = float4; using A = float2; };
-template <> struct VecT<1> { using D = float2; using A = float;  };
-
-template <int CW>
-__device__ __forceinline__ void unpack(const typename VecT<CW>::D &v, float (&kap)[CW], float (&src)[CW]);
-template <>
-__device__ __forceinline__ void unpack<2>(const float4 &v, float (&kap)[2], float (&src)[2])
-{ kap[0] = v.x; src[0] = v.y; kap[1] = v.z; src[1] = v.w; }
-template <>
-__device__ __forceinline__ void unpack<1>(const float2 &v, float (&kap)[1], float (&src)[1])
-{ kap[0] = v.x; src[0] = v.y; }
-
-template <int CW>
-__device__ __forceinline__ typename VecT<CW>::A acc_new(const typename VecT<CW>::A &o, const float (&part)[CW], float w);
-template <>
-__device__ __forceinline__ float2 acc_new<2>(const float2 &o, const float (&part)[2], float w)
-{ return make_float2(fmaf(part[0], w, o.x), fmaf(part[1], w, o.y)); }
-template <>
-__device__ __forceinline__ float acc_new<1>(const float &o, const float (&part)[1], float w)
-{ return fmaf(part[0], w, o); }
 
 constexpr int kWarpsPerCta = kOwnedWarpsPerCta;
 
@@ -111,56 +134,50 @@ constexpr int kPatD    = F_SB1 | F_SC1 | F_P1;
 //             offset.  Row R is the seam row (valid only if some piece steps along c).
 //   rowp[r] : this lane's position in the global accumulator row of ray row r (r = R: seam
 //             accumulator).  New accumulator values go straight to global memory (one writer per cell).
-//   I[r][g][i][d] : intensity of the ray currently in column i of chunk g of ray row r, direction d;
-//             i is in MEMORY order.
+//   I[r][g][d] : intensities of the rays currently in the CW columns of chunk g of ray row r,
+//             direction d; elements in MEMORY order.
 // ------------------------------------------------------------------------------------------------
 template <int CW, int G, int R, int MODE, int FLC, int V>
-__device__ __forceinline__ void slab_rows(const unsigned fl_rt, float (&I)[R][G][CW][(V == 2) ? 2 : 1],
+__device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>::T (&I)[R][G][(V == 2) ? 2 : 1],
                                           const unsigned char *__restrict__ sp, const unsigned char *__restrict__ sa,
                                           const float len0, const float len1, const float len2,
                                           const float Ibc, const float invL, const int lane, const int lwrap,
                                           float *const (&rowp)[R + 1])
 {
-    using DV = typename VecT<CW>::D;
-    using AV = typename VecT<CW>::A;
+    using T = typename VT<CW>::T;
+    using DV = typename VT<CW>::D;
     constexpr int ND = (V == 2) ? 2 : 1;
     constexpr bool REV = (V == 1);
     constexpr int kRowP = 32 * CW * G * (int)sizeof(float2), kRowA = 32 * CW * G * (int)sizeof(float);
     constexpr unsigned FULL = 0xffffffffu;
     constexpr float LOG2E = 1.4426950408889634f;
     const unsigned fl = (FLC >= 0) ? (unsigned)FLC : fl_rt;
-    const float ct0 = -len0 * LOG2E, ct1 = -len1 * LOG2E, ct2 = -len2 * LOG2E;
+    const T ct0 = vsplat<T>(-len0 * LOG2E), ct1 = vsplat<T>(-len1 * LOG2E), ct2 = vsplat<T>(-len2 * LOG2E);
+    const T invLv = vsplat<T>(invL);
     const bool anySC = (fl & (F_SC1 | F_SC2)) != 0;
     // memory chunk of canonical chunk g, as element offsets within a row
 #define RT_MG(g) ((REV ? (G - 1 - (g)) : (g)) * 32 * CW)
 
-    float part_cur[G][CW];
+    T part_cur[G];
 #pragma unroll
-    for (int g = 0; g < G; ++g)
-#pragma unroll
-        for (int i = 0; i < CW; ++i) part_cur[g][i] = 0.0f;
+    for (int g = 0; g < G; ++g) part_cur[g] = vsplat<T>(0.0f);
 
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         const bool wrap_r = (r == lwrap);
-        float part_next[G][CW];
-        float kc[G][CW], sc[G][CW], kn[G][CW], sn[G][CW];
+        T part_next[G];
+        T kc[G], sc[G], kn[G], sn[G];
 #pragma unroll
         for (int g = 0; g < G; ++g) {
-            unpack<CW>(*reinterpret_cast<const DV *>(sp + r * kRowP + RT_MG(g) * (int)sizeof(float2)), kc[g], sc[g]);
+            unpack(*reinterpret_cast<const DV *>(sp + r * kRowP + RT_MG(g) * (int)sizeof(float2)), kc[g], sc[g]);
             if (anySC)
-                unpack<CW>(*reinterpret_cast<const DV *>(sp + (r + 1) * kRowP + RT_MG(g) * (int)sizeof(float2)), kn[g], sn[g]);
-#pragma unroll
-            for (int i = 0; i < CW; ++i) {
-                part_next[g][i] = 0.0f;
-                if (!anySC) { kn[g][i] = kc[g][i]; sn[g][i] = sc[g][i]; }
-            }
+                unpack(*reinterpret_cast<const DV *>(sp + (r + 1) * kRowP + RT_MG(g) * (int)sizeof(float2)), kn[g], sn[g]);
+            else { kn[g] = kc[g]; sn[g] = sc[g]; }
+            part_next[g] = vsplat<T>(0.0f);
         }
-        float (&Ir)[G][CW][ND] = I[r];
+        T (&Ir)[G][ND] = I[r];
 #pragma unroll
-        for (int g = 0; g < G; ++g)
-#pragma unroll
-            for (int i = 0; i < CW; ++i) seg_update<MODE, ND>(Ir[g][i], kc[g][i], sc[g][i], len0, ct0, part_cur[g][i]);
+        for (int g = 0; g < G; ++g) seg_update<MODE, ND, T>(Ir[g], kc[g], sc[g], len0, ct0, part_cur[g]);
         bool sel = false;
 #pragma unroll
         for (int stage = 1; stage <= 2; ++stage) {
@@ -168,7 +185,7 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, float (&I)[R][G]
             const unsigned fsc = (stage == 1) ? F_SC1 : F_SC2;
             const unsigned fp = (stage == 1) ? F_P1 : F_P2;
             const float len = (stage == 1) ? len1 : len2;
-            const float ct = (stage == 1) ? ct1 : ct2;
+            const T ct = (stage == 1) ? ct1 : ct2;
             if (fl & (fsb | fsc)) {
                 if (MODE == MODE_J) {
                     if (fl & fsb) {
@@ -178,23 +195,22 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, float (&I)[R][G]
                         float carry = Ibc;
 #pragma unroll
                         for (int g = 0; g < G; ++g) {
-                            const float out = REV ? Ir[g][0][0] : Ir[g][CW - 1][0];
+                            const float out = REV ? vfirst(Ir[g][0]) : vlast(Ir[g][0]);
                             const float t = __shfl_sync(FULL, out, (lane + 31) & 31);
                             const float in = (lane == 0) ? carry : t;
                             carry = t;
-                            if (REV) { if (CW == 2) Ir[g][0][0] = Ir[g][CW - 1][0]; Ir[g][CW - 1][0] = in; }
-                            else     { if (CW == 2) Ir[g][CW - 1][0] = Ir[g][0][0]; Ir[g][0][0] = in; }
+                            if (REV) vshift_down(Ir[g][0], in);
+                            else     vshift_up(Ir[g][0], in);
                         }
                         if (ND == 2) {
                             // mirrored direction: towards lower columns; a new ray enters the last column
                             carry = Ibc;
 #pragma unroll
                             for (int g = G - 1; g >= 0; --g) {
-                                const float t = __shfl_sync(FULL, Ir[g][0][ND - 1], (lane + 1) & 31);
+                                const float t = __shfl_sync(FULL, vfirst(Ir[g][ND - 1]), (lane + 1) & 31);
                                 const float in = (lane == 31) ? carry : t;
                                 carry = t;
-                                if (CW == 2) Ir[g][0][ND - 1] = Ir[g][CW - 1][ND - 1];
-                                Ir[g][CW - 1][ND - 1] = in;
+                                vshift_down(Ir[g][ND - 1], in);
                             }
                         }
                     }
@@ -202,39 +218,33 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, float (&I)[R][G]
 #pragma unroll
                         for (int g = 0; g < G; ++g)
 #pragma unroll
-                            for (int i = 0; i < CW; ++i)
-#pragma unroll
-                                for (int d = 0; d < ND; ++d) Ir[g][i][d] = Ibc;
+                            for (int d = 0; d < ND; ++d) Ir[g][d] = vsplat<T>(Ibc);
                     }
                 }
                 if (fl & fsc) sel = true;
             }
             if (fl & fp) {
 #pragma unroll
-                for (int g = 0; g < G; ++g)
-#pragma unroll
-                    for (int i = 0; i < CW; ++i) {
-                        if (sel) seg_update<MODE, ND>(Ir[g][i], kn[g][i], sn[g][i], len, ct, part_next[g][i]);
-                        else     seg_update<MODE, ND>(Ir[g][i], kc[g][i], sc[g][i], len, ct, part_cur[g][i]);
-                    }
+                for (int g = 0; g < G; ++g) {
+                    if (sel) seg_update<MODE, ND, T>(Ir[g], kn[g], sn[g], len, ct, part_next[g]);
+                    else     seg_update<MODE, ND, T>(Ir[g], kc[g], sc[g], len, ct, part_cur[g]);
+                }
             }
         }
         // row r's partial is complete (own pieces + pieces of ray row r-1 that stepped along c)
 #pragma unroll
         for (int g = 0; g < G; ++g)
-            *reinterpret_cast<AV *>(rowp[r] + RT_MG(g)) =
-                acc_new<CW>(*reinterpret_cast<const AV *>(sa + r * kRowA + RT_MG(g) * (int)sizeof(float)), part_cur[g], invL);
+            *reinterpret_cast<T *>(rowp[r] + RT_MG(g)) =
+                vfma(part_cur[g], invLv, *reinterpret_cast<const T *>(sa + r * kRowA + RT_MG(g) * (int)sizeof(float)));
 #pragma unroll
-        for (int g = 0; g < G; ++g)
-#pragma unroll
-            for (int i = 0; i < CW; ++i) part_cur[g][i] = part_next[g][i];
+        for (int g = 0; g < G; ++g) part_cur[g] = part_next[g];
     }
     if (anySC) {
         // seam: the partial of the memory row above the warp's last ray row has another owner
 #pragma unroll
         for (int g = 0; g < G; ++g)
-            *reinterpret_cast<AV *>(rowp[R] + RT_MG(g)) =
-                acc_new<CW>(*reinterpret_cast<const AV *>(sa + R * kRowA + RT_MG(g) * (int)sizeof(float)), part_cur[g], invL);
+            *reinterpret_cast<T *>(rowp[R] + RT_MG(g)) =
+                vfma(part_cur[g], invLv, *reinterpret_cast<const T *>(sa + R * kRowA + RT_MG(g) * (int)sizeof(float)));
     }
 #undef RT_MG
 }
@@ -363,15 +373,13 @@ k_sweep_tma(const SweepLaunch L)
 #pragma unroll 1
     for (int kk = 0; kk < D && kk < Na; ++kk) produce(kk);
 
-    float I[R][G][CW][ND];
+    typename VT<CW>::T I[R][G][ND];
 #pragma unroll
     for (int r = 0; r < R; ++r)
 #pragma unroll
         for (int g = 0; g < G; ++g)
 #pragma unroll
-            for (int i = 0; i < CW; ++i)
-#pragma unroll
-                for (int d = 0; d < ND; ++d) I[r][g][i][d] = Ibc;
+            for (int d = 0; d < ND; ++d) I[r][g][d] = vsplat<typename VT<CW>::T>(Ibc);
 
     // this lane's first memory column (canonical chunk 0 is memory chunk G-1 when REV)
     const int lcol = CW * (REV ? 31 - lane : lane);
