@@ -49,7 +49,7 @@ struct rt_ctx {
     // singles[l] everything that has no partner (zero b slope, or an unsymmetric user set)
     std::vector<int> pairs[2], singles[2];
     bool pair_enable = true;
-    int hint = 0;
+    int handoff = 0;
     int slots_pair[2] = {0, 0}, slots_single[2] = {0, 0};
     bool fast[2] = {false, false};   // owned kernel usable for the layout
     int pp[2] = {0, 0};              // packed field of the layout is pair-packed (rt_internal.h)
@@ -207,7 +207,8 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     auto by_class = [&](int x, int y) {
         if (c->hd[x].a != c->hd[y].a) return c->hd[x].a < c->hd[y].a;
         if (c->hd[x].refl[c->hd[x].a] != c->hd[y].refl[c->hd[y].a]) return c->hd[x].refl[c->hd[x].a] < c->hd[y].refl[c->hd[y].a];
-        if (c->hd[x].refl[c->hd[x].b] != c->hd[y].refl[c->hd[y].b]) return c->hd[x].refl[c->hd[x].b] < c->hd[y].refl[c->hd[y].b];
+        const int rx = c->hd[x].Mb == 0 ? 0 : c->hd[x].refl[c->hd[x].b], ry = c->hd[y].Mb == 0 ? 0 : c->hd[y].refl[c->hd[y].b];
+        if (rx != ry) return rx < ry;
         return c->hd[x].work > c->hd[y].work;
     };
     for (int l = 0; l < 2; ++l) std::stable_sort(c->order[l].begin(), c->order[l].end(), by_class);
@@ -277,10 +278,10 @@ extern "C" int rt_tune(rt_ctx *c, const char *key, int value)
     if (!c || !key) return RT_EINVAL;
     if (c->buffers_ready) return RT_ESTATE;
     if (!strcmp(key, "slots")) { if (value < 1 || value > 4096) return RT_EINVAL; c->slots_req = value; return RT_OK; }
-    if (!strcmp(key, "stages")) { if (!(value >= 2 && value <= 4)) return RT_EINVAL; c->stages = value; return RT_OK; }
-    if (!strcmp(key, "l2hint")) { if (value < 0 || value > 3) return RT_EINVAL; c->hint = value; return RT_OK; }
+    if (!strcmp(key, "stages")) { if (!(value >= 2 && value <= 3) || (c->handoff && value != 2)) return RT_EINVAL; c->stages = value; return RT_OK; }
+    if (!strcmp(key, "handoff")) { if ((value != 0 && value != 1) || (value && c->stages != 2)) return RT_EINVAL; c->handoff = value; return RT_OK; }
     if (!strcmp(key, "pair")) { if (value != 0 && value != 1) return RT_EINVAL; c->pair_enable = value != 0; return RT_OK; }
-    if (!strcmp(key, "rows")) { if (!(value == 1 || value == 2 || value == 4)) return RT_EINVAL; c->rows = value; return RT_OK; }
+    if (!strcmp(key, "rows")) { if (!(value == 1 || value == 2)) return RT_EINVAL; c->rows = value; return RT_OK; }
     return RT_EINVAL;
 }
 
@@ -395,7 +396,7 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
         memset(&L, 0, sizeof(L));
         L.P = c->d_P[l]; L.acc = c->d_acc[l]; L.accC = c->d_accC[l];
         L.dirs = c->d_dirs; L.prog = c->d_prog; L.nbins = nbins; L.ncell = c->ncell; L.Ibc = c->d_Ibc;
-        L.rows = rows_for(c, l); L.mode = mode; L.stages = c->stages; L.hint = c->hint;
+        L.rows = rows_for(c, l); L.mode = mode; L.stages = c->stages; L.handoff = c->handoff;
         L.Nb = (l == 0) ? c->nx : c->ny; L.pp = c->pp[l];
         const bool owned_l = c->fast[l];
         // the lists this traversal walks: (direction list, position in d_batch, slots per launch, paired)
@@ -417,11 +418,13 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
             // batches never mix dominant axes (Nc differs between y- and z-dominant directions)
             int i = 0;
             while (i < nl) {
+                // march sense along b: irrelevant for a zero b-slope (no ray ever changes column), so those
+                // directions join forward batches whatever their sign
+                auto eff_rev = [&](int d) { return c->hd[d].Mb == 0 ? 0 : c->hd[d].refl[c->hd[d].b]; };
                 const int a = c->hd[list[i]].a;
-                const int rev = c->hd[list[i]].refl[c->hd[list[i]].b];
+                const int rev = eff_rev(list[i]);
                 int n = 0;
-                while (i + n < nl && n < S && c->hd[list[i + n]].a == a &&
-                       c->hd[list[i + n]].refl[c->hd[list[i + n]].b] == rev) ++n;
+                while (i + n < nl && n < S && c->hd[list[i + n]].a == a && eff_rev(list[i + n]) == rev) ++n;
                 int first = i, count = n;
                 if (only_dir >= 0) {
                     if (list[i] != only_dir) { i += 1; continue; }

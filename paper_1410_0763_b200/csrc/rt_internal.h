@@ -53,10 +53,10 @@ struct SweepLaunch {
     int variant;             // generic kernel: 0 = four groups (one launch per group), 1 = atomics
     int group;               // generic kernel: group id 0..3
     int stages;              // owned kernel: depth of the TMA shared-memory ring (2..4)
-    int hint;                // owned TMA kernel: bit 0 = field rows evict_last in L2, bit 1 = accumulator rows evict_first
     int rev;                 // owned kernel, single directions: all slots have a reflected b component (sj < 0)
     int pair;                // owned TMA kernel, MODE_J: every slot carries a direction and its b-mirror (rt_kernels.cu "mirror pairs")
     int pp;                  // P is pair-packed (below)
+    int handoff;             // owned kernel: seam partials are handed to the next warp of the CTA in shared memory (ablation)
 };
 
 // Packed-field layouts.  Interleaved: float2 (kappa, S) per cell.  Pair-packed (layouts swept by the

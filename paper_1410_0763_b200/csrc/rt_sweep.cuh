@@ -11,9 +11,12 @@
 // inflow intensity enters the first column).  Along c the warp owns RAYS: the memory row of ray
 // row r is (q0 + r + shift_k) mod Nc, pure address arithmetic; pieces that fall into the next
 // memory row use the next row's data and add to the next row's partial, both held by the same
-// thread.  Only the partial of the row above the warp's last ray row has another owner; it goes
-// to the seam accumulator accC with plain stores.  Every cell therefore has exactly one writer
-// per accumulator array and launch: no atomics, deterministic sums.
+// thread.  Only the partial of the row above the warp's last ray row (the "seam") has another
+// owner; it goes to the seam accumulator accC in global memory with plain stores (or, with the
+// "handoff" ablation, into the next warp's staged accumulator row in shared memory, announced
+// through an mbarrier; rows are processed top-down, so it is ready early in a slab and needed at
+// its end).  Every cell therefore has exactly one writer per accumulator array and launch: no
+// atomics on the data path, deterministic sums.
 //
 // Variants (template parameter V):
 //   V = 0  one direction per warp, rays move towards higher memory columns
@@ -127,22 +130,50 @@ constexpr int kPatCB   = F_SC1 | F_P1 | F_SB2 | F_P2;
 constexpr int kPatD    = F_SB1 | F_SC1 | F_P1;
 
 // ------------------------------------------------------------------------------------------------
-// One slab for the R ray rows of a warp, stage-major: every chunk does piece 0, then the step, then
-// piece 1, ... (a mirror pair needs its chunk-to-chunk carries in both chunk orders).
-//   sp / sa : this lane's position in row 0 of the stage's packed-field rows / accumulator rows
-//             (shared memory); row r is at + r * kRowP / kRowA, canonical chunk g at a compile-time
-//             offset.  Row R is the seam row (valid only if some piece steps along c).
+// mbarrier helpers used inside the slab body (the rest of the TMA helpers are further down)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@!p bra WAIT_%=;\n\t}"
+        :: "r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar)
+{ asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory"); }
+
+// who owns the rows around this warp's tile (warp-uniform)
+struct Seam {
+    bool first;          // first warp of the CTA: nobody hands a seam partial in (the CTA below wrote it to accC)
+    bool last;           // last active warp of the CTA: the seam partial goes to accC in global memory
+    unsigned bar_out;    // mbarrier on which this warp announces its seam partial (if !last)
+    unsigned bar_in;     // mbarrier on which the warp below announces its seam partial (if !first)
+    unsigned par_in;     // parity to wait for on bar_in
+    unsigned char *up;   // this lane's position in the next warp's staged old-accumulator row 0 (if !last)
+};
+
+// ------------------------------------------------------------------------------------------------
+// One slab for the R ray rows of a warp, rows top-down (r = R-1 ... 0), stage-major within a row:
+// every chunk does piece 0, then the step, then piece 1, ... (a mirror pair needs its
+// chunk-to-chunk carries in both chunk orders).
+//   sp / sa : this lane's position in the warp's row 0 of the stage's packed-field rows / old
+//             accumulator rows (shared memory); row r is at + r * kRowP / kRowA, canonical chunk g
+//             at a compile-time offset.  Row R is the seam row = row 0 of the next warp (valid only
+//             if some piece steps along c).
 //   rowp[r] : this lane's position in the global accumulator row of ray row r (r = R: seam
-//             accumulator).  New accumulator values go straight to global memory (one writer per cell).
+//             accumulator, used by the CTA's last warp).  New accumulator values go straight to
+//             global memory (one writer per cell).
 //   I[r][g][d] : intensities of the rays currently in the CW columns of chunk g of ray row r,
 //             direction d; elements in MEMORY order.
 // ------------------------------------------------------------------------------------------------
 template <int CW, int G, int R, int MODE, int FLC, int V>
 __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>::T (&I)[R][G][(V == 2) ? 2 : 1],
-                                          const unsigned char *__restrict__ sp, const unsigned char *__restrict__ sa,
+                                          const unsigned char *__restrict__ sp, unsigned char *__restrict__ sa,
                                           const float len0, const float len1, const float len2,
                                           const float Ibc, const float invL, const int lane, const int lwrap,
-                                          float *const (&rowp)[R + 1])
+                                          float *const (&rowp)[R + 1], const Seam &seam)
 {
     using T = typename VT<CW>::T;
     using DV = typename VT<CW>::D;
@@ -157,15 +188,16 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
     const bool anySC = (fl & (F_SC1 | F_SC2)) != 0;
     // memory chunk of canonical chunk g, as element offsets within a row
 #define RT_MG(g) ((REV ? (G - 1 - (g)) : (g)) * 32 * CW)
+#define RT_OLD(r, g) (*reinterpret_cast<T *>(sa + (r) * kRowA + RT_MG(g) * (int)sizeof(float)))
 
-    T part_cur[G];
+    T part_hi[G];                 // partial of memory row r + 1
 #pragma unroll
-    for (int g = 0; g < G; ++g) part_cur[g] = vsplat<T>(0.0f);
+    for (int g = 0; g < G; ++g) part_hi[g] = vsplat<T>(0.0f);
 
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
+    for (int r = R - 1; r >= 0; --r) {
         const bool wrap_r = (r == lwrap);
-        T part_next[G];
+        T part_lo[G];             // partial of memory row r
         T kc[G], sc[G], kn[G], sn[G];
 #pragma unroll
         for (int g = 0; g < G; ++g) {
@@ -173,11 +205,11 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
             if (anySC)
                 unpack(*reinterpret_cast<const DV *>(sp + (r + 1) * kRowP + RT_MG(g) * (int)sizeof(float2)), kn[g], sn[g]);
             else { kn[g] = kc[g]; sn[g] = sc[g]; }
-            part_next[g] = vsplat<T>(0.0f);
+            part_lo[g] = vsplat<T>(0.0f);
         }
         T (&Ir)[G][ND] = I[r];
 #pragma unroll
-        for (int g = 0; g < G; ++g) seg_update<MODE, ND, T>(Ir[g], kc[g], sc[g], len0, ct0, part_cur[g]);
+        for (int g = 0; g < G; ++g) seg_update<MODE, ND, T>(Ir[g], kc[g], sc[g], len0, ct0, part_lo[g]);
         bool sel = false;
 #pragma unroll
         for (int stage = 1; stage <= 2; ++stage) {
@@ -226,26 +258,45 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
             if (fl & fp) {
 #pragma unroll
                 for (int g = 0; g < G; ++g) {
-                    if (sel) seg_update<MODE, ND, T>(Ir[g], kn[g], sn[g], len, ct, part_next[g]);
-                    else     seg_update<MODE, ND, T>(Ir[g], kc[g], sc[g], len, ct, part_cur[g]);
+                    if (sel) seg_update<MODE, ND, T>(Ir[g], kn[g], sn[g], len, ct, part_hi[g]);
+                    else     seg_update<MODE, ND, T>(Ir[g], kc[g], sc[g], len, ct, part_lo[g]);
                 }
             }
         }
-        // row r's partial is complete (own pieces + pieces of ray row r-1 that stepped along c)
+        // memory row r + 1 is complete: its own pieces (previous iteration) + the pieces of ray row r
+        // that stepped along c
+        if (r == R - 1) {
+            if (anySC) {
+                if (seam.last) {
+                    // the row above the CTA's tile has another owner: seam accumulator, plain stores
 #pragma unroll
-        for (int g = 0; g < G; ++g)
-            *reinterpret_cast<T *>(rowp[r] + RT_MG(g)) =
-                vfma(part_cur[g], invLv, *reinterpret_cast<const T *>(sa + r * kRowA + RT_MG(g) * (int)sizeof(float)));
+                    for (int g = 0; g < G; ++g)
+                        *reinterpret_cast<T *>(rowp[R] + RT_MG(g)) = vfma(part_hi[g], invLv, RT_OLD(R, g));
+                } else {
+                    // row 0 of the next warp: add into its staged old-accumulator row and announce it
 #pragma unroll
-        for (int g = 0; g < G; ++g) part_cur[g] = part_next[g];
+                    for (int g = 0; g < G; ++g) {
+                        T *o = reinterpret_cast<T *>(seam.up + RT_MG(g) * (int)sizeof(float));
+                        *o = vfma(part_hi[g], invLv, *o);
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(seam.bar_out);
+                }
+            }
+        } else {
+#pragma unroll
+            for (int g = 0; g < G; ++g)
+                *reinterpret_cast<T *>(rowp[r + 1] + RT_MG(g)) = vfma(part_hi[g], invLv, RT_OLD(r + 1, g));
+        }
+#pragma unroll
+        for (int g = 0; g < G; ++g) part_hi[g] = part_lo[g];
     }
-    if (anySC) {
-        // seam: the partial of the memory row above the warp's last ray row has another owner
+    // memory row 0: own pieces + the seam partial the warp below added to the staged row
+    if (anySC && !seam.first) mbar_wait(seam.bar_in, seam.par_in);
 #pragma unroll
-        for (int g = 0; g < G; ++g)
-            *reinterpret_cast<T *>(rowp[R] + RT_MG(g)) =
-                vfma(part_cur[g], invLv, *reinterpret_cast<const T *>(sa + R * kRowA + RT_MG(g) * (int)sizeof(float)));
-    }
+    for (int g = 0; g < G; ++g)
+        *reinterpret_cast<T *>(rowp[0] + RT_MG(g)) = vfma(part_hi[g], invLv, RT_OLD(0, g));
+#undef RT_OLD
 #undef RT_MG
 }
 
@@ -269,15 +320,6 @@ __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
 { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory"); }
 __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
 { asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory"); }
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
-{
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@!p bra WAIT_%=;\n\t}"
-        :: "r"(bar), "r"(parity) : "memory");
-}
 __device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned bar)
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -286,7 +328,7 @@ __device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned
 
 // Row bookkeeping of one march, advanced slab by slab with adds only:
 //   frac = fractional part of 1/2 + k*m_c in units of 2^-20 (m_c = Mc / 2^20 <= 1)
-//   lb   = (q0 + floor(1/2 + k*m_c)) mod Nc : memory row of the warp's first ray row at slab k
+//   lb   = (q0 + floor(1/2 + k*m_c)) mod Nc : memory row of the first ray row at slab k
 //   offk = k * sk                            : element offset of slab k
 struct RowState {
     int lb, offk;
@@ -302,35 +344,46 @@ struct RowState {
     }
 };
 
-template <int CW, int G, int R>
+// Shared memory of a warp: D stages, each the packed-field rows and the old accumulator rows of one
+// slab for the warp's R ray rows plus the seam row above them; then the warp's mbarriers.
+template <int CW, int G, int R, int D>
 struct StageGeom {
     static constexpr int kNb = 32 * CW * G;
     static constexpr int kRowP = kNb * (int)sizeof(float2);
     static constexpr int kRowA = kNb * (int)sizeof(float);
     static constexpr int kStage = (R + 1) * (kRowP + kRowA);
+    static constexpr int kBarFull = D * kStage;               // D mbarriers: stage filled (transaction bytes)
+    static constexpr int kBarHand = kBarFull + 32;            // D mbarriers: this warp's seam partial of stage s added
+    static constexpr int kLanded = kBarHand + 32;             // int: 1 + last slab whose rows this warp has seen landed
+    static constexpr int kWarpBytes = D * kStage + 128;
+    static_assert(D <= 4, "barrier block holds 4 stages");
 };
 
-// Each warp owns D stages; stage (k mod D) holds slab k's packed field rows and old accumulator
-// rows, copied by bulk async copies (SASS UBLKCP) issued by lane 0 D slabs ahead and tracked by one
-// mbarrier per stage (transaction-byte count).  No registers are spent on data in flight, so the
-// prefetch depth is set by shared memory, not by the register file.
-template <int CW, int G, int R, int MODE, int D, int V>
-__global__ void __launch_bounds__(32 * kWarpsPerCta)
+// Each warp owns a private ring of D stages; stage (k mod D) holds slab k's packed field rows and old
+// accumulator rows, copied by bulk async copies (SASS UBLKCP) issued by lane 0 D slabs ahead and
+// tracked by one mbarrier per stage (transaction-byte count).  No registers are spent on data in
+// flight, so the prefetch depth is set by shared memory.  With HO (rt_tune "handoff", a
+// measured ablation, off by default) warps meet on slabs with a step along c, where warp w adds its
+// seam partial into the staged row 0 of warp w + 1 instead of the seam accumulator: 17 % less DRAM
+// traffic, but the warps of a CTA are forced into near lock-step and the sweep gets slower.
+template <int CW, int G, int R, int MODE, int D, int V, int W, bool HO>
+__global__ void __launch_bounds__(32 * W)
 k_sweep_tma(const SweepLaunch L)
 {
-    using SG = StageGeom<CW, G, R>;
+    using SG = StageGeom<CW, G, R, D>;
+    using T = typename VT<CW>::T;
     constexpr int ND = (V == 2) ? 2 : 1;
     constexpr bool REV = (V == 1);
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    constexpr int kWarpBytes = D * SG::kStage + 128;
 
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int slot = blockIdx.y, bin = blockIdx.z;
     const DirDev *__restrict__ Dp = L.dirs + L.batch[slot];
     const int Nc = Dp->Nc, Na = Dp->Na, Mc = Dp->Mc;
-    const int q0 = (blockIdx.x * kWarpsPerCta + wid) * R;
-    if (q0 >= Nc) return;
-    const int sk = (int)Dp->sk, sl = (int)Dp->sl;        // |offsets| < 2^31: checked by rt_create
+    const int q0c = blockIdx.x * (W * R);                        // first ray row of the CTA (grid.x covers Nc)
+    const int nact = min(W, (Nc - q0c) / R);                     // warps of this CTA that own rows (Nc % R == 0)
+    const int q0 = q0c + wid * R;
+    const int sk = (int)Dp->sk, sl = (int)Dp->sl;                // |offsets| < 2^31: checked by rt_create
     const float invL = (MODE == MODE_J) ? Dp->invL : 1.0f;
     const float Ibc = L.Ibc[bin];
     const SlabProg *__restrict__ prog = L.prog + Dp->prog_off;
@@ -340,32 +393,41 @@ k_sweep_tma(const SweepLaunch L)
     float *__restrict__ acc = L.acc + ((long long)slot * L.nbins) * L.ncell + foff;
     float *__restrict__ accC = L.accC + ((long long)slot * L.nbins) * L.ncell + foff;
 
-    unsigned char *wbase = smem_raw + wid * kWarpBytes;
+    unsigned char *wbase = smem_raw + wid * SG::kWarpBytes;
     const unsigned wbase_s = smem_u32(wbase);
-    const unsigned bars = wbase_s + D * SG::kStage;
+    const unsigned bars = wbase_s + SG::kBarFull;
     if (lane == 0) {
 #pragma unroll
-        for (int s = 0; s < D; ++s) mbar_init(bars + 8 * s, 1);
+        for (int s = 0; s < D; ++s) { mbar_init(bars + 8 * s, 1); mbar_init(wbase_s + SG::kBarHand + 8 * s, 1); }
+        *reinterpret_cast<volatile int *>(wbase + SG::kLanded) = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    __syncwarp();
+    __syncthreads();                                             // every warp's barriers exist before a neighbour touches them
+    if (wid >= nact) return;
 
-    // producer (lane 0): ask the TMA engine for the rows of the slab described by `ps` into stage s
+    Seam seam;
+    seam.first = !HO || (wid == 0);
+    seam.last = !HO || (wid == nact - 1);
+
+    // producer (lane 0): ask the TMA engine for the rows of the slab described by `ps` into stage s.
+    // The seam row's old accumulator is needed only by the CTA's last warp (the others add their seam
+    // partial into the next warp's stage).
     RowState ps;
     ps.init(q0);
     auto produce = [&](int s) {
         if (lane == 0) {
             const unsigned st = wbase_s + s * SG::kStage, bar = bars + 8 * s;
-            const bool seam = ps.steps(Mc);
-            const int nrows = R + (seam ? 1 : 0);
-            mbar_expect_tx(bar, (unsigned)(nrows * ((MODE == MODE_J ? SG::kRowP : 0) + SG::kRowA)));
+            const bool stp = ps.steps(Mc);
+            const int nP = (MODE == MODE_J) ? R + (stp ? 1 : 0) : 0;
+            const int nA = R + ((stp && seam.last) ? 1 : 0);
+            mbar_expect_tx(bar, (unsigned)(nP * SG::kRowP + nA * SG::kRowA));
 #pragma unroll
             for (int r = 0; r <= R; ++r) {
-                if (r == R && !seam) break;
                 int l = ps.lb + r; if (l >= Nc) l -= Nc;
                 const int o = ps.offk + l * sl;
-                if (MODE == MODE_J) bulk_g2s(st + r * SG::kRowP, P + o, SG::kRowP, bar);
-                bulk_g2s(st + (R + 1) * SG::kRowP + r * SG::kRowA, (r < R ? acc : accC) + o, SG::kRowA, bar);
+                // packed rows: 2 floats per cell in either packed layout, rows start at even cells
+                if (r < nP) bulk_g2s(st + r * SG::kRowP, P + o, SG::kRowP, bar);
+                if (r < nA) bulk_g2s(st + (R + 1) * SG::kRowP + r * SG::kRowA, (r < R ? acc : accC) + o, SG::kRowA, bar);
             }
         }
         ps.advance(Mc, Nc, sk);
@@ -373,20 +435,23 @@ k_sweep_tma(const SweepLaunch L)
 #pragma unroll 1
     for (int kk = 0; kk < D && kk < Na; ++kk) produce(kk);
 
-    typename VT<CW>::T I[R][G][ND];
+    T I[R][G][ND];
 #pragma unroll
     for (int r = 0; r < R; ++r)
 #pragma unroll
         for (int g = 0; g < G; ++g)
 #pragma unroll
-            for (int d = 0; d < ND; ++d) I[r][g][d] = vsplat<typename VT<CW>::T>(Ibc);
+            for (int d = 0; d < ND; ++d) I[r][g][d] = vsplat<T>(Ibc);
 
     // this lane's first memory column (canonical chunk 0 is memory chunk G-1 when REV)
     const int lcol = CW * (REV ? 31 - lane : lane);
     const unsigned char *lane_p = wbase + lcol * (int)sizeof(float2);
-    const unsigned char *lane_a = wbase + (R + 1) * SG::kRowP + lcol * (int)sizeof(float);
+    unsigned char *lane_a = wbase + (R + 1) * SG::kRowP + lcol * (int)sizeof(float);
     float *const acc_l = acc + lcol;
     float *const accC_l = accC + lcol;
+    volatile int *const landed_own = reinterpret_cast<volatile int *>(wbase + SG::kLanded);
+    volatile int *const landed_up = reinterpret_cast<volatile int *>(wbase + SG::kWarpBytes + SG::kLanded);
+    unsigned hand_par = 0;               // bit s: parity of the next completion of the incoming barrier of stage s
 
     RowState cs;
     cs.init(q0);
@@ -407,11 +472,27 @@ k_sweep_tma(const SweepLaunch L)
         }
         const int lwrap = Nc - 1 - cs.lb;
         const unsigned char *sp = lane_p + s * SG::kStage;
-        const unsigned char *sa = lane_a + s * SG::kStage;
+        unsigned char *sa = lane_a + s * SG::kStage;
+        const bool anySC = (fl & (F_SC1 | F_SC2)) != 0;
+        seam.bar_out = wbase_s + SG::kBarHand + 8 * s;
+        seam.bar_in = wbase_s - SG::kWarpBytes + SG::kBarHand + 8 * s;
+        seam.par_in = (hand_par >> s) & 1u;
+        seam.up = sa + SG::kWarpBytes;
+        if (anySC && !seam.first) hand_par ^= (1u << s);
         mbar_wait(bars + 8 * s, phase);
-        RT_DISPATCH_SLAB(fl, fl, I, sp, sa, len0, len1, len2, Ibc, invL, lane, lwrap, rowp)
-        __syncwarp();                     // every lane is done reading stage s
-        if (k + D < Na) produce(s);
+        if (!seam.first && lane == 0) *landed_own = k + 1;
+        if (anySC && !seam.last) {
+            // the next warp's stage s must hold slab k before this warp adds its seam partial to it.  That
+            // warp cannot pass slab k without the partial, so "has seen slab k land" is exactly landed == k + 1.
+            while (*landed_up < k + 1) { }
+            mbar_wait(bars + SG::kWarpBytes + 8 * s, phase);     // acquire the copy's writes
+        }
+        RT_DISPATCH_SLAB(fl, fl, I, sp, sa, len0, len1, len2, Ibc, invL, lane, lwrap, rowp, seam)
+        __syncwarp();                     // every lane is done with stage s
+        if (k + D < Na) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            produce(s);
+        }
         cs.advance(Mc, Nc, sk);
         if (++s == D) { s = 0; phase ^= 1u; }
     }
@@ -420,19 +501,29 @@ k_sweep_tma(const SweepLaunch L)
 // ------------------------------------------------------------------------------------------------
 // Launchers for one width Nb = 32*CW*G (instantiated in rt_sweep_nb*.cu)
 // ------------------------------------------------------------------------------------------------
-template <int CW, int G, int R, int D>
-constexpr int sweep_smem_bytes() { return kWarpsPerCta * (D * StageGeom<CW, G, R>::kStage + 128); }
+constexpr int kW = kOwnedWarpsPerCta;
+
+template <int CW, int G, int R, int MODE, int D, int V, bool HO>
+static cudaError_t launch_tma_ho(const SweepLaunch &L, dim3 grid, cudaStream_t st)
+{
+    constexpr int smem = kW * StageGeom<CW, G, R, D>::kWarpBytes;
+    if (smem > 227 * 1024) return cudaErrorInvalidValue;
+    auto kern = k_sweep_tma<CW, G, R, MODE, D, V, kW, HO>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, dim3(32 * kW), smem, st>>>(L);
+    return cudaGetLastError();
+}
 
 template <int CW, int G, int R, int MODE, int D, int V>
 static cudaError_t launch_tma(const SweepLaunch &L, dim3 grid, cudaStream_t st)
 {
-    constexpr int smem = sweep_smem_bytes<CW, G, R, D>();
-    if (smem > 227 * 1024) return cudaErrorInvalidValue;
-    auto kern = k_sweep_tma<CW, G, R, MODE, D, V>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    kern<<<grid, dim3(32 * kWarpsPerCta), smem, st>>>(L);
-    return cudaGetLastError();
+    if constexpr (D == 2) {                       // the handoff ablation exists for the default depth only
+        if (L.handoff) return launch_tma_ho<CW, G, R, MODE, D, V, true>(L, grid, st);
+    } else {
+        if (L.handoff) return cudaErrorInvalidValue;
+    }
+    return launch_tma_ho<CW, G, R, MODE, D, V, false>(L, grid, st);
 }
 
 template <int CW, int G, int R, int MODE, int D>
@@ -449,14 +540,12 @@ static cudaError_t launch_variant(const SweepLaunch &L, dim3 grid, cudaStream_t 
 template <int CW, int G, int R>
 static cudaError_t launch_rows(const SweepLaunch &L, cudaStream_t st)
 {
-    const int tiles = L.Nc / R;
-    const dim3 grid((tiles + kWarpsPerCta - 1) / kWarpsPerCta, L.nslots, L.nbins);
+    const dim3 grid((L.Nc + kW * R - 1) / (kW * R), L.nslots, L.nbins);
     if (L.mode == MODE_COUNT) return launch_variant<CW, G, R, MODE_COUNT, 2>(L, grid, st);   // diagnostics: depth 2
     if (L.mode == MODE_DS)    return launch_variant<CW, G, R, MODE_DS, 2>(L, grid, st);
     switch (L.stages) {
-    case 2:  return launch_variant<CW, G, R, MODE_J, 2>(L, grid, st);
     case 3:  return launch_variant<CW, G, R, MODE_J, 3>(L, grid, st);
-    default: return launch_variant<CW, G, R, MODE_J, 4>(L, grid, st);
+    default: return launch_variant<CW, G, R, MODE_J, 2>(L, grid, st);
     }
 }
 
@@ -466,7 +555,6 @@ cudaError_t launch_sweep_nb(const SweepLaunch &L, cudaStream_t st)
     switch (L.rows) {
     case 1: return launch_rows<CW, G, 1>(L, st);
     case 2: return launch_rows<CW, G, 2>(L, st);
-    case 4: return launch_rows<CW, G, 4>(L, st);
     }
     return cudaErrorInvalidValue;
 }
@@ -474,14 +562,14 @@ cudaError_t launch_sweep_nb(const SweepLaunch &L, cudaStream_t st)
 template <int CW, int G, int R, int D>
 static int ctas_per_sm_one(bool pair)
 {
-    constexpr int smem = sweep_smem_bytes<CW, G, R, D>();
+    constexpr int smem = kW * StageGeom<CW, G, R, D>::kWarpBytes;
     if (smem > 227 * 1024) return 0;
     int n = 0;
     auto q = [&](auto kern) {
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, 32 * kWarpsPerCta, smem);
+        return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, 32 * kW, smem);
     };
-    const cudaError_t e = pair ? q(k_sweep_tma<CW, G, R, MODE_J, D, 2>) : q(k_sweep_tma<CW, G, R, MODE_J, D, 0>);
+    const cudaError_t e = pair ? q(k_sweep_tma<CW, G, R, MODE_J, D, 2, kW, false>) : q(k_sweep_tma<CW, G, R, MODE_J, D, 0, kW, false>);
     return e == cudaSuccess ? n : 0;
 }
 
@@ -489,20 +577,18 @@ template <int CW, int G, int R>
 static int ctas_per_sm_rows(int stages, bool pair)
 {
     switch (stages) {
-    case 2:  return ctas_per_sm_one<CW, G, R, 2>(pair);
     case 3:  return ctas_per_sm_one<CW, G, R, 3>(pair);
-    default: return ctas_per_sm_one<CW, G, R, 4>(pair);
+    default: return ctas_per_sm_one<CW, G, R, 2>(pair);
     }
 }
 
-// resident CTAs (of kWarpsPerCta warps) per SM of the J-mode kernel; 0 if the configuration cannot launch
+// resident CTAs (of kOwnedWarpsPerCta warps) per SM of the J-mode kernel; 0 if the configuration cannot launch
 template <int CW, int G>
 int ctas_per_sm_nb(int rows, int stages, bool pair)
 {
     switch (rows) {
     case 1: return ctas_per_sm_rows<CW, G, 1>(stages, pair);
     case 2: return ctas_per_sm_rows<CW, G, 2>(stages, pair);
-    case 4: return ctas_per_sm_rows<CW, G, 4>(stages, pair);
     }
     return 0;
 }
