@@ -52,6 +52,7 @@ typedef struct rt_ctx rt_ctx;
 /* rt_sweep `what` */
 #define RT_J_IN     0u           /* eq. 13 */
 #define RT_J_TOTAL  1u           /* eq. 12: J_in + S */
+#define RT_SUM_IN   2u           /* N_d * J_in of this context's directions: the un-normalised sum of eq. 13 (for rt_combine) */
 
 /*
  * HEALPix ring-scheme pixel centres (Gorski et al. 2005, cited at PAPER.md:183, 463).
@@ -94,10 +95,42 @@ int rt_set_inflow(rt_ctx *ctx, const float *I_bc_host);
 /*
  * One full sweep over all directions ("one iteration" of PAPER.md:322).
  *   J_dev : DEVICE, fp32 [nbins][nz][ny][nx], caller-owned, fully overwritten
- *   what  : RT_J_IN or RT_J_TOTAL
+ *   what  : RT_J_IN, RT_J_TOTAL or RT_SUM_IN
  * Asynchronous on `cuda_stream`.  RT_ESTATE if rt_set_fields has not been called.
  */
 int rt_sweep(rt_ctx *ctx, float *J_dev, unsigned what, void *cuda_stream);
+
+/*
+ * Combine step of a direction-sharded sweep, the paper's multi-accelerator scheme (every
+ * device holds the whole mesh and a share of the directions; the partial mean intensities are summed).  Each
+ * shard is a context created with its own directions and swept with RT_SUM_IN; the caller adds the shards'
+ * results element-wise (one all-reduce(sum), e.g. NCCL through torch.distributed) and then calls
+ *     J_in = sum / ndirs_total (eq. 13),   J = J_in + S (eq. 12)
+ *   sum_dev     : DEVICE, fp32 [nbins][nz][ny][nx], the added RT_SUM_IN results of all shards
+ *   ndirs_total : number of directions of the whole set
+ *   what        : RT_J_IN or RT_J_TOTAL
+ *   J_dev       : DEVICE, fp32 [nbins][nz][ny][nx], fully overwritten; may alias sum_dev
+ * Asynchronous on `cuda_stream`.  RT_ESTATE if rt_set_fields has not been called (S comes from the packed fields).
+ */
+int rt_combine(rt_ctx *ctx, const float *sum_dev, long long ndirs_total, unsigned what, float *J_dev, void *cuda_stream);
+
+/*
+ * One full sweep followed by the rates epilogue instead of J: the photo-ionisation and photo-heating
+ * rates of the diffuse field (eqs. 14-15) for a spectrum of rectangular bins
+ * (eqs. 22-23), per cell
+ *     Gamma = sum_b  wG[b] * J_in[b] + lG[b] * S[b]
+ *     Heat  = sum_b  wH[b] * J_in[b] + lH[b] * S[b]
+ * with caller-supplied per-bin weights ("estimated prior to the simulations"):
+ *     wG[b] = 4 pi int_bin sigma/(h nu) dnu,  wH[b] = 4 pi int_bin sigma (1 - nu_i/nu) dnu   (J_in flat in the bin, eq. 19)
+ *     lG[b], lH[b] = the same integrals weighted by S_nu / S[b] (the source function's shape inside the bin).
+ * With one bin, S of eq. 18 and its shape in lG, lH this is eqs. 20-21: lG*S is the local
+ * term  delta_alpha n_e n_HII / n_HI.  Passing lG = wG, lH = wH gives eq. 14-15 applied to J = J_in + S.
+ *   Gamma_dev, Heat_dev : DEVICE, fp32 [nz][ny][nx], caller-owned, fully overwritten
+ *   wG, lG, wH, lH      : HOST, fp64 [nbins] (converted to fp32), finite
+ * Asynchronous on `cuda_stream`.  RT_ESTATE if rt_set_fields has not been called.
+ */
+int rt_sweep_rates(rt_ctx *ctx, float *Gamma_dev, float *Heat_dev, const double *wG, const double *lG,
+                   const double *wH, const double *lH, void *cuda_stream);
 
 /*
  * Diagnostics required by the parity gates (integer traversal data, summed ds).  They run the same

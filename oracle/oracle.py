@@ -160,5 +160,23 @@ def sweep_cells(kappa, S, dirs, cells, Ibc=None, cell_width: float = 1.0, nthrea
     return {"Jin": Jin, "J": J, "cnt": cnt}
 
 
+def rates(Jin, S, wG, lG, wH, lH):
+    """Rates epilogue, fp64 (eqs. 14-15 with the rectangular bins of eqs. 22-23,
+    PAPER.md:163-175): per cell  Gamma = sum_b wG[b] Jin[b] + lG[b] S[b],  Heat = sum_b wH[b] Jin[b] + lH[b] S[b].
+    wG, wH integrate a J_in that is flat inside the bin (eq. 19); lG, lH carry the shape of S_nu inside the
+    bin, so that with one bin and S of eq. 18 the second terms are those of eqs. 20-21.
+    Pinned by tests/test_oracle_pins.py::test_rates_* against numerical quadrature of eqs. 14-15."""
+    Jin = np.asarray(Jin, dtype=np.float64)
+    S = np.asarray(S, dtype=np.float64)
+    if Jin.ndim == 3:
+        Jin, S = Jin[None], S[None]
+    G = np.zeros(Jin.shape[1:], dtype=np.float64)
+    H = np.zeros(Jin.shape[1:], dtype=np.float64)
+    for b in range(Jin.shape[0]):
+        G += float(wG[b]) * Jin[b] + float(lG[b]) * S[b]
+        H += float(wH[b]) * Jin[b] + float(lH[b]) * S[b]
+    return G, H
+
+
 def num_threads() -> int:
     return int(lib().orc_num_threads())

@@ -9,10 +9,10 @@ import numpy as np
 from . import build as _build
 
 RT_OWNED, RT_ATOMIC_ABLATION, RT_PAPER_GROUPS = 0, 1, 2
-RT_J_IN, RT_J_TOTAL = 0, 1
+RT_J_IN, RT_J_TOTAL, RT_SUM_IN = 0, 1, 2
 
 EXPORTED_SYMBOLS = [
-    "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_sweep", "rt_segment_counts",
+    "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_sweep", "rt_combine", "rt_sweep_rates", "rt_segment_counts",
     "rt_sum_ds", "rt_total_segments", "rt_direction_records", "rt_tune", "rt_last_launch_count",
     "rt_last_sweep_kernel_ms", "rt_destroy", "rt_strerror", "rt_last_cuda_error",
 ]
@@ -49,6 +49,10 @@ def load_library():
     L.rt_set_inflow.restype = C.c_int
     L.rt_sweep.argtypes = [vp, vp, C.c_uint, vp]
     L.rt_sweep.restype = C.c_int
+    L.rt_combine.argtypes = [vp, vp, C.c_longlong, C.c_uint, vp, vp]
+    L.rt_combine.restype = C.c_int
+    L.rt_sweep_rates.argtypes = [vp, vp, vp, dp, dp, dp, dp, vp]
+    L.rt_sweep_rates.restype = C.c_int
     L.rt_segment_counts.argtypes = [vp, C.c_int, vp, vp]
     L.rt_segment_counts.restype = C.c_int
     L.rt_sum_ds.argtypes = [vp, dp, dp, dp, vp]
@@ -134,6 +138,23 @@ def rt_sweep(h, J, numel, what=RT_J_IN, stream=None):
     _check(load_library().rt_sweep(h, _dev_ptr(J, torch.float32, numel, "J"), int(what), _stream(stream)), "rt_sweep")
 
 
+def rt_combine(h, total, ndirs_total, J, numel, what=RT_J_IN, stream=None):
+    import torch
+    _check(load_library().rt_combine(h, _dev_ptr(total, torch.float32, numel, "sum"), int(ndirs_total), int(what),
+                                     _dev_ptr(J, torch.float32, numel, "J"), _stream(stream)), "rt_combine")
+
+
+def rt_sweep_rates(h, Gamma, Heat, ncell, nbins, wG, lG, wH, lH, stream=None):
+    import torch
+    w = [np.ascontiguousarray(a, dtype=np.float64).reshape(-1) for a in (wG, lG, wH, lH)]
+    if any(a.shape[0] != nbins for a in w):
+        raise ValueError("rate weights must have one entry per bin")
+    p = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+    _check(load_library().rt_sweep_rates(h, _dev_ptr(Gamma, torch.float32, ncell, "Gamma"),
+                                         _dev_ptr(Heat, torch.float32, ncell, "Heat"), p(w[0]), p(w[1]), p(w[2]), p(w[3]),
+                                         _stream(stream)), "rt_sweep_rates")
+
+
 def rt_segment_counts(h, dir_index, counts, numel, stream=None):
     import torch
     _check(load_library().rt_segment_counts(h, int(dir_index), _dev_ptr(counts, torch.int32, numel, "counts"),
@@ -202,6 +223,21 @@ class RayTracer:
             out = torch.empty(self.shape(), dtype=torch.float32, device="cuda")
         rt_sweep(self.h, out, self.numel, what, stream)
         return out
+
+    def combine(self, total, ndirs_total, what=RT_J_IN, out=None, stream=None):
+        """rt_combine: J from the all-reduced RT_SUM_IN results of a direction-sharded sweep."""
+        if out is None:
+            out = total
+        rt_combine(self.h, total, ndirs_total, out, self.numel, what, stream)
+        return out
+
+    def sweep_rates(self, wG, lG, wH, lH, stream=None):
+        """rt_sweep_rates: (Gamma, Heat), each [nz][ny][nx] fp32."""
+        import torch
+        G = torch.empty((self.nz, self.ny, self.nx), dtype=torch.float32, device="cuda")
+        H = torch.empty_like(G)
+        rt_sweep_rates(self.h, G, H, self.nx * self.ny * self.nz, self.nbins, wG, lG, wH, lH, stream)
+        return G, H
 
     def segment_counts(self, dir_index=-1, stream=None):
         import torch

@@ -460,7 +460,7 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
 
 extern "C" int rt_sweep(rt_ctx *c, float *J_dev, unsigned what, void *stream)
 {
-    if (!c || !J_dev || what > 1u) return RT_EINVAL;
+    if (!c || !J_dev || what > 2u) return RT_EINVAL;
     if (!c->fields_set) return RT_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
     int launches = 0;
@@ -468,7 +468,40 @@ extern "C" int rt_sweep(rt_ctx *c, float *J_dev, unsigned what, void *stream)
     int rc = run_traversal(c, MODE_J, -1, c->nbins, st, &launches, used);
     if (rc != RT_OK) return rc;
     CK(launch_normalise(J_dev, c->d_P[0], c->pp[0], c->d_acc[0], c->d_accC[0], used[0], c->d_acc[1], c->d_accC[1], used[1],
-                        c->nx, c->ny, c->nz, c->nbins, (float)(1.0 / (double)c->ndirs), what == RT_J_TOTAL ? 1 : 0, st));
+                        c->nx, c->ny, c->nz, c->nbins, what == RT_SUM_IN ? 1.0f : (float)(1.0 / (double)c->ndirs),
+                        what == RT_J_TOTAL ? 1 : 0, st));
+    c->last_launches = launches + 1;
+    return RT_OK;
+}
+
+extern "C" int rt_combine(rt_ctx *c, const float *sum_dev, long long ndirs_total, unsigned what, float *J_dev, void *stream)
+{
+    if (!c || !sum_dev || !J_dev || ndirs_total < 1 || what > 1u) return RT_EINVAL;
+    if (!c->fields_set) return RT_ESTATE;
+    CK(launch_combine(J_dev, sum_dev, c->d_P[0], c->pp[0], (size_t)c->ncell * c->nbins, (float)(1.0 / (double)ndirs_total),
+                      what == RT_J_TOTAL ? 1 : 0, (cudaStream_t)stream));
+    return RT_OK;
+}
+
+extern "C" int rt_sweep_rates(rt_ctx *c, float *Gamma_dev, float *Heat_dev, const double *wG, const double *lG,
+                              const double *wH, const double *lH, void *stream)
+{
+    if (!c || !Gamma_dev || !Heat_dev || !wG || !lG || !wH || !lH) return RT_EINVAL;
+    if (!c->fields_set) return RT_ESTATE;
+    std::vector<float> w4(4 * (size_t)c->nbins);
+    const double *src[4] = {wG, lG, wH, lH};
+    for (int k = 0; k < 4; ++k)
+        for (int b = 0; b < c->nbins; ++b) {
+            if (!std::isfinite(src[k][b])) return RT_EINVAL;
+            w4[(size_t)k * c->nbins + b] = (float)src[k][b];
+        }
+    cudaStream_t st = (cudaStream_t)stream;
+    int launches = 0;
+    int used[2];
+    int rc = run_traversal(c, MODE_J, -1, c->nbins, st, &launches, used);
+    if (rc != RT_OK) return rc;
+    CK(launch_rates(Gamma_dev, Heat_dev, c->d_P[0], c->pp[0], c->d_acc[0], c->d_accC[0], used[0], c->d_acc[1], c->d_accC[1],
+                    used[1], c->nx, c->ny, c->nz, c->nbins, (float)(1.0 / (double)c->ndirs), w4.data(), st));
     c->last_launches = launches + 1;
     return RT_OK;
 }

@@ -80,6 +80,11 @@ cudaError_t launch_sweep_generic(const SweepLaunch &L, int max_lattice_b, int ma
 cudaError_t launch_normalise(float *J, const float2 *Pnat, int ppN, const float *accN, const float *accNC, int slotsN,
                              const float *accT, const float *accTC, int slotsT,
                              int nx, int ny, int nz, int nbins, float inv_nd, int add_S, cudaStream_t st);
+cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN, const float *accN, const float *accNC,
+                         int slotsN, const float *accT, const float *accTC, int slotsT, int nx, int ny, int nz, int nbins,
+                         float inv_nd, const float *w4, cudaStream_t st);
+cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int ppN, size_t n, float inv_nd, int add_S,
+                           cudaStream_t st);
 cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const float *accNC, int slotsN,
                                    const float *accT, const float *accTC, int slotsT,
                                    int nx, int ny, int nz, cudaStream_t st);

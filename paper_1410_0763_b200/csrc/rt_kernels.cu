@@ -324,6 +324,104 @@ cudaError_t launch_normalise(float *J, const float2 *Pnat, int ppN, const float 
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------
+// Rates epilogue (eqs. 14-15 with the rectangular bins of eqs. 22-23; eqs. 20-21 are its one-bin case):
+//   Gamma = sum_b wG[b] * J_in[b] + lG[b] * S[b],   Heat = sum_b wH[b] * J_in[b] + lH[b] * S[b]
+// fused with the normalisation (the accumulators are read once, J is never written).
+// ------------------------------------------------------------------------------------------------
+struct RateWeights { float wG[16], lG[16], wH[16], lH[16]; };
+
+__global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, const float2 *__restrict__ Pnat, int ppN,
+                        const float *__restrict__ accN, const float *__restrict__ accNC, int slotsN,
+                        const float *__restrict__ accT, const float *__restrict__ accTC, int slotsT,
+                        int nx, int ny, int nz, int nbins, float inv_nd, const RateWeights W)
+{
+    __shared__ float tile[32][33];
+    const int z = blockIdx.z;
+    const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
+    const size_t ncell = (size_t)nx * ny * nz;
+    const size_t slot_stride = ncell * nbins;
+    const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
+    float g[4] = {0.0f, 0.0f, 0.0f, 0.0f}, h[4] = {0.0f, 0.0f, 0.0f, 0.0f};      // rows threadIdx.y + 8 j
+    for (int bin = 0; bin < nbins; ++bin) {
+        // transposed layout [x][z][y]: coalesced along y
+        for (int dx = threadIdx.y; dx < 32; dx += blockDim.y) {
+            const int x = x0 + dx, y = y0 + threadIdx.x;
+            float s = 0.0f;
+            if (x < nx && y < ny) {
+                const size_t i = (size_t)bin * ncell + ((size_t)x * nz + z) * ny + y;
+                for (int sl = 0; sl < slotsT; ++sl) s += accT[sl * slot_stride + i] + accTC[sl * slot_stride + i];
+            }
+            tile[dx][threadIdx.x] = s;
+        }
+        __syncthreads();
+        int j = 0;
+        for (int dy = threadIdx.y; dy < 32; dy += blockDim.y, ++j) {
+            const int x = x0 + threadIdx.x, y = y0 + dy;
+            if (x < nx && y < ny) {
+                const size_t i = (size_t)bin * ncell + ((size_t)z * ny + y) * nx + x;
+                float s = tile[threadIdx.x][dy];
+                for (int sl = 0; sl < slotsN; ++sl) s += accN[sl * slot_stride + i] + accNC[sl * slot_stride + i];
+                const size_t o = field_index(i, ppN);
+                const float kap = fN[o], src = fN[o + field_s_offset(ppN)];
+                const float jin = s * inv_nd / kap;
+                g[j] = fmaf(W.wG[bin], jin, fmaf(W.lG[bin], src, g[j]));
+                h[j] = fmaf(W.wH[bin], jin, fmaf(W.lH[bin], src, h[j]));
+            }
+        }
+        __syncthreads();
+    }
+    int j = 0;
+    for (int dy = threadIdx.y; dy < 32; dy += blockDim.y, ++j) {
+        const int x = x0 + threadIdx.x, y = y0 + dy;
+        if (x < nx && y < ny) {
+            const size_t i = ((size_t)z * ny + y) * nx + x;
+            Gamma[i] = g[j];
+            Heat[i] = h[j];
+        }
+    }
+}
+
+cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN, const float *accN, const float *accNC,
+                         int slotsN, const float *accT, const float *accTC, int slotsT, int nx, int ny, int nz, int nbins,
+                         float inv_nd, const float *w4 /* host: wG, lG, wH, lH, each [nbins] */, cudaStream_t st)
+{
+    RateWeights W;
+    for (int b = 0; b < 16; ++b) {
+        const bool in = b < nbins;
+        W.wG[b] = in ? w4[b] : 0.0f;             W.lG[b] = in ? w4[nbins + b] : 0.0f;
+        W.wH[b] = in ? w4[2 * nbins + b] : 0.0f; W.lH[b] = in ? w4[3 * nbins + b] : 0.0f;
+    }
+    dim3 grid((nx + 31) / 32, (ny + 31) / 32, nz), block(32, 8);
+    k_rates<<<grid, block, 0, st>>>(Gamma, Heat, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT, nx, ny, nz, nbins,
+                                   inv_nd, W);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Combine step of a direction-sharded sweep: the un-normalised sums of all
+// shards have been added (all-reduce); J_in = sum / N_d (eq. 13), J = J_in + S (eq. 12).
+// ------------------------------------------------------------------------------------------------
+__global__ void k_combine(float *__restrict__ J, const float *__restrict__ sum, const float2 *__restrict__ Pnat, int ppN,
+                          size_t n, float inv_nd, int add_S)
+{
+    const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        float v = sum[i] * inv_nd;
+        if (add_S) v += fN[field_index(i, ppN) + field_s_offset(ppN)];
+        J[i] = v;
+    }
+}
+
+cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int ppN, size_t n, float inv_nd, int add_S,
+                           cudaStream_t st)
+{
+    size_t blocks = (n + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    k_combine<<<(unsigned)blocks, 256, 0, st>>>(J, sum, Pnat, ppN, n, inv_nd, add_S);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const float *accNC, int slotsN,
                                    const float *accT, const float *accTC, int slotsT,
                                    int nx, int ny, int nz, cudaStream_t st)

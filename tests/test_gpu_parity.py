@@ -297,6 +297,64 @@ def test_inflow_cellwidth_multibin(orc):
     check_full(orc, kap, S, dirs, out, ref, cell_width=0.7)
 
 
+@pytest.mark.parametrize("name,dims,nside", [("C5", (64, 32, 48), 2), ("C2", (32, 32, 32), 2), ("C5", (20, 12, 10), 1)])
+def test_rates_epilogue(orc, name, dims, nside):
+    """rt_sweep_rates against the oracle's rates() of the oracle's J_in (eqs. 14-15, 20-23): 1e-5."""
+    import paper_1410_0763_b200 as rt
+    from rt_inputs import make_fields
+    torch = _torch()
+    kap, S = make_fields(name, dims=dims)
+    nb = kap.shape[0]
+    dirs = orc.healpix_dirs(nside)
+    rng = np.random.default_rng(3)
+    w = rng.uniform(0.2, 3.0, (4, nb))
+    ref = orc.sweep(kap, S, dirs, want_counts=False)
+    Gr, Hr = orc.rates(ref["Jin"], S.astype(np.float64), w[0], w[1], w[2], w[3])
+    tr = rt.RayTracer(dims, nb, dirs)
+    try:
+        tr.set_fields(torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda())
+        G, H = tr.sweep_rates(w[0], w[1], w[2], w[3])
+        G, H = G.cpu().numpy(), H.cpu().numpy()
+        Jin = tr.sweep(what=rt.RT_J_IN).cpu().numpy()      # the sweep is unchanged by the epilogue call
+    finally:
+        tr.close()
+    assert rel_err(G, Gr).max() <= J_TOL and rel_err(H, Hr).max() <= J_TOL
+    assert rel_err(Jin, ref["Jin"]).max() <= J_TOL
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_direction_shards_combine(orc, world):
+    """Direction sharding on one GPU: one context per share swept with RT_SUM_IN, the
+    shares added (what the all-reduce does), rt_combine -> J of the whole set within 1e-5 of the oracle."""
+    import paper_1410_0763_b200 as rt
+    from rt_inputs import make_fields
+    torch = _torch()
+    dims = (64, 32, 48)
+    kap, S = make_fields("C3", dims=dims)
+    dirs = orc.healpix_dirs(4)
+    ref = orc.sweep(kap, S, dirs, want_counts=False)
+    kd, sd = torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda()
+    total = None
+    trs = []
+    try:
+        for r in range(world):
+            tr = rt.RayTracer(dims, 1, dirs[rt.shard_directions(dirs, world, r)])
+            trs.append(tr)
+            tr.set_fields(kd, sd)
+            part = tr.sweep(what=rt.RT_SUM_IN)
+            total = part if total is None else total + part
+        Jin = trs[0].combine(total.clone(), len(dirs), what=rt.RT_J_IN).cpu().numpy()
+        J = trs[-1].combine(total.clone(), len(dirs), what=rt.RT_J_TOTAL).cpu().numpy()
+        one = rt.sweep_sharded(trs[0], len(trs[0].dirs), what=rt.RT_J_IN).cpu().numpy()   # world of 1: no collective
+        ref0 = trs[0].sweep(what=rt.RT_J_IN).cpu().numpy()
+    finally:
+        for tr in trs:
+            tr.close()
+    assert rel_err(Jin, ref["Jin"]).max() <= J_TOL
+    assert rel_err(J, ref["J"]).max() <= J_TOL
+    assert rel_err(one, ref0).max() <= 1e-6
+
+
 def test_degenerate_directions(orc):
     """Axis-aligned, exact diagonals, unit slopes, half slopes (crossings on slab planes), near-degenerate."""
     kap, S = _rand((32, 32, 32), 13)

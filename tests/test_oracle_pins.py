@@ -373,3 +373,59 @@ def test_cell_width_scales_optical_depth(orc):
     a = orc.sweep(kap, S, dirs, cell_width=2.0)
     b = orc.sweep((kap * np.float32(2.0)), S, dirs, cell_width=1.0)
     assert np.allclose(a["Jin"], b["Jin"], rtol=1e-12)
+
+
+# ---------------------------------------------------------------------------------------------
+# Rates epilogue (eqs. 14-15, 20-23)
+def _quad(f, a, b, n=20001):
+    """Composite Simpson on [a, b] (n odd), plain numpy: the independent quadrature of the pins."""
+    x = np.linspace(a, b, n)
+    y = f(x)
+    h = (b - a) / (n - 1)
+    return h / 3.0 * (y[0] + y[-1] + 4.0 * y[1:-1:2].sum() + 2.0 * y[2:-1:2].sum())
+
+
+def test_rates_one_bin_reproduces_eqs_20_21(orc):
+    """One bin, S of eq. 18 and J_in flat in the band (eq. 19): the epilogue must give
+    eq. 20 / eq. 21, i.e. the local terms  X/n_HI  and  X h dnu / (2 n_HI)  with
+    X = delta_alpha n_e n_HII, and the J_in terms 4 pi J int sigma/(h nu) and 4 pi J int (1-nu0/nu) sigma.
+    Weights come from numerical quadrature of eqs. 14-15 written out with S_nu(nu) of eq. 18."""
+    h_pl, nu0, sig0 = 6.62607015e-27, 3.288e15, 6.3e-18
+    dnu = 0.0262 * nu0                                     # k_B T / h at 1e4 K is about 2.08e14 Hz
+    sigma = lambda nu: sig0 * (nu / nu0) ** -3.0
+    rng = np.random.default_rng(5)
+    X = rng.uniform(1e-14, 1e-12, (3, 4, 5))               # delta_alpha n_e n_HII per cell
+    nHI = rng.uniform(1e-4, 1e-2, (3, 4, 5))
+    Jin = rng.uniform(0.0, 1e-20, (1, 3, 4, 5))
+    S_nu = lambda nu, c=1.0: c * h_pl * nu / (4 * math.pi * sigma(nu) * dnu)     # eq. 18 per unit X/n_HI
+    S0 = (X / nHI * S_nu(nu0))[None]                       # the bin's stored S: eq. 18 at nu0
+    shape = lambda nu: S_nu(nu) / S_nu(nu0)
+    wG = 4 * math.pi * _quad(lambda nu: sigma(nu) / (h_pl * nu), nu0, nu0 + dnu)
+    wH = 4 * math.pi * _quad(lambda nu: sigma(nu) * (1 - nu0 / nu), nu0, nu0 + dnu)
+    lG = 4 * math.pi * _quad(lambda nu: shape(nu) * sigma(nu) / (h_pl * nu), nu0, nu0 + dnu)
+    lH = 4 * math.pi * _quad(lambda nu: shape(nu) * sigma(nu) * (1 - nu0 / nu), nu0, nu0 + dnu)
+    G, H = orc.rates(Jin, S0, [wG], [lG], [wH], [lH])
+    G20 = wG * Jin[0] + X / nHI                                              # eq. 20
+    H21 = wH * Jin[0] + X / (2 * nHI) * h_pl * dnu                           # eq. 21
+    assert np.abs(G / G20 - 1).max() < 1e-10
+    assert np.abs(H / H21 - 1).max() < 1e-10
+    # closed forms of the power-law integrals (a dropped factor or a swapped weight fails here)
+    assert abs(wG / (4 * math.pi * sig0 * nu0 ** 3 / (3 * h_pl) * (nu0 ** -3 - (nu0 + dnu) ** -3)) - 1) < 1e-10
+    assert abs(lG / (4 * math.pi * sig0 * dnu / (h_pl * nu0)) - 1) < 1e-10
+
+
+def test_rates_bins_are_additive_and_linear(orc):
+    """Eq. 22: the spectrum is a sum of rectangular bins, so the rates are a plain sum over bins,
+    linear in every weight; with lG = wG, lH = wH they are eq. 14-15 applied to J = J_in + S."""
+    rng = np.random.default_rng(6)
+    Jin = rng.uniform(0, 1, (3, 2, 3, 4))
+    S = rng.uniform(0, 1, (3, 2, 3, 4))
+    w = rng.uniform(0.1, 2.0, (4, 3))
+    G, H = orc.rates(Jin, S, w[0], w[1], w[2], w[3])
+    Gs = sum(orc.rates(Jin[b:b + 1], S[b:b + 1], w[0, b:b + 1], w[1, b:b + 1], w[2, b:b + 1], w[3, b:b + 1])[0] for b in range(3))
+    assert np.allclose(G, Gs, rtol=1e-14, atol=0)
+    G2, H2 = orc.rates(Jin, S, w[0], w[0], w[2], w[2])
+    assert np.allclose(G2, np.tensordot(w[0], Jin + S, axes=(0, 0)), rtol=1e-14)
+    assert np.allclose(H2, np.tensordot(w[2], Jin + S, axes=(0, 0)), rtol=1e-14)
+    G3, _ = orc.rates(Jin, S, 2 * w[0], w[1], w[2], w[3])
+    assert np.allclose(G3 - G, np.tensordot(w[0], Jin, axes=(0, 0)), rtol=1e-12)
