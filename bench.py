@@ -29,7 +29,7 @@ UNIT = "updates/s"
 ALGO_BYTES_PER_CELL_DIR_BIN = 16.0     # read kappa,S (8 B) + read-modify-write J accumulator (8 B), SURVEY 8(d)
 # dram__bytes_read.sum + dram__bytes_write.sum per cell-direction-bin of the hot kernel, from the ncu --set full
 # capture named beside it (profiles/); multiplied by the cell-direction-bins of one launch to give `traffic`.
-NCU_DRAM_BYTES_PER_CELL_DIR_BIN = {"C4": (2.77e9 / (13 * 256 ** 3), "profiles/r1a_sweep_tma_full_c4.md")}
+NCU_DRAM_BYTES_PER_CELL_DIR_BIN = {"C4": (2.535e9 / (26 * 256 ** 3), "profiles/r1c_sweep_tma_full_c4.md")}
 
 
 def measured_peaks():
@@ -140,7 +140,7 @@ def main():
     ap.add_argument("--config", default="C4")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-dirs", type=int, default=8, help="directions per step of the reference arm")
-    ap.add_argument("--cpu-dirs", type=int, default=16, help="directions of the cpu_baseline sample")
+    ap.add_argument("--cpu-dirs", type=int, default=48, help="directions of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--slots", type=int, default=None)
     ap.add_argument("--rows", type=int, default=None)
@@ -148,6 +148,9 @@ def main():
     ap.add_argument("--pair", type=int, default=None, help="0: switch the mirror-pair schedule off (ablation)")
     ap.add_argument("--tune", action="append", default=[], help="key=value passed to rt_tune (experiments)")
     ap.add_argument("--flags", type=int, default=0, help="0 owned, 1 atomic ablation, 2 paper's four groups")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "directions"],
+                    help="N > 1: independent replicas (default; north_star fixes one GPU) or the paper's direction "
+                         "sharding with one all-reduce (PAPER.md:228-230)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -169,6 +172,10 @@ def main():
     spec = CONFIGS[args.config]
     kap, S = make_fields(args.config)
     dirs = rt.healpix_dirs(spec.nside)
+    sharded = world > 1 and args.shard == "directions"
+    ndirs_total = dirs.shape[0]
+    if sharded:
+        dirs = dirs[rt.shard_directions(dirs, world, rank)]
     tr = rt.RayTracer(spec.dims, spec.nbins, dirs, flags=args.flags, slots=args.slots, rows=args.rows, stages=args.stages, pair=args.pair,
                       tune=dict((kv.split('=')[0], int(kv.split('=')[1])) for kv in args.tune))
     stream = torch.cuda.current_stream()
@@ -180,7 +187,17 @@ def main():
     J_h = torch.empty(tr.shape(), dtype=torch.float32).pin_memory()
     tr.set_fields(kd, sd)
     updates_per_sweep = tr.total_segments() * spec.nbins        # exact integer traversal count x bins
-    cell_dir_bins = spec.ncell * spec.ndirs * spec.nbins
+    cell_dir_bins = spec.ncell * dirs.shape[0] * spec.nbins
+    if sharded:                                                  # whole-job updates: sum over the shares
+        t = torch.tensor([updates_per_sweep], device="cuda", dtype=torch.int64)
+        dist.all_reduce(t)
+        updates_per_sweep = int(t.item())
+
+    def step():
+        if sharded:
+            rt.sweep_sharded(tr, ndirs_total, what=rt.RT_J_IN, out=J)
+        else:
+            tr.sweep(out=J)
 
     def barrier():
         if dist is not None:
@@ -189,7 +206,7 @@ def main():
 
     # ---------------- device-resident timing (value) ----------------
     for _ in range(max(args.warmup, 3)):
-        tr.sweep(out=J)
+        step()
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
@@ -199,7 +216,7 @@ def main():
     barrier()
     e0.record(stream)
     for _ in range(args.steps):
-        tr.sweep(out=J)
+        step()
     e1.record(stream)
     barrier()
     clocks = sampler.stop() if rank == 0 else None
@@ -211,7 +228,8 @@ def main():
         t = torch.tensor([ms], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
-    value = world * updates_per_sweep * args.steps / (ms * 1e-3)
+    jobs = 1 if sharded else world                               # replicas: every rank sweeps the whole set
+    value = jobs * updates_per_sweep * args.steps / (ms * 1e-3)
 
     # ---------------- end-to-end through the C ABI with host buffers ----------------
     barrier()
@@ -221,7 +239,7 @@ def main():
         kd.copy_(kap_h, non_blocking=True)
         sd.copy_(S_h, non_blocking=True)
         tr.set_fields(kd, sd)
-        tr.sweep(out=J)
+        step()
         J_h.copy_(J, non_blocking=True)
     f1.record(stream)
     barrier()
@@ -230,7 +248,7 @@ def main():
         t = torch.tensor([ms_e2e], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms_e2e = float(t.item())
-    e2e_value = world * updates_per_sweep * args.steps / (ms_e2e * 1e-3)
+    e2e_value = jobs * updates_per_sweep * args.steps / (ms_e2e * 1e-3)
     tr.close()
 
     if rank != 0:
@@ -250,6 +268,10 @@ def main():
         traffic = per * cell_dir_bins / n_sweep_launches
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "traffic_source": traffic_src, "peak_kind": peak_kind, "kernel": "k_sweep_tma",
+                # the same launches against the DRAM bytes ncu measured (mirror pairs share loads, so the
+                # algorithmic-byte fraction above exceeds 1; this one is the bandwidth the kernel really draws)
+                "dram_gbs_from_traffic": (traffic / (avg_launch_ms * 1e-3) / 1e9) if traffic else None,
+                "dram_frac_from_traffic": (traffic / (avg_launch_ms * 1e-3) / 1e9 / peak) if traffic else None,
                 "launches_per_step": n_sweep_launches, "avg_launch_ms": avg_launch_ms,
                 "algorithmic_bytes_per_launch": bytes_per_launch,
                 "kernel_share_of_step": kernel_ms[0] / (ms / args.steps)}
@@ -270,10 +292,10 @@ def main():
 
     print(json.dumps({
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+        "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong" if sharded else "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_name(spec), "updates_per_step": updates_per_sweep,
-                   "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "parallelism": ("directions sharded, 1 all-reduce" if sharded else "replicas only") if world > 1 else "1 gpu",
                    "l2": "working set (packed fields + slot accumulators) larger than L2",
                    "variant": ["owned", "atomic_ablation", "paper_groups"][args.flags]},
         "clocks": clocks, "gpu_launches": launches_per_sweep * args.steps,
