@@ -126,6 +126,7 @@ typedef struct {
     const float *kappa, *S;     /* [nbins][nz][ny][nx] */
     const double *Ibc;          /* [nbins] or NULL (=0) */
     double cell_width;
+    int rays;                   /* r: rays per cell width in each transverse axis (O3, A13); 0 means 1 */
     /* per-direction scratch (owned by the calling thread) */
     double *num;                /* [nbins][ncell] */
     double *den;                /* [ncell] */
@@ -164,7 +165,10 @@ static void trace_ray(orc_work_t *w, const orc_dir_t *d, int64_t p, int64_t q)
 {
     const int Na = w->dims[d->a], Nb = w->dims[d->b], Nc = w->dims[d->c];
     const int64_t ONE = ORC_ONE;
-    const int64_t U0 = p * ONE + ONE / 2, V0 = q * ONE + ONE / 2;   /* cell-centre offsets (A2), r = 1 */
+    /* O3: lattice of spacing 1/r; ray (p,q) meets the plane a = 0 at U0 = (2p+1) ONE/(2r), V0 = (2q+1) ONE/(2r)
+       (r divides 2^19, checked by the callers; r = 1: cell-centre offsets, A2) */
+    const int64_t r_ = w->rays > 0 ? w->rays : 1;
+    const int64_t U0 = (2 * p + 1) * (ONE / (2 * r_)), V0 = (2 * q + 1) * (ONE / (2 * r_));
     const double Lw = d->L * w->cell_width;
     double I[16];
     for (int bin = 0; bin < w->nbins; ++bin) I[bin] = w->Ibc ? w->Ibc[bin] : 0.0;
@@ -248,8 +252,9 @@ static void sweep_direction(orc_work_t *w, const orc_dir_t *d)
     lattice_range(w->dims, d, &pmin, &qmin);
     w->pmin = pmin; w->qmin = qmin;
     w->np = w->dims[d->b] - pmin; w->nq = w->dims[d->c] - qmin;
-    for (int64_t q = qmin; q < w->dims[d->c]; ++q)
-        for (int64_t p = pmin; p < w->dims[d->b]; ++p)
+    const int64_t r_ = w->rays > 0 ? w->rays : 1;                  /* O3: p from r*pmin to r*Nb - 1, q likewise */
+    for (int64_t q = r_ * qmin; q < r_ * w->dims[d->c]; ++q)
+        for (int64_t p = r_ * pmin; p < r_ * w->dims[d->b]; ++p)
             trace_ray(w, d, p, q);
 }
 
@@ -268,14 +273,15 @@ static void sweep_direction(orc_work_t *w, const orc_dir_t *d)
  *   nthreads   : OpenMP threads over directions (<=0: default)
  * Returns 0, or <0 on bad arguments / allocation failure.
  */
-int orc_sweep(int nx, int ny, int nz, int nbins,
+int orc_sweep_rays(int nx, int ny, int nz, int nbins,
               const float *kappa, const float *S,
-              const double *dirs, int ndirs, const double *Ibc, double cell_width,
+              const double *dirs, int ndirs, const double *Ibc, double cell_width, int rays,
               double *Jin, double *J, double *sum_ds, unsigned long long *seg_total,
               uint32_t *cnt_sum, const int *cnt_dirs, int ncnt, uint32_t *cnt_out,
               double *min_den, double *max_den, int nthreads)
 {
     if (nx < 1 || ny < 1 || nz < 1 || nbins < 1 || nbins > 16 || !kappa || !S || !dirs || ndirs < 1) return -1;
+    if (rays < 1 || rays > (1 << 19) || (rays & (rays - 1)) != 0) return -1;      /* r must divide 2^(F-1) (O3) */
     const size_t ncell = (size_t)nx * ny * nz;
     int fail = 0;
     unsigned long long total = 0;
@@ -290,6 +296,7 @@ int orc_sweep(int nx, int ny, int nz, int nbins,
         memset(&w, 0, sizeof(w));
         w.dims[0] = nx; w.dims[1] = ny; w.dims[2] = nz;
         w.nbins = nbins; w.ncell = ncell; w.kappa = kappa; w.S = S; w.Ibc = Ibc; w.cell_width = cell_width;
+        w.rays = rays;
         w.num = (double *)calloc(ncell * nbins, sizeof(double));
         w.den = (double *)calloc(ncell, sizeof(double));
         w.cnt = (uint32_t *)calloc(ncell, sizeof(uint32_t));
@@ -341,6 +348,18 @@ int orc_sweep(int nx, int ny, int nz, int nbins,
     if (J && Jin)                                                   /* eq. 12 */
         for (size_t o = 0; o < ncell * nbins; ++o) J[o] = Jin[o] + (double)S[o];
     return 0;
+}
+
+/* r = 1: one ray per cell cross-section (all five configs) */
+int orc_sweep(int nx, int ny, int nz, int nbins,
+              const float *kappa, const float *S,
+              const double *dirs, int ndirs, const double *Ibc, double cell_width,
+              double *Jin, double *J, double *sum_ds, unsigned long long *seg_total,
+              uint32_t *cnt_sum, const int *cnt_dirs, int ncnt, uint32_t *cnt_out,
+              double *min_den, double *max_den, int nthreads)
+{
+    return orc_sweep_rays(nx, ny, nz, nbins, kappa, S, dirs, ndirs, Ibc, cell_width, 1, Jin, J, sum_ds, seg_total,
+                          cnt_sum, cnt_dirs, ncnt, cnt_out, min_den, max_den, nthreads);
 }
 
 /*

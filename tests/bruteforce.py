@@ -41,12 +41,13 @@ def round_half_even(x):
     return f
 
 
-def ray_intervals(dims, n, p, q):
+def ray_intervals(dims, n, p, q, rays=1):
     """Exact (cell, fraction_of_L) list, in marching order, for lattice ray (p, q) of direction n."""
     a, b, c, refl, Mb, Mc, L = dir_record(n)
     Na, Nb, Nc = dims[a], dims[b], dims[c]
     mb, mc = Fraction(Mb, ONE), Fraction(Mc, ONE)
-    b0, c0 = Fraction(2 * p + 1, 2), Fraction(2 * q + 1, 2)      # cell-centre offsets on the plane a = 0
+    # lattice of spacing 1/rays on the plane a = 0 (rays = 1: cell-centre offsets)
+    b0, c0 = Fraction(2 * p + 1, 2 * rays), Fraction(2 * q + 1, 2 * rays)
     events = {Fraction(k) for k in range(Na + 1)}
     if Mb:
         lo, hi = math.floor(b0), math.ceil(b0 + mb * Na)
@@ -79,19 +80,19 @@ def ray_intervals(dims, n, p, q):
     return out, L
 
 
-def lattice(dims, n):
+def lattice(dims, n, rays=1):
     a, b, c, refl, Mb, Mc, L = dir_record(n)
     Na, Nb, Nc = dims[a], dims[b], dims[c]
     pmin = -math.ceil(Fraction(Na * Mb, ONE)) - 1
     qmin = -math.ceil(Fraction(Na * Mc, ONE)) - 1
-    return [(p, q) for q in range(qmin, Nc) for p in range(pmin, Nb)]
+    return [(p, q) for q in range(rays * qmin, rays * Nc) for p in range(rays * pmin, rays * Nb)]
 
 
 def f_of(x):
     return 1.0 - 0.5 * x if x < 1e-8 else -math.expm1(-x) / x
 
 
-def sweep(kappa, S, dirs, Ibc=0.0, linear=False):
+def sweep(kappa, S, dirs, Ibc=0.0, linear=False, rays=1):
     """kappa, S: nested [z][y][x] python/numpy arrays (single bin).  Returns dict of per-cell dicts.
 
     linear=True replaces eq. 7 by the optically thin limit I += kappa*S*ds and f by 1 (pin P6).
@@ -101,8 +102,8 @@ def sweep(kappa, S, dirs, Ibc=0.0, linear=False):
     Jin, cnt_tot, per_dir = {}, {}, []
     for n in dirs:
         num, den, cnt, exits = {}, {}, {}, {}
-        for (p, q) in lattice(dims, n):
-            iv, L = ray_intervals(dims, n, p, q)
+        for (p, q) in lattice(dims, n, rays):
+            iv, L = ray_intervals(dims, n, p, q, rays)
             I = float(Ibc)
             chord = 0.0
             for (x, y, z), frac in iv:

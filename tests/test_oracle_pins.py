@@ -429,3 +429,44 @@ def test_rates_bins_are_additive_and_linear(orc):
     assert np.allclose(H2, np.tensordot(w[2], Jin + S, axes=(0, 0)), rtol=1e-14)
     G3, _ = orc.rates(Jin, S, 2 * w[0], w[1], w[2], w[3])
     assert np.allclose(G3 - G, np.tensordot(w[0], Jin, axes=(0, 0)), rtol=1e-12)
+
+
+# ---------------------------------------------------------------------------------------------
+# r > 1 rays per cell width (O3, A13)
+@pytest.mark.parametrize("rays", [2, 4])
+def test_p12_rays_per_cell_bruteforce_and_closed_forms(orc, rays):
+    """Lattice of spacing 1/r: independent exact-rational brute force (counts bit-exact, J_in to 1e-12),
+    per cell and direction sum ds = r^2 L (pin P3 with r rays per cell width), hence
+    sum ds = volume / per-ray cross-section, and the uniform-medium thick limit is unchanged."""
+    dims = (5, 4, 3)
+    kap, S = rand_fields(dims, 31)
+    dirs = np.array([[0.37, 1, 0.81], [1, 0.5, 0.25], [-1, 1, 1], [0.2, -0.3, -1], [0, -1, 0]], dtype=np.float64)
+    ref = bf.sweep(kap[0], S[0], dirs, Ibc=0.25, rays=rays)
+    r = orc.sweep(kap, S, dirs, Ibc=[0.25], count_dirs=range(len(dirs)), rays_per_cell=rays)
+    nx, ny, nz = dims
+    for i, n in enumerate(dirs):
+        cnt = np.zeros((nz, ny, nx), dtype=np.uint32)
+        for (x, y, z), c in ref["per_dir"][i]["cnt"].items():
+            cnt[z, y, x] = c
+        assert np.array_equal(cnt, r["cnt_dirs"][i])
+        L = orc.dir_record(n)["L"]
+        assert abs(r["min_den"][i] / (rays ** 2 * L) - 1) < 1e-12 and abs(r["max_den"][i] / (rays ** 2 * L) - 1) < 1e-12
+        assert abs(r["sum_ds"][i] / (nx * ny * nz * rays ** 2 * L) - 1) < 1e-12
+    Jin = np.zeros((nz, ny, nx))
+    for (x, y, z), v in ref["Jin"].items():
+        Jin[z, y, x] = v
+    assert np.allclose(r["Jin"][0], Jin, rtol=1e-12, atol=1e-15)
+    assert r["seg_total"] == sum(ref["cnt"].values())
+
+
+def test_p12_rays_per_cell_refines_the_same_quadrature(orc):
+    """In a uniform medium J_in of an interior cell is a smooth function of the ray offset, so r = 1, 2, 4
+    agree to the quadrature error and differences shrink with r; r is rejected unless a power of two."""
+    kap = np.full((1, 12, 12, 12), 0.3, dtype=np.float32)
+    S = np.ones_like(kap)
+    dirs = orc.healpix_dirs(1)
+    J = [orc.sweep(kap, S, dirs, rays_per_cell=r, want_counts=False)["Jin"][0, 6, 6, 6] for r in (1, 2, 4, 8)]
+    assert abs(J[1] - J[3]) < abs(J[0] - J[3]) and abs(J[2] - J[3]) < abs(J[1] - J[3])
+    assert abs(J[0] / J[3] - 1) < 0.05 and abs(J[2] / J[3] - 1) < 2e-3
+    with pytest.raises(RuntimeError):
+        orc.sweep(kap, S, dirs, rays_per_cell=3)
