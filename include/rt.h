@@ -70,7 +70,10 @@ int rt_healpix_dirs(int nside, double *dirs_out);
  *   nx, ny, nz    : mesh dimensions (x fastest)
  *   nbins         : frequency bins sharing one geometry (eq. 22), 1..16
  *   dirs, ndirs   : HOST, fp64 [ndirs][3], need not be normalised, none may be zero; copied
- *   rays_per_cell : rays per cell width in each transverse axis; only 1 is supported (RT_EINVAL otherwise)
+ *   rays_per_cell : r = rays per cell width in each transverse axis, i.e. ray spacing = dH / r;
+ *                   a power of two, 1..16 (RT_EINVAL otherwise).  r > 1 is swept as r^2 interleaved unit lattices
+ *                   with offsets (2 alpha + 1)/(2 r), each with its own slab program; per cell and direction
+ *                   sum ds = r^2 L, which the normalisation accounts for.  Cost and segment counts scale with r^2.
  *   cell_width    : mesh spacing dH (> 0); kappa is per unit length, so dtau = kappa * ds * dH
  *   flags         : RT_OWNED | RT_ATOMIC_ABLATION | RT_PAPER_GROUPS
  * Synchronises the device once (table build).  Returns RT_OK / RT_EINVAL / RT_ENOMEM / RT_ECUDA.
@@ -152,7 +155,7 @@ int rt_total_segments(rt_ctx *ctx, unsigned long long *n_host, void *cuda_stream
 /*
  * Per-direction record as quantised by the library (for cross-checks against the oracle).
  *   rec_host : HOST, long long [ndirs][6] = {dominant axis, reflect_x | reflect_y<<1 | reflect_z<<2,
- *              M_b, M_c, kernel path (0 = owned fast path, 1 = generic), 0}
+ *              M_b, M_c, kernel path (0 = owned fast path, 1 = generic), rays_per_cell}
  *   L_host   : HOST, fp64 [ndirs] slab length in cell widths, or NULL
  */
 int rt_direction_records(rt_ctx *ctx, long long *rec_host, double *L_host);

@@ -190,13 +190,14 @@ def rt_destroy(h):
 class RayTracer:
     """Owns one rt_ctx.  Fields and outputs are torch CUDA tensors [nbins][nz][ny][nx] fp32."""
 
-    def __init__(self, dims, nbins, dirs, cell_width=1.0, flags=RT_OWNED, slots=None, rows=None, stages=None, pair=None, tune=None):
+    def __init__(self, dims, nbins, dirs, cell_width=1.0, flags=RT_OWNED, slots=None, rows=None, stages=None, pair=None, tune=None,
+                 rays_per_cell=1):
         self.nx, self.ny, self.nz = (int(v) for v in dims)
         self.nbins = int(nbins)
         self.dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
         self.ndirs = self.dirs.shape[0]
         self.numel = self.nx * self.ny * self.nz * self.nbins
-        self.h = rt_create(self.nx, self.ny, self.nz, self.nbins, self.dirs, 1, cell_width, flags)
+        self.h = rt_create(self.nx, self.ny, self.nz, self.nbins, self.dirs, rays_per_cell, cell_width, flags)
         if slots is not None:
             rt_tune(self.h, "slots", slots)
         if rows is not None:

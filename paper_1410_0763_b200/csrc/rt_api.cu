@@ -33,10 +33,14 @@ struct HostDir {
     int layout;           // 0 native, 1 transposed
     int Na, Nb, Nc;
     double work;          // 1 + mb + mc
+    int parent;           // index of the direction in the caller's set
+    int sub;              // alpha | beta << 8 | r << 16 (rt_internal.h sub_offset)
 };
 
 struct rt_ctx {
     int nx = 0, ny = 0, nz = 0, nbins = 1, ndirs = 0;
+    int rays = 1;                    // r rays per cell width: every direction is r^2 unit sub-lattices ("virtual directions")
+    int nv = 0;                      // ndirs * r^2: hd, d_dirs, d_prog and the batch lists are indexed by virtual direction
     long long ncell = 0;
     double cell_width = 1.0;
     unsigned flags = 0;
@@ -134,7 +138,8 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     if (!out) return RT_EINVAL;
     *out = nullptr;
     if (nx < 1 || ny < 1 || nz < 1 || nbins < 1 || nbins > 16 || !dirs || ndirs < 1) return RT_EINVAL;
-    if (rays_per_cell != 1) return RT_EINVAL;
+    if (rays_per_cell < 1 || rays_per_cell > 16 || (rays_per_cell & (rays_per_cell - 1)) != 0) return RT_EINVAL;
+    if ((long long)ndirs * rays_per_cell * rays_per_cell > (1ll << 24)) return RT_EINVAL;
     if (!(cell_width > 0.0) || !std::isfinite(cell_width)) return RT_EINVAL;
     if (flags > 2u) return RT_EINVAL;
     if ((long long)nx * ny * nz >= (1ll << 31) || (long long)nx * ny * nz * nbins >= (1ll << 40)) return RT_EINVAL;
@@ -146,18 +151,21 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     rt_ctx *c = new (std::nothrow) rt_ctx;
     if (!c) return RT_ENOMEM;
     c->nx = nx; c->ny = ny; c->nz = nz; c->nbins = nbins; c->ndirs = ndirs;
+    c->rays = rays_per_cell;
+    const int r2 = rays_per_cell * rays_per_cell, nv = ndirs * r2;
+    c->nv = nv;
     c->ncell = (long long)nx * ny * nz; c->cell_width = cell_width; c->flags = flags;
     cudaGetDevice(&c->device);
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device);
     const int dims[3] = {nx, ny, nz};
 
     // ---- direction records (reading O2): plain IEEE fp64 operations in a fixed order
-    std::vector<DirDev> dd(ndirs);
-    std::vector<double> Lv(ndirs);
-    c->hd.resize(ndirs);
+    std::vector<DirDev> dd(nv);
+    std::vector<double> Lv(nv);
+    c->hd.resize(nv);
     long long prog_total = 0;
-    for (int i = 0; i < ndirs; ++i) {
-        const double *n = dirs + 3 * i;
+    for (int i = 0; i < nv; ++i) {
+        const double *n = dirs + 3 * (i / r2);
         const double ab[3] = {std::fabs(n[0]), std::fabs(n[1]), std::fabs(n[2])};
         if (!(ab[0] > 0.0 || ab[1] > 0.0 || ab[2] > 0.0) || !std::isfinite(ab[0] + ab[1] + ab[2])) { delete c; return RT_EINVAL; }
         HostDir h;
@@ -175,6 +183,8 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
         h.layout = (h.a == 0) ? 1 : 0;
         h.Na = dims[h.a]; h.Nb = dims[h.b]; h.Nc = dims[h.c];
         h.work = 1.0 + fb + fc;
+        h.parent = i / r2;
+        h.sub = rays_per_cell == 1 ? 0 : ((i % r2) % rays_per_cell) | (((i % r2) / rays_per_cell) << 8) | (rays_per_cell << 16);
         c->hd[i] = h;
         Lv[i] = h.L;
 
@@ -190,8 +200,8 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
         d.sj = h.refl[h.b] ? -1 : 1;           // st[h.b] == 1 by construction of the layouts
         d.Na = h.Na; d.Nb = h.Nb; d.Nc = h.Nc; d.layout = h.layout;
         d.prog_off = (int)prog_total;
-        d.invL = (float)(1.0 / (h.L * cell_width));
-        d.Mb = (int)h.Mb; d.Mc = (int)h.Mc; d.pad = 0;
+        d.invL = (float)(1.0 / (h.L * cell_width * (double)r2));      // per cell and direction sum ds = r^2 L (pin P3)
+        d.Mb = (int)h.Mb; d.Mc = (int)h.Mc; d.sub = h.sub;
         prog_total += h.Na;
         if (prog_total > 0x7fffffffll) { delete c; return RT_EINVAL; }
         dd[i] = d;
@@ -214,15 +224,15 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     for (int l = 0; l < 2; ++l) std::stable_sort(c->order[l].begin(), c->order[l].end(), by_class);
     // mirror pairs: same dominant axis, same reflections of a and c, same quantised slopes, opposite b
     {
-        typedef std::tuple<int, int, int, long long, long long> Key;
+        typedef std::tuple<int, int, int, long long, long long, int> Key;
         std::map<Key, std::vector<int>> pos, neg;
-        for (int i = 0; i < ndirs; ++i) {
+        for (int i = 0; i < nv; ++i) {
             const HostDir &h = c->hd[i];
             if (h.Mb == 0) continue;
-            Key k(h.a, h.refl[h.a], h.refl[h.c], h.Mb, h.Mc);
+            Key k(h.a, h.refl[h.a], h.refl[h.c], h.Mb, h.Mc, h.sub);     // same canonical sub-lattice offsets
             (h.refl[h.b] ? neg : pos)[k].push_back(i);
         }
-        std::vector<char> paired(ndirs, 0);
+        std::vector<char> paired(nv, 0);
         for (auto &kv : pos) {
             auto it = neg.find(kv.first);
             if (it == neg.end()) continue;
@@ -245,16 +255,16 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     }
 
 #define CKC(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { int rc__ = (e__ == cudaErrorMemoryAllocation) ? RT_ENOMEM : cuda_fail(e__); free_device(c); delete c; return rc__; } } while (0)
-    CKC(cudaMalloc(&c->d_dirs, sizeof(DirDev) * ndirs));
-    CKC(cudaMalloc(&c->d_L, sizeof(double) * ndirs));
+    CKC(cudaMalloc(&c->d_dirs, sizeof(DirDev) * nv));
+    CKC(cudaMalloc(&c->d_L, sizeof(double) * nv));
     CKC(cudaMalloc(&c->d_prog, sizeof(SlabProg) * prog_total));
-    CKC(cudaMalloc(&c->d_batch, sizeof(int) * 2 * ndirs));
+    CKC(cudaMalloc(&c->d_batch, sizeof(int) * 2 * nv));
     CKC(cudaMalloc(&c->d_Ibc, sizeof(float) * nbins));
     CKC(cudaMalloc(&c->d_red, sizeof(double) * 3));
     CKC(cudaMalloc(&c->d_u64, sizeof(unsigned long long)));
     CKC(cudaMemset(c->d_Ibc, 0, sizeof(float) * nbins));
-    CKC(cudaMemcpy(c->d_dirs, dd.data(), sizeof(DirDev) * ndirs, cudaMemcpyHostToDevice));
-    CKC(cudaMemcpy(c->d_L, Lv.data(), sizeof(double) * ndirs, cudaMemcpyHostToDevice));
+    CKC(cudaMemcpy(c->d_dirs, dd.data(), sizeof(DirDev) * nv, cudaMemcpyHostToDevice));
+    CKC(cudaMemcpy(c->d_L, Lv.data(), sizeof(double) * nv, cudaMemcpyHostToDevice));
     {
         std::vector<int> batch;
         for (int l = 0; l < 2; ++l) batch.insert(batch.end(), c->order[l].begin(), c->order[l].end());
@@ -264,7 +274,7 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
         }
         CKC(cudaMemcpy(c->d_batch, batch.data(), sizeof(int) * batch.size(), cudaMemcpyHostToDevice));
     }
-    CKC(launch_build_programs(c->d_dirs, ndirs, c->d_prog, cell_width, c->d_L, 0));
+    CKC(launch_build_programs(c->d_dirs, nv, c->d_prog, cell_width, c->d_L, 0));
     CKC(cudaEventCreate(&c->ev0));
     CKC(cudaEventCreate(&c->ev1));
     CKC(cudaDeviceSynchronize());
@@ -374,24 +384,25 @@ extern "C" int rt_set_inflow(rt_ctx *c, const float *I_bc_host)
 // number of slots of layout l that hold results afterwards.
 static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStream_t st, int *launches, int used[2])
 {
+    const int r2 = c->rays * c->rays;
     const size_t acc_bytes = sizeof(float) * (size_t)c->ncell * nbins;
     used[0] = used[1] = 0;
     for (int l = 0; l < 2; ++l) {
-        if (c->order[l].empty() || (only_dir >= 0 && c->hd[only_dir].layout != l)) continue;
+        if (c->order[l].empty() || (only_dir >= 0 && c->hd[(size_t)only_dir * r2].layout != l)) continue;
         const int S = (only_dir >= 0) ? 1 : c->slots[l];
         CK(cudaMemsetAsync(c->d_acc[l], 0, acc_bytes * S, st));
         CK(cudaMemsetAsync(c->d_accC[l], 0, acc_bytes * S, st));
     }
     if (mode == MODE_J) CK(cudaEventRecord(c->ev0, st));
     int off_all = 0;                 // position of the layout's list in d_batch: order[] region ...
-    int off_j = c->ndirs;            // ... and pairs[]/singles[] region
+    int off_j = c->nv;            // ... and pairs[]/singles[] region
     for (int l = 0; l < 2; ++l) {
         const int nd = (int)c->order[l].size();
         const int my_all = off_all, my_j = off_j;
         off_all += nd;
         off_j += (int)(c->pairs[l].size() + c->singles[l].size());
         if (nd == 0) continue;
-        if (only_dir >= 0 && c->hd[only_dir].layout != l) continue;
+        if (only_dir >= 0 && c->hd[(size_t)only_dir * r2].layout != l) continue;
         SweepLaunch L;
         memset(&L, 0, sizeof(L));
         L.P = c->d_P[l]; L.acc = c->d_acc[l]; L.accC = c->d_accC[l];
@@ -427,7 +438,7 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
                 while (i + n < nl && n < S && c->hd[list[i + n]].a == a && eff_rev(list[i + n]) == rev) ++n;
                 int first = i, count = n;
                 if (only_dir >= 0) {
-                    if (list[i] != only_dir) { i += 1; continue; }
+                    if (c->hd[list[i]].parent != only_dir) { i += 1; continue; }      // all r^2 sub-lattices, one by one
                     count = 1;
                 }
                 used[l] = std::max(used[l], count);
@@ -559,7 +570,7 @@ extern "C" int rt_sum_ds(rt_ctx *c, double *sum_host, double *min_host, double *
         int launches = 0, used[2];
         rc = run_traversal(c, MODE_DS, i, 1, st, &launches, used);
         if (rc != RT_OK) { cudaFree(d_all); return rc; }
-        const int l = c->hd[i].layout;
+        const int l = c->hd[(size_t)i * c->rays * c->rays].layout;
         e = launch_ds_reduce(d_all + 3 * i, c->d_acc[l], c->d_accC[l], c->ncell, st);
         if (e != cudaSuccess) { cudaFree(d_all); return cuda_fail(e); }
     }
@@ -579,13 +590,13 @@ extern "C" int rt_direction_records(rt_ctx *c, long long *rec, double *L_host)
 {
     if (!c || !rec) return RT_EINVAL;
     for (int i = 0; i < c->ndirs; ++i) {
-        const HostDir &h = c->hd[i];
+        const HostDir &h = c->hd[(size_t)i * c->rays * c->rays];
         rec[6 * i + 0] = h.a;
         rec[6 * i + 1] = h.refl[0] | (h.refl[1] << 1) | (h.refl[2] << 2);
         rec[6 * i + 2] = h.Mb;
         rec[6 * i + 3] = h.Mc;
         rec[6 * i + 4] = (c->fast[h.layout] && owned_supported(h.Nb, h.Nc, rows_for(c, h.layout))) ? 0 : 1;
-        rec[6 * i + 5] = 0;
+        rec[6 * i + 5] = c->rays;
         if (L_host) L_host[i] = h.L;
     }
     return RT_OK;

@@ -30,9 +30,18 @@ struct DirDev {
     int prog_off;        // index of the first SlabProg of this direction
     float invL;          // 1 / (L * cell_width)
     int Mb, Mc;          // quantised slopes (generic kernel recomputes the traversal per ray)
-    int pad;
+    int sub;             // sub-lattice of an r-rays-per-cell set: alpha | beta << 8 | r << 16 (0 = the r = 1 lattice)
 };
 static_assert(sizeof(DirDev) == 64, "DirDev layout");
+
+// Offset (in units of 2^-20 cells) of a sub-lattice's rays on the plane a = 0 along b (which = 0) or c (which = 1):
+// (2 alpha + 1) / (2 r) (reading O3).  r rays per cell width = r^2 unit lattices with these offsets.
+__host__ __device__ __forceinline__ int sub_offset(int sub, int which)
+{
+    const int r = (sub >> 16) > 0 ? (sub >> 16) : 1;
+    const int idx = which ? ((sub >> 8) & 255) : (sub & 255);
+    return (2 * idx + 1) * (int)(kOne / (2 * r));
+}
 
 enum Mode : int { MODE_J = 0, MODE_COUNT = 1, MODE_DS = 2 };
 

@@ -27,10 +27,10 @@ __global__ void k_build_programs(const DirDev *__restrict__ dirs, int ndirs, Sla
     if (k >= D.Na) return;
     const long long ONE = kOne;
     const long long Mb = D.Mb, Mc = D.Mc;
-    // fractional entry position inside the entry cell; the same for every lattice ray (offsets are
-    // whole cells): U = p*ONE + ONE/2 + k*Mb
-    const long long u = (ONE / 2 + (long long)k * Mb) & (ONE - 1);
-    const long long v = (ONE / 2 + (long long)k * Mc) & (ONE - 1);
+    // fractional entry position inside the entry cell; the same for every ray of the (sub-)lattice
+    // (offsets are whole cells): U = p*ONE + u0 + k*Mb, u0 = ONE/2 for one ray per cell
+    const long long u = ((long long)sub_offset(D.sub, 0) + (long long)k * Mb) & (ONE - 1);
+    const long long v = ((long long)sub_offset(D.sub, 1) + (long long)k * Mc) & (ONE - 1);
     const long long Db = ONE - u, Dc = ONE - v;          // distance to the next cell boundary, >= 1
     const bool crossb = (u + Mb > ONE), touchb = (u + Mb == ONE);
     const bool crossc = (v + Mc > ONE), touchc = (v + Mc == ONE);
@@ -204,10 +204,11 @@ k_sweep_generic(const SweepLaunch L, int np_max, int nq_max)
     const float *__restrict__ Pf = reinterpret_cast<const float *>(L.P);
     float *acc = L.acc + ((long long)slot * L.nbins) * L.ncell + foff;
     const float invL = (MODE == MODE_J) ? D.invL : 1.0f;
-    const float Lw = 1.0f / D.invL;
+    const int rr = (D.sub >> 16) > 0 ? (D.sub >> 16) : 1;
+    const float Lw = 1.0f / (D.invL * (float)(rr * rr));              // slab length L * cell_width (invL carries 1 / r^2)
     const bool rev = D.sj < 0;
     float I = L.Ibc[bin];
-    const long long U0 = (long long)p * ONE + ONE / 2, V0 = (long long)q * ONE + ONE / 2;
+    const long long U0 = (long long)p * ONE + sub_offset(D.sub, 0), V0 = (long long)q * ONE + sub_offset(D.sub, 1);
     for (int k = 0; k < D.Na; ++k) {
         const long long U = U0 + (long long)k * D.Mb, V = V0 + (long long)k * D.Mc;
         const long long j = U >> kF, l = V >> kF;

@@ -327,13 +327,13 @@ __device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned
 }
 
 // Row bookkeeping of one march, advanced slab by slab with adds only:
-//   frac = fractional part of 1/2 + k*m_c in units of 2^-20 (m_c = Mc / 2^20 <= 1)
+//   frac = fractional part of v0 + k*m_c in units of 2^-20, v0 = 1/2 for one ray per cell (m_c = Mc / 2^20 <= 1)
 //   lb   = (q0 + floor(1/2 + k*m_c)) mod Nc : memory row of the first ray row at slab k
 //   offk = k * sk                            : element offset of slab k
 struct RowState {
     int lb, offk;
     unsigned frac;
-    __device__ __forceinline__ void init(int q0) { lb = q0; offk = 0; frac = (unsigned)(kOne >> 1); }
+    __device__ __forceinline__ void init(int q0, int v0) { lb = q0; offk = 0; frac = (unsigned)v0; }
     // true iff the rays step along c inside the current slab (cross or exact touch)
     __device__ __forceinline__ bool steps(int Mc) const { return frac + (unsigned)Mc >= (unsigned)kOne; }
     __device__ __forceinline__ void advance(int Mc, int Nc, int sk)
@@ -413,7 +413,7 @@ k_sweep_tma(const SweepLaunch L)
     // The seam row's old accumulator is needed only by the CTA's last warp (the others add their seam
     // partial into the next warp's stage).
     RowState ps;
-    ps.init(q0);
+    ps.init(q0, sub_offset(Dp->sub, 1));
     auto produce = [&](int s) {
         if (lane == 0) {
             const unsigned st = wbase_s + s * SG::kStage, bar = bars + 8 * s;
@@ -454,7 +454,7 @@ k_sweep_tma(const SweepLaunch L)
     unsigned hand_par = 0;               // bit s: parity of the next completion of the incoming barrier of stage s
 
     RowState cs;
-    cs.init(q0);
+    cs.init(q0, sub_offset(Dp->sub, 1));
     SlabProg pr = prog[0];
     int s = 0;
     unsigned phase = 0;

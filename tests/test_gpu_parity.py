@@ -355,6 +355,41 @@ def test_direction_shards_combine(orc, world):
     assert rel_err(one, ref0).max() <= 1e-6
 
 
+@pytest.mark.parametrize("dims,rays,flags", [((64, 32, 16), 2, 0), ((32, 64, 24), 4, 0), ((20, 12, 10), 2, 0), ((32, 32, 8), 2, 1)])
+def test_rays_per_cell(orc, dims, rays, flags):
+    """r > 1 rays per cell width (ray spacing dH / r; reading O3/A13): r^2 interleaved unit
+    lattices.  Counts bit-exact (per direction and summed), sum ds = r^2 N_m L to 1e-6, J to 1e-5; owned
+    (mirror-pair) path, generic path and the atomic ablation."""
+    import paper_1410_0763_b200 as rt
+    torch = _torch()
+    kap, S = _rand(dims, 23, nb=2)
+    dirs = np.concatenate([orc.healpix_dirs(1), np.array([[1, 1, 1], [1, 0.5, 0.25], [0, -1, 0], [0.3, 0.2, -1]], dtype=np.float64)])
+    cd = [0, 5, 12, 13, 14, 15]
+    ref = orc.sweep(kap, S, dirs, Ibc=[0.3, 0.0], count_dirs=cd, rays_per_cell=rays)
+    tr = rt.RayTracer(dims, 2, dirs, flags=flags, rays_per_cell=rays)
+    try:
+        tr.set_inflow([0.3, 0.0])
+        tr.set_fields(torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda())
+        Jin = tr.sweep(what=rt.RT_J_IN).cpu().numpy()
+        J = tr.sweep(what=rt.RT_J_TOTAL).cpu().numpy()
+        cnt = tr.segment_counts(-1).cpu().numpy().astype(np.uint32)
+        cnt_d = np.stack([tr.segment_counts(i).cpu().numpy().astype(np.uint32) for i in cd])
+        nseg = tr.total_segments()
+        s, mn, mx = tr.sum_ds()
+        rec, L = tr.direction_records()
+    finally:
+        tr.close()
+    assert np.all(rec[:, 5] == rays)
+    assert np.array_equal(cnt, ref["cnt_sum"]) and nseg == ref["seg_total"]
+    assert np.array_equal(cnt_d, ref["cnt_dirs"])
+    ncell = dims[0] * dims[1] * dims[2]
+    assert np.abs(s / ref["sum_ds"] - 1).max() <= DS_TOL
+    assert np.abs(s / (ncell * rays ** 2 * L) - 1).max() <= DS_TOL
+    assert np.abs(mn / (rays ** 2 * L) - 1).max() <= 2e-6 and np.abs(mx / (rays ** 2 * L) - 1).max() <= 2e-6
+    assert rel_err(Jin, ref["Jin"]).max() <= J_TOL
+    assert rel_err(J, ref["J"]).max() <= J_TOL
+
+
 def test_degenerate_directions(orc):
     """Axis-aligned, exact diagonals, unit slopes, half slopes (crossings on slab planes), near-degenerate."""
     kap, S = _rand((32, 32, 32), 13)
@@ -387,7 +422,7 @@ def test_error_codes():
     import paper_1410_0763_b200 as rt
     torch = _torch()
     d = rt.healpix_dirs(1)
-    for bad in [dict(nx=0), dict(nbins=0), dict(nbins=17), dict(rays=2), dict(cw=0.0), dict(flags=7)]:
+    for bad in [dict(nx=0), dict(nbins=0), dict(nbins=17), dict(rays=3), dict(rays=32), dict(cw=0.0), dict(flags=7)]:
         with pytest.raises(rt.RtError) as ei:
             rt.rt_create(bad.get("nx", 8), 8, 8, bad.get("nbins", 1), d, bad.get("rays", 1), bad.get("cw", 1.0),
                          bad.get("flags", 0))
