@@ -42,6 +42,8 @@ struct rt_ctx {
     int rays = 1;                    // r rays per cell width: every direction is r^2 unit sub-lattices ("virtual directions")
     int nv = 0;                      // ndirs * r^2: hd, d_dirs, d_prog and the batch lists are indexed by virtual direction
     long long ncell = 0;
+    int pitch[2] = {0, 0};           // row pitch (cells) of the packed fields / accumulators of a layout: nx, ny padded to 32/64/128/256
+    long long ncell_l[2] = {0, 0};   // cells per bin of a layout including the pad columns
     double cell_width = 1.0;
     unsigned flags = 0;
     int device = 0;
@@ -158,6 +160,22 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     cudaGetDevice(&c->device);
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device);
     const int dims[3] = {nx, ny, nz};
+    // The owned kernel wants the memory-contiguous transverse extent to be 32/64/128/256: narrower or odd
+    // rows are padded to the next such width (pad cells hold kappa = 0, S = 0: a ray crossing them keeps
+    // its intensity and adds nothing, and a chain ray is replaced by the inflow where it wraps, after the pad).
+    {
+        const int NbL0[2] = {nx, ny};
+        for (int l = 0; l < 2; ++l) {
+            int p = NbL0[l];
+            if (flags == RT_OWNED && p <= 256) { p = 32; while (p < NbL0[l]) p *= 2; }
+            c->fast[l] = (flags == RT_OWNED) && NbL0[l] <= 256;
+            c->pitch[l] = p;
+            c->pp[l] = (c->fast[l] && p >= 64) ? 1 : 0;          // two columns per chunk
+        }
+        c->ncell_l[0] = (long long)c->pitch[0] * ny * nz;
+        c->ncell_l[1] = (long long)c->pitch[1] * nz * nx;
+        if (c->ncell_l[0] >= (1ll << 31) || c->ncell_l[1] >= (1ll << 31)) { delete c; return RT_EINVAL; }
+    }
 
     // ---- direction records (reading O2): plain IEEE fp64 operations in a fixed order
     std::vector<DirDev> dd(nv);
@@ -190,8 +208,8 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
 
         // strides of the canonical axes in the layout this direction sweeps
         long long st[3];                       // element stride of x, y, z
-        if (h.layout == 0) { st[0] = 1; st[1] = nx; st[2] = (long long)nx * ny; }          // [z][y][x]
-        else               { st[1] = 1; st[2] = ny; st[0] = (long long)ny * nz; }          // [x][z][y]
+        if (h.layout == 0) { st[0] = 1; st[1] = c->pitch[0]; st[2] = (long long)c->pitch[0] * ny; }          // [z][y][x]
+        else               { st[1] = 1; st[2] = c->pitch[1]; st[0] = (long long)c->pitch[1] * nz; }          // [x][z][y]
         DirDev d;
         d.sk = st[h.a]; d.sl = st[h.c];
         d.base = 0;
@@ -247,13 +265,6 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
                 else if (paired[i] == 0) c->singles[l].push_back(i);
             }
     }
-    // owned kernel: the memory-contiguous transverse extent must be 32/64/128/256 (one warp owns full rows)
-    const int NbL[2] = {nx, ny};
-    for (int l = 0; l < 2; ++l) {
-        c->fast[l] = (flags == RT_OWNED) && (NbL[l] == 32 || NbL[l] == 64 || NbL[l] == 128 || NbL[l] == 256);
-        c->pp[l] = (c->fast[l] && NbL[l] >= 64) ? 1 : 0;      // two columns per chunk
-    }
-
 #define CKC(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { int rc__ = (e__ == cudaErrorMemoryAllocation) ? RT_ENOMEM : cuda_fail(e__); free_device(c); delete c; return rc__; } } while (0)
     CKC(cudaMalloc(&c->d_dirs, sizeof(DirDev) * nv));
     CKC(cudaMalloc(&c->d_L, sizeof(double) * nv));
@@ -307,8 +318,8 @@ static int rows_for(const rt_ctx *c, int layout)
 static int ensure_buffers(rt_ctx *c)
 {
     if (c->buffers_ready) return RT_OK;
-    const size_t field_bytes = sizeof(float2) * (size_t)c->ncell * c->nbins;
-    const size_t acc_bytes = sizeof(float) * (size_t)c->ncell * c->nbins;
+    const size_t field_bytes_l[2] = {sizeof(float2) * (size_t)c->ncell_l[0] * c->nbins, sizeof(float2) * (size_t)c->ncell_l[1] * c->nbins};
+    const size_t acc_bytes_l[2] = {sizeof(float) * (size_t)c->ncell_l[0] * c->nbins, sizeof(float) * (size_t)c->ncell_l[1] * c->nbins};
     size_t freeb = 0, totalb = 0;
     CK(cudaMemGetInfo(&freeb, &totalb));
     // slots: enough concurrent directions to fill the machine, bounded by memory (1/3 of free)
@@ -325,7 +336,7 @@ static int ensure_buffers(rt_ctx *c)
                 const int rows = rows_for(c, l);
                 const int ctas_dir = ((Nc / rows + kOwnedWarpsPerCta - 1) / kOwnedWarpsPerCta) * c->nbins;
                 auto wave = [&](bool pair) {
-                    int per_sm = c->fast[l] ? owned_ctas_per_sm(l == 0 ? c->nx : c->ny, rows, c->stages, pair) : 0;
+                    int per_sm = c->fast[l] ? owned_ctas_per_sm(c->pitch[l], rows, c->stages, pair) : 0;
                     if (per_sm < 1) per_sm = 4;
                     const int resident = per_sm * c->sm_count;
                     return std::max(1, std::min(nd, resident / std::max(1, ctas_dir)));
@@ -336,8 +347,8 @@ static int ensure_buffers(rt_ctx *c)
                 if (!c->fast[l]) want = std::min(nd, 16);
             }
             const size_t budget = freeb / 3;
-            const size_t need_fixed = 2 * field_bytes;
-            size_t maxs = budget > need_fixed ? (budget - need_fixed) / (4 * acc_bytes) : 1;
+            const size_t need_fixed = field_bytes_l[0] + field_bytes_l[1];
+            size_t maxs = budget > need_fixed ? (budget - need_fixed) / (4 * acc_bytes_l[l]) : 1;
             if (maxs < 1) maxs = 1;
             want = (int)std::min<size_t>((size_t)want, maxs);
         }
@@ -347,12 +358,13 @@ static int ensure_buffers(rt_ctx *c)
     }
     for (int l = 0; l < 2; ++l) {
         {   // both packed copies are always kept (the pack kernel writes both in one pass)
-            cudaError_t e = cudaMalloc(&c->d_P[l], field_bytes);
+            cudaError_t e = cudaMalloc(&c->d_P[l], field_bytes_l[l]);
+            if (e == cudaSuccess) e = cudaMemset(c->d_P[l], 0, field_bytes_l[l]);      // pad cells stay zero
             if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RT_ENOMEM : cuda_fail(e);
         }
         if (c->slots[l] > 0) {
-            cudaError_t e = cudaMalloc(&c->d_acc[l], acc_bytes * c->slots[l]);
-            if (e == cudaSuccess) e = cudaMalloc(&c->d_accC[l], acc_bytes * c->slots[l]);
+            cudaError_t e = cudaMalloc(&c->d_acc[l], acc_bytes_l[l] * c->slots[l]);
+            if (e == cudaSuccess) e = cudaMalloc(&c->d_accC[l], acc_bytes_l[l] * c->slots[l]);
             if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RT_ENOMEM : cuda_fail(e);
         }
     }
@@ -366,7 +378,7 @@ extern "C" int rt_set_fields(rt_ctx *c, const float *kappa_dev, const float *S_d
     int rc = ensure_buffers(c);
     if (rc != RT_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    CK(launch_pack_fields(kappa_dev, S_dev, c->d_P[0], c->d_P[1], c->pp[0], c->pp[1], c->nx, c->ny, c->nz, c->nbins, st));
+    CK(launch_pack_fields(kappa_dev, S_dev, c->d_P[0], c->d_P[1], c->pp[0], c->pp[1], c->nx, c->ny, c->nz, c->pitch[0], c->pitch[1], c->nbins, st));
     c->fields_set = true;
     return RT_OK;
 }
@@ -385,11 +397,11 @@ extern "C" int rt_set_inflow(rt_ctx *c, const float *I_bc_host)
 static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStream_t st, int *launches, int used[2])
 {
     const int r2 = c->rays * c->rays;
-    const size_t acc_bytes = sizeof(float) * (size_t)c->ncell * nbins;
     used[0] = used[1] = 0;
     for (int l = 0; l < 2; ++l) {
         if (c->order[l].empty() || (only_dir >= 0 && c->hd[(size_t)only_dir * r2].layout != l)) continue;
         const int S = (only_dir >= 0) ? 1 : c->slots[l];
+        const size_t acc_bytes = sizeof(float) * (size_t)c->ncell_l[l] * nbins;
         CK(cudaMemsetAsync(c->d_acc[l], 0, acc_bytes * S, st));
         CK(cudaMemsetAsync(c->d_accC[l], 0, acc_bytes * S, st));
     }
@@ -406,9 +418,9 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
         SweepLaunch L;
         memset(&L, 0, sizeof(L));
         L.P = c->d_P[l]; L.acc = c->d_acc[l]; L.accC = c->d_accC[l];
-        L.dirs = c->d_dirs; L.prog = c->d_prog; L.nbins = nbins; L.ncell = c->ncell; L.Ibc = c->d_Ibc;
+        L.dirs = c->d_dirs; L.prog = c->d_prog; L.nbins = nbins; L.ncell = c->ncell_l[l]; L.Ibc = c->d_Ibc;
         L.rows = rows_for(c, l); L.mode = mode; L.stages = c->stages; L.handoff = c->handoff;
-        L.Nb = (l == 0) ? c->nx : c->ny; L.pp = c->pp[l];
+        L.Nb = c->pitch[l]; L.pp = c->pp[l];
         const bool owned_l = c->fast[l];
         // the lists this traversal walks: (direction list, position in d_batch, slots per launch, paired)
         struct Pass { const std::vector<int> *list; int off; int S; int pair; };
@@ -479,7 +491,7 @@ extern "C" int rt_sweep(rt_ctx *c, float *J_dev, unsigned what, void *stream)
     int rc = run_traversal(c, MODE_J, -1, c->nbins, st, &launches, used);
     if (rc != RT_OK) return rc;
     CK(launch_normalise(J_dev, c->d_P[0], c->pp[0], c->d_acc[0], c->d_accC[0], used[0], c->d_acc[1], c->d_accC[1], used[1],
-                        c->nx, c->ny, c->nz, c->nbins, what == RT_SUM_IN ? 1.0f : (float)(1.0 / (double)c->ndirs),
+                        c->nx, c->ny, c->nz, c->pitch[0], c->pitch[1], c->nbins, what == RT_SUM_IN ? 1.0f : (float)(1.0 / (double)c->ndirs),
                         what == RT_J_TOTAL ? 1 : 0, st));
     c->last_launches = launches + 1;
     return RT_OK;
@@ -489,7 +501,7 @@ extern "C" int rt_combine(rt_ctx *c, const float *sum_dev, long long ndirs_total
 {
     if (!c || !sum_dev || !J_dev || ndirs_total < 1 || what > 1u) return RT_EINVAL;
     if (!c->fields_set) return RT_ESTATE;
-    CK(launch_combine(J_dev, sum_dev, c->d_P[0], c->pp[0], (size_t)c->ncell * c->nbins, (float)(1.0 / (double)ndirs_total),
+    CK(launch_combine(J_dev, sum_dev, c->d_P[0], c->pp[0], (size_t)c->ncell * c->nbins, c->nx, c->pitch[0], (float)(1.0 / (double)ndirs_total),
                       what == RT_J_TOTAL ? 1 : 0, (cudaStream_t)stream));
     return RT_OK;
 }
@@ -512,7 +524,7 @@ extern "C" int rt_sweep_rates(rt_ctx *c, float *Gamma_dev, float *Heat_dev, cons
     int rc = run_traversal(c, MODE_J, -1, c->nbins, st, &launches, used);
     if (rc != RT_OK) return rc;
     CK(launch_rates(Gamma_dev, Heat_dev, c->d_P[0], c->pp[0], c->d_acc[0], c->d_accC[0], used[0], c->d_acc[1], c->d_accC[1],
-                    used[1], c->nx, c->ny, c->nz, c->nbins, (float)(1.0 / (double)c->ndirs), w4.data(), st));
+                    used[1], c->nx, c->ny, c->nz, c->pitch[0], c->pitch[1], c->nbins, (float)(1.0 / (double)c->ndirs), w4.data(), st));
     c->last_launches = launches + 1;
     return RT_OK;
 }
@@ -528,7 +540,7 @@ extern "C" int rt_segment_counts(rt_ctx *c, int dir_index, unsigned int *counts_
     rc = run_traversal(c, MODE_COUNT, dir_index, 1, st, &launches, used);
     if (rc != RT_OK) return rc;
     CK(launch_counts_finalise(counts_dev, c->d_acc[0], c->d_accC[0], used[0], c->d_acc[1], c->d_accC[1], used[1],
-                              c->nx, c->ny, c->nz, st));
+                              c->nx, c->ny, c->nz, c->pitch[0], c->pitch[1], st));
     return RT_OK;
 }
 
@@ -571,7 +583,7 @@ extern "C" int rt_sum_ds(rt_ctx *c, double *sum_host, double *min_host, double *
         rc = run_traversal(c, MODE_DS, i, 1, st, &launches, used);
         if (rc != RT_OK) { cudaFree(d_all); return rc; }
         const int l = c->hd[(size_t)i * c->rays * c->rays].layout;
-        e = launch_ds_reduce(d_all + 3 * i, c->d_acc[l], c->d_accC[l], c->ncell, st);
+        e = launch_ds_reduce(d_all + 3 * i, c->d_acc[l], c->d_accC[l], c->ncell_l[l], c->pitch[l], l == 0 ? c->nx : c->ny, st);
         if (e != cudaSuccess) { cudaFree(d_all); return cuda_fail(e); }
     }
     e = cudaMemcpyAsync(res.data(), d_all, sizeof(double) * res.size(), cudaMemcpyDeviceToHost, st);
@@ -595,7 +607,7 @@ extern "C" int rt_direction_records(rt_ctx *c, long long *rec, double *L_host)
         rec[6 * i + 1] = h.refl[0] | (h.refl[1] << 1) | (h.refl[2] << 2);
         rec[6 * i + 2] = h.Mb;
         rec[6 * i + 3] = h.Mc;
-        rec[6 * i + 4] = (c->fast[h.layout] && owned_supported(h.Nb, h.Nc, rows_for(c, h.layout))) ? 0 : 1;
+        rec[6 * i + 4] = (c->fast[h.layout] && owned_supported(c->pitch[h.layout], h.Nc, rows_for(c, h.layout))) ? 0 : 1;
         rec[6 * i + 5] = c->rays;
         if (L_host) L_host[i] = h.L;
     }

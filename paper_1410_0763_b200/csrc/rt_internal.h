@@ -80,7 +80,7 @@ __host__ __device__ __forceinline__ int field_s_offset(int pp) { return pp ? 2 :
 cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, SlabProg *prog, double cell_width,
                                   const double *Lvals, cudaStream_t st);
 cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat, float2 *PT, int ppN, int ppT,
-                               int nx, int ny, int nz, int nbins, cudaStream_t st);
+                               int nx, int ny, int nz, int nxp, int nyp, int nbins, cudaStream_t st);
 bool owned_supported(int Nb, int Nc, int rows);
 int owned_ctas_per_sm(int Nb, int rows, int stages, bool pair);
 constexpr int kOwnedWarpsPerCta = 4;
@@ -88,17 +88,18 @@ cudaError_t launch_sweep_owned(const SweepLaunch &L, cudaStream_t st);
 cudaError_t launch_sweep_generic(const SweepLaunch &L, int max_lattice_b, int max_lattice_c, cudaStream_t st);
 cudaError_t launch_normalise(float *J, const float2 *Pnat, int ppN, const float *accN, const float *accNC, int slotsN,
                              const float *accT, const float *accTC, int slotsT,
-                             int nx, int ny, int nz, int nbins, float inv_nd, int add_S, cudaStream_t st);
+                             int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, int add_S, cudaStream_t st);
 cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN, const float *accN, const float *accNC,
-                         int slotsN, const float *accT, const float *accTC, int slotsT, int nx, int ny, int nz, int nbins,
-                         float inv_nd, const float *w4, cudaStream_t st);
-cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int ppN, size_t n, float inv_nd, int add_S,
-                           cudaStream_t st);
+                         int slotsN, const float *accT, const float *accTC, int slotsT, int nx, int ny, int nz,
+                         int nxp, int nyp, int nbins, float inv_nd, const float *w4, cudaStream_t st);
+cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int ppN, size_t n, int nx, int nxp,
+                           float inv_nd, int add_S, cudaStream_t st);
 cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const float *accNC, int slotsN,
                                    const float *accT, const float *accTC, int slotsT,
-                                   int nx, int ny, int nz, cudaStream_t st);
+                                   int nx, int ny, int nz, int nxp, int nyp, cudaStream_t st);
 // per-cell sum of ds of ONE direction held in slot 0 of the given layout: writes {sum, min, max} (fp64)
-cudaError_t launch_ds_reduce(double *out3, const float *acc, const float *accC, long long ncell, cudaStream_t st);
+cudaError_t launch_ds_reduce(double *out3, const float *acc, const float *accC, long long ncell, int pitch, int width,
+                             cudaStream_t st);
 cudaError_t launch_sum_u32(unsigned long long *out, const unsigned *counts, long long n, cudaStream_t st);
 
 }  // namespace rt

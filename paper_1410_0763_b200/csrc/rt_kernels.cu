@@ -78,7 +78,8 @@ cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, SlabProg *prog,
 // Field packing: native copy and (x,y)-transposed copy, kappa floored at kKappaMin
 // ------------------------------------------------------------------------------------------------
 __global__ void k_pack_fields(const float *__restrict__ kappa, const float *__restrict__ S,
-                              float2 *__restrict__ Pnat, float2 *__restrict__ PT, int ppN, int ppT, int nx, int ny, int nz)
+                              float2 *__restrict__ Pnat, float2 *__restrict__ PT, int ppN, int ppT, int nx, int ny, int nz,
+                              int nxp, int nyp)
 {
     float *__restrict__ fN = reinterpret_cast<float *>(Pnat);
     float *__restrict__ fT = reinterpret_cast<float *>(PT);
@@ -87,12 +88,15 @@ __global__ void k_pack_fields(const float *__restrict__ kappa, const float *__re
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
     const size_t ncell = (size_t)nx * ny * nz;
     const size_t boff = (size_t)bin * ncell;
+    // rows of the packed copies have pitch nxp / nyp >= nx / ny (pad cells stay zero: kappa = 0 and S = 0
+    // leave a ray unchanged and add nothing to an accumulator)
+    const size_t boffN = (size_t)bin * nxp * ny * nz, boffT = (size_t)bin * nyp * nz * nx;
     for (int dy = threadIdx.y; dy < 32; dy += blockDim.y) {
         int x = x0 + threadIdx.x, y = y0 + dy;
         if (x < nx && y < ny) {
             size_t i = boff + ((size_t)z * ny + y) * nx + x;
             float2 v = make_float2(fmaxf(kappa[i], kKappaMin), S[i]);
-            const size_t o = field_index(i, ppN);
+            const size_t o = field_index(boffN + ((size_t)z * ny + y) * nxp + x, ppN);
             fN[o] = v.x; fN[o + field_s_offset(ppN)] = v.y;
             tile[dy][threadIdx.x] = v;
         }
@@ -102,17 +106,17 @@ __global__ void k_pack_fields(const float *__restrict__ kappa, const float *__re
         int x = x0 + dx, y = y0 + threadIdx.x;
         if (x < nx && y < ny) {
             const float2 v = tile[threadIdx.x][dx];
-            const size_t o = field_index(boff + ((size_t)x * nz + z) * ny + y, ppT);
+            const size_t o = field_index(boffT + ((size_t)x * nz + z) * nyp + y, ppT);
             fT[o] = v.x; fT[o + field_s_offset(ppT)] = v.y;
         }
     }
 }
 
 cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat, float2 *PT, int ppN, int ppT,
-                               int nx, int ny, int nz, int nbins, cudaStream_t st)
+                               int nx, int ny, int nz, int nxp, int nyp, int nbins, cudaStream_t st)
 {
     dim3 grid((nx + 31) / 32, (ny + 31) / 32, nz * nbins), block(32, 8);
-    k_pack_fields<<<grid, block, 0, st>>>(kappa, S, Pnat, PT, ppN, ppT, nx, ny, nz);
+    k_pack_fields<<<grid, block, 0, st>>>(kappa, S, Pnat, PT, ppN, ppT, nx, ny, nz, nxp, nyp);
     return cudaGetLastError();
 }
 
@@ -278,20 +282,21 @@ template <bool COUNTS>
 __global__ void k_finalise(float *__restrict__ J, unsigned *__restrict__ counts, const float2 *__restrict__ Pnat, int ppN,
                            const float *__restrict__ accN, const float *__restrict__ accNC, int slotsN,
                            const float *__restrict__ accT, const float *__restrict__ accTC, int slotsT,
-                           int nx, int ny, int nz, int nbins, float inv_nd, int add_S)
+                           int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, int add_S)
 {
     __shared__ float tile[32][33];
     const int bin = blockIdx.z / nz, z = blockIdx.z % nz;
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
     const size_t ncell = (size_t)nx * ny * nz;
-    const size_t slot_stride = ncell * nbins;
+    const size_t ncellN = (size_t)nxp * ny * nz, ncellT = (size_t)nyp * nz * nx;      // padded row pitch per layout
+    const size_t strideN = ncellN * nbins, strideT = ncellT * nbins;
     // transposed layout [x][z][y]: coalesced along y
     for (int dx = threadIdx.y; dx < 32; dx += blockDim.y) {
         const int x = x0 + dx, y = y0 + threadIdx.x;
         float s = 0.0f;
         if (x < nx && y < ny) {
-            const size_t i = (size_t)bin * ncell + ((size_t)x * nz + z) * ny + y;
-            for (int sl = 0; sl < slotsT; ++sl) s += accT[sl * slot_stride + i] + accTC[sl * slot_stride + i];
+            const size_t i = (size_t)bin * ncellT + ((size_t)x * nz + z) * nyp + y;
+            for (int sl = 0; sl < slotsT; ++sl) s += accT[sl * strideT + i] + accTC[sl * strideT + i];
         }
         tile[dx][threadIdx.x] = s;
     }
@@ -300,13 +305,14 @@ __global__ void k_finalise(float *__restrict__ J, unsigned *__restrict__ counts,
         const int x = x0 + threadIdx.x, y = y0 + dy;
         if (x < nx && y < ny) {
             const size_t i = (size_t)bin * ncell + ((size_t)z * ny + y) * nx + x;
+            const size_t ip = (size_t)bin * ncellN + ((size_t)z * ny + y) * nxp + x;
             float s = tile[threadIdx.x][dy];
-            for (int sl = 0; sl < slotsN; ++sl) s += accN[sl * slot_stride + i] + accNC[sl * slot_stride + i];
+            for (int sl = 0; sl < slotsN; ++sl) s += accN[sl * strideN + ip] + accNC[sl * strideN + ip];
             if (COUNTS) {
                 counts[i] = (unsigned)__float2uint_rn(s);
             } else {
                 const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
-                const size_t o = field_index(i, ppN);
+                const size_t o = field_index(ip, ppN);
                 const float2 ks = make_float2(fN[o], fN[o + field_s_offset(ppN)]);
                 const float jin = s * inv_nd / ks.x;
                 J[i] = add_S ? jin + ks.y : jin;
@@ -317,11 +323,11 @@ __global__ void k_finalise(float *__restrict__ J, unsigned *__restrict__ counts,
 
 cudaError_t launch_normalise(float *J, const float2 *Pnat, int ppN, const float *accN, const float *accNC, int slotsN,
                              const float *accT, const float *accTC, int slotsT,
-                             int nx, int ny, int nz, int nbins, float inv_nd, int add_S, cudaStream_t st)
+                             int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, int add_S, cudaStream_t st)
 {
     dim3 grid((nx + 31) / 32, (ny + 31) / 32, nz * nbins), block(32, 8);
     k_finalise<false><<<grid, block, 0, st>>>(J, nullptr, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT,
-                                              nx, ny, nz, nbins, inv_nd, add_S);
+                                              nx, ny, nz, nxp, nyp, nbins, inv_nd, add_S);
     return cudaGetLastError();
 }
 
@@ -335,13 +341,13 @@ struct RateWeights { float wG[16], lG[16], wH[16], lH[16]; };
 __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, const float2 *__restrict__ Pnat, int ppN,
                         const float *__restrict__ accN, const float *__restrict__ accNC, int slotsN,
                         const float *__restrict__ accT, const float *__restrict__ accTC, int slotsT,
-                        int nx, int ny, int nz, int nbins, float inv_nd, const RateWeights W)
+                        int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, const RateWeights W)
 {
     __shared__ float tile[32][33];
     const int z = blockIdx.z;
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
-    const size_t ncell = (size_t)nx * ny * nz;
-    const size_t slot_stride = ncell * nbins;
+    const size_t ncellN = (size_t)nxp * ny * nz, ncellT = (size_t)nyp * nz * nx;
+    const size_t strideN = ncellN * nbins, strideT = ncellT * nbins;
     const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
     float g[4] = {0.0f, 0.0f, 0.0f, 0.0f}, h[4] = {0.0f, 0.0f, 0.0f, 0.0f};      // rows threadIdx.y + 8 j
     for (int bin = 0; bin < nbins; ++bin) {
@@ -350,8 +356,8 @@ __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, con
             const int x = x0 + dx, y = y0 + threadIdx.x;
             float s = 0.0f;
             if (x < nx && y < ny) {
-                const size_t i = (size_t)bin * ncell + ((size_t)x * nz + z) * ny + y;
-                for (int sl = 0; sl < slotsT; ++sl) s += accT[sl * slot_stride + i] + accTC[sl * slot_stride + i];
+                const size_t i = (size_t)bin * ncellT + ((size_t)x * nz + z) * nyp + y;
+                for (int sl = 0; sl < slotsT; ++sl) s += accT[sl * strideT + i] + accTC[sl * strideT + i];
             }
             tile[dx][threadIdx.x] = s;
         }
@@ -360,9 +366,9 @@ __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, con
         for (int dy = threadIdx.y; dy < 32; dy += blockDim.y, ++j) {
             const int x = x0 + threadIdx.x, y = y0 + dy;
             if (x < nx && y < ny) {
-                const size_t i = (size_t)bin * ncell + ((size_t)z * ny + y) * nx + x;
+                const size_t i = (size_t)bin * ncellN + ((size_t)z * ny + y) * nxp + x;
                 float s = tile[threadIdx.x][dy];
-                for (int sl = 0; sl < slotsN; ++sl) s += accN[sl * slot_stride + i] + accNC[sl * slot_stride + i];
+                for (int sl = 0; sl < slotsN; ++sl) s += accN[sl * strideN + i] + accNC[sl * strideN + i];
                 const size_t o = field_index(i, ppN);
                 const float kap = fN[o], src = fN[o + field_s_offset(ppN)];
                 const float jin = s * inv_nd / kap;
@@ -384,7 +390,8 @@ __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, con
 }
 
 cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN, const float *accN, const float *accNC,
-                         int slotsN, const float *accT, const float *accTC, int slotsT, int nx, int ny, int nz, int nbins,
+                         int slotsN, const float *accT, const float *accTC, int slotsT, int nx, int ny, int nz,
+                         int nxp, int nyp, int nbins,
                          float inv_nd, const float *w4 /* host: wG, lG, wH, lH, each [nbins] */, cudaStream_t st)
 {
     RateWeights W;
@@ -394,8 +401,8 @@ cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN,
         W.wH[b] = in ? w4[2 * nbins + b] : 0.0f; W.lH[b] = in ? w4[3 * nbins + b] : 0.0f;
     }
     dim3 grid((nx + 31) / 32, (ny + 31) / 32, nz), block(32, 8);
-    k_rates<<<grid, block, 0, st>>>(Gamma, Heat, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT, nx, ny, nz, nbins,
-                                   inv_nd, W);
+    k_rates<<<grid, block, 0, st>>>(Gamma, Heat, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT, nx, ny, nz, nxp, nyp,
+                                   nbins, inv_nd, W);
     return cudaGetLastError();
 }
 
@@ -404,32 +411,33 @@ cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN,
 // shards have been added (all-reduce); J_in = sum / N_d (eq. 13), J = J_in + S (eq. 12).
 // ------------------------------------------------------------------------------------------------
 __global__ void k_combine(float *__restrict__ J, const float *__restrict__ sum, const float2 *__restrict__ Pnat, int ppN,
-                          size_t n, float inv_nd, int add_S)
+                          size_t n, int nx, int nxp, float inv_nd, int add_S)
 {
     const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         float v = sum[i] * inv_nd;
-        if (add_S) v += fN[field_index(i, ppN) + field_s_offset(ppN)];
+        const size_t ip = (i / nx) * nxp + (i % nx);              // rows of the packed copy have pitch nxp
+        if (add_S) v += fN[field_index(ip, ppN) + field_s_offset(ppN)];
         J[i] = v;
     }
 }
 
-cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int ppN, size_t n, float inv_nd, int add_S,
-                           cudaStream_t st)
+cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int ppN, size_t n, int nx, int nxp,
+                           float inv_nd, int add_S, cudaStream_t st)
 {
     size_t blocks = (n + 255) / 256;
     if (blocks > 148 * 16) blocks = 148 * 16;
-    k_combine<<<(unsigned)blocks, 256, 0, st>>>(J, sum, Pnat, ppN, n, inv_nd, add_S);
+    k_combine<<<(unsigned)blocks, 256, 0, st>>>(J, sum, Pnat, ppN, n, nx, nxp, inv_nd, add_S);
     return cudaGetLastError();
 }
 
 cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const float *accNC, int slotsN,
                                    const float *accT, const float *accTC, int slotsT,
-                                   int nx, int ny, int nz, cudaStream_t st)
+                                   int nx, int ny, int nz, int nxp, int nyp, cudaStream_t st)
 {
     dim3 grid((nx + 31) / 32, (ny + 31) / 32, nz), block(32, 8);
     k_finalise<true><<<grid, block, 0, st>>>(nullptr, counts, nullptr, 0, accN, accNC, slotsN, accT, accTC, slotsT,
-                                             nx, ny, nz, 1, 1.0f, 0);
+                                             nx, ny, nz, nxp, nyp, 1, 1.0f, 0);
     return cudaGetLastError();
 }
 
@@ -440,11 +448,13 @@ __device__ __forceinline__ double warp_sum(double v)
 }
 
 // out3 = {sum, min, max} over cells of (acc + accC); out3 must be pre-initialised to {0, +inf, 0}
-__global__ void k_ds_reduce(double *out3, const float *__restrict__ acc, const float *__restrict__ accC, long long ncell)
+__global__ void k_ds_reduce(double *out3, const float *__restrict__ acc, const float *__restrict__ accC, long long ncell,
+                            int pitch, int width)
 {
     double s = 0.0;
     float mn = 3.0e38f, mx = 0.0f;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < ncell; i += (long long)gridDim.x * blockDim.x) {
+        if ((int)(i % pitch) >= width) continue;                 // pad cells of a row
         const float v = acc[i] + accC[i];
         s += (double)v;
         mn = fminf(mn, v); mx = fmaxf(mx, v);
@@ -462,11 +472,12 @@ __global__ void k_ds_reduce(double *out3, const float *__restrict__ acc, const f
     }
 }
 
-cudaError_t launch_ds_reduce(double *out3, const float *acc, const float *accC, long long ncell, cudaStream_t st)
+cudaError_t launch_ds_reduce(double *out3, const float *acc, const float *accC, long long ncell, int pitch, int width,
+                             cudaStream_t st)
 {
     int blocks = (int)((ncell + 1023) / 1024);
     if (blocks > 592) blocks = 592;
-    k_ds_reduce<<<blocks, 256, 0, st>>>(out3, acc, accC, ncell);
+    k_ds_reduce<<<blocks, 256, 0, st>>>(out3, acc, accC, ncell, pitch, width);
     return cudaGetLastError();
 }
 

@@ -243,6 +243,24 @@ def test_generic_fallback_dims(orc, dims):
     check_full(orc, kap, S, dirs, out, ref)
 
 
+@pytest.mark.parametrize("dims,nb", [((100, 60, 24), 1), ((130, 200, 8), 1), ((33, 7, 5), 2), ((250, 31, 9), 1), ((300, 16, 8), 1)])
+def test_padded_rows_take_the_owned_path(orc, dims, nb):
+    """Row widths other than 32/64/128/256 are padded to the next such width (pad cells: kappa = 0, S = 0)
+    and swept by the owned kernel (mirror pairs, reversed singles and counting modes all cross the pad);
+    nx > 256 still falls back to the generic kernel for the layout it affects.  Same gates, with inflow."""
+    kap, S = _rand(dims, 29, nb=nb)
+    dirs = np.concatenate([orc.healpix_dirs(2), np.array([[1, 1, 1], [-1, 0.5, 0.25], [0.3, -1, 0]], dtype=np.float64)])
+    Ibc = [0.4, 0.1][:nb]
+    cd = [0, 7, 20, 33, 48, 49, 50]
+    out = gpu_run(kap, S, dirs, Ibc=Ibc, count_dirs=cd)
+    ref = orc.sweep(kap, S, dirs, Ibc=Ibc, count_dirs=cd)
+    check_records(orc, dirs, out)
+    layout_fast = {0: dims[0] <= 256, 1: dims[1] <= 256}
+    for i in range(len(dirs)):
+        assert out["rec"][i, 4] == (0 if layout_fast[1 if out["rec"][i, 0] == 0 else 0] else 1)
+    check_full(orc, kap, S, dirs, out, ref)
+
+
 @pytest.mark.parametrize("flags", [1, 2])
 def test_ablation_variants_pass_the_same_gates(orc, flags):
     """RT_ATOMIC_ABLATION and RT_PAPER_GROUPS differ from the owned path only by summation order."""
