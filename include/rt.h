@@ -96,6 +96,16 @@ int rt_set_fields(rt_ctx *ctx, const float *kappa_dev, const float *S_dev, void 
 int rt_set_inflow(rt_ctx *ctx, const float *I_bc_host);
 
 /*
+ * Boundary inflow per bin and entry face (boundary illumination as in the paper's Test 3).
+ *   I_face_host : HOST, fp32 [nbins][6], faces in the order -x, +x, -y, +y, -z, +z, each >= 0 and finite.
+ * A ray starts with the value of the face through which it enters the box, i.e. the face it crosses last: a
+ * ray marching towards +x that starts inside the transverse extent enters through -x; one that comes in from
+ * the side enters through that side face; through an edge (both side planes at once): the c-axis face
+ * (reading A10).  rt_set_inflow(v) is the same as all six faces = v.  Synchronous copy.
+ */
+int rt_set_inflow_faces(rt_ctx *ctx, const float *I_face_host);
+
+/*
  * One full sweep over all directions ("one iteration" of PAPER.md:322).
  *   J_dev : DEVICE, fp32 [nbins][nz][ny][nx], caller-owned, fully overwritten
  *   what  : RT_J_IN, RT_J_TOTAL or RT_SUM_IN

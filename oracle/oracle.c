@@ -125,6 +125,7 @@ typedef struct {
     size_t ncell;
     const float *kappa, *S;     /* [nbins][nz][ny][nx] */
     const double *Ibc;          /* [nbins] or NULL (=0) */
+    const double *Ibc6;         /* [nbins][6] per entry face (-x,+x,-y,+y,-z,+z) or NULL: overrides Ibc (A10) */
     double cell_width;
     int rays;                   /* r: rays per cell width in each transverse axis (O3, A13); 0 means 1 */
     /* per-direction scratch (owned by the calling thread) */
@@ -172,6 +173,19 @@ static void trace_ray(orc_work_t *w, const orc_dir_t *d, int64_t p, int64_t q)
     const double Lw = d->L * w->cell_width;
     double I[16];
     for (int bin = 0; bin < w->nbins; ++bin) I[bin] = w->Ibc ? w->Ibc[bin] : 0.0;
+    if (w->Ibc6) {
+        /* A10: the ray starts with the inflow of the face through which it enters the box, i.e. the
+           face it crosses last: the a-face if it starts inside the transverse extent, else the side
+           face (b or c) whose plane it reaches later (exact integers; both at once: c). */
+        const int64_t j0 = U0 >> ORC_F, l0 = V0 >> ORC_F;
+        int ax;
+        if (j0 >= 0 && l0 >= 0) ax = d->a;
+        else if (j0 >= 0) ax = d->c;
+        else if (l0 >= 0) ax = d->b;
+        else ax = ((-V0) * d->Mb >= (-U0) * d->Mc) ? d->c : d->b;
+        const int face = 2 * ax + (d->refl[ax] ? 1 : 0);            /* marching towards -axis enters through the + face */
+        for (int bin = 0; bin < w->nbins; ++bin) I[bin] = w->Ibc6[6 * bin + face];
+    }
     double chord = 0.0;
     size_t stride[3] = {1, (size_t)w->dims[0], (size_t)w->dims[0] * w->dims[1]};
 
@@ -273,9 +287,26 @@ static void sweep_direction(orc_work_t *w, const orc_dir_t *d)
  *   nthreads   : OpenMP threads over directions (<=0: default)
  * Returns 0, or <0 on bad arguments / allocation failure.
  */
+int orc_sweep_faces(int nx, int ny, int nz, int nbins, const float *kappa, const float *S, const double *dirs, int ndirs,
+                    const double *Ibc, const double *Ibc6, double cell_width, int rays, double *Jin, double *J,
+                    double *sum_ds, unsigned long long *seg_total, uint32_t *cnt_sum, const int *cnt_dirs, int ncnt,
+                    uint32_t *cnt_out, double *min_den, double *max_den, int nthreads);
+
 int orc_sweep_rays(int nx, int ny, int nz, int nbins,
               const float *kappa, const float *S,
               const double *dirs, int ndirs, const double *Ibc, double cell_width, int rays,
+              double *Jin, double *J, double *sum_ds, unsigned long long *seg_total,
+              uint32_t *cnt_sum, const int *cnt_dirs, int ncnt, uint32_t *cnt_out,
+              double *min_den, double *max_den, int nthreads)
+{
+    return orc_sweep_faces(nx, ny, nz, nbins, kappa, S, dirs, ndirs, Ibc, NULL, cell_width, rays, Jin, J, sum_ds,
+                           seg_total, cnt_sum, cnt_dirs, ncnt, cnt_out, min_den, max_den, nthreads);
+}
+
+/* as orc_sweep_rays, with an inflow intensity per bin and entry face: Ibc6 [nbins][6] or NULL */
+int orc_sweep_faces(int nx, int ny, int nz, int nbins,
+              const float *kappa, const float *S,
+              const double *dirs, int ndirs, const double *Ibc, const double *Ibc6, double cell_width, int rays,
               double *Jin, double *J, double *sum_ds, unsigned long long *seg_total,
               uint32_t *cnt_sum, const int *cnt_dirs, int ncnt, uint32_t *cnt_out,
               double *min_den, double *max_den, int nthreads)
@@ -296,7 +327,7 @@ int orc_sweep_rays(int nx, int ny, int nz, int nbins,
         memset(&w, 0, sizeof(w));
         w.dims[0] = nx; w.dims[1] = ny; w.dims[2] = nz;
         w.nbins = nbins; w.ncell = ncell; w.kappa = kappa; w.S = S; w.Ibc = Ibc; w.cell_width = cell_width;
-        w.rays = rays;
+        w.rays = rays; w.Ibc6 = Ibc6;
         w.num = (double *)calloc(ncell * nbins, sizeof(double));
         w.den = (double *)calloc(ncell, sizeof(double));
         w.cnt = (uint32_t *)calloc(ncell, sizeof(uint32_t));

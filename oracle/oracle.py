@@ -49,6 +49,9 @@ def lib():
         L.orc_sweep_rays.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, fp, fp, dp, C.c_int, dp, C.c_double, C.c_int,
                                      dp, dp, dp, C.POINTER(C.c_ulonglong), up, ip, C.c_int, up, dp, dp, C.c_int]
         L.orc_sweep_rays.restype = C.c_int
+        L.orc_sweep_faces.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, fp, fp, dp, C.c_int, dp, dp, C.c_double, C.c_int,
+                                      dp, dp, dp, C.POINTER(C.c_ulonglong), up, ip, C.c_int, up, dp, dp, C.c_int]
+        L.orc_sweep_faces.restype = C.c_int
         L.orc_trace_direction.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, fp, fp, dp, dp, C.c_double,
                                           ip, dp, dp, C.POINTER(C.c_long)]
         L.orc_trace_direction.restype = C.c_int
@@ -94,9 +97,10 @@ def dir_record(n) -> dict:
 
 
 def sweep(kappa, S, dirs, Ibc=None, cell_width: float = 1.0, count_dirs=(), nthreads: int = 0,
-          want_counts: bool = True, rays_per_cell: int = 1) -> dict:
+          want_counts: bool = True, rays_per_cell: int = 1, Ibc_faces=None) -> dict:
     """Full sweep.  Returns dict(Jin, J, sum_ds, seg_total, cnt_sum, cnt_dirs, min_den, max_den).
-    rays_per_cell = r: ray spacing = cell width / r in both transverse axes (O3, A13; a power of two)."""
+    rays_per_cell = r: ray spacing = cell width / r in both transverse axes (O3, A13; a power of two).
+    Ibc_faces [nbins][6]: inflow per bin and entry face (-x, +x, -y, +y, -z, +z), overrides Ibc (A10)."""
     kappa, S = _fields(kappa, S)
     nb, nz, ny, nx = kappa.shape
     dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
@@ -111,8 +115,9 @@ def sweep(kappa, S, dirs, Ibc=None, cell_width: float = 1.0, count_dirs=(), nthr
     cd = np.ascontiguousarray(list(count_dirs), dtype=np.int32)
     cnt_out = np.zeros((len(cd), nz, ny, nx), dtype=np.uint32) if len(cd) else None
     ibc = None if Ibc is None else np.ascontiguousarray(Ibc, dtype=np.float64)
-    rc = lib().orc_sweep_rays(nx, ny, nz, nb, _p(kappa, C.c_float), _p(S, C.c_float), _p(dirs, C.c_double), nd,
-                         _p(ibc, C.c_double), float(cell_width), int(rays_per_cell), _p(Jin, C.c_double), _p(J, C.c_double),
+    ibc6 = None if Ibc_faces is None else np.ascontiguousarray(Ibc_faces, dtype=np.float64).reshape(nb, 6)
+    rc = lib().orc_sweep_faces(nx, ny, nz, nb, _p(kappa, C.c_float), _p(S, C.c_float), _p(dirs, C.c_double), nd,
+                         _p(ibc, C.c_double), _p(ibc6, C.c_double), float(cell_width), int(rays_per_cell), _p(Jin, C.c_double), _p(J, C.c_double),
                          _p(sum_ds, C.c_double), C.byref(seg), _p(cnt_sum, C.c_uint32),
                          _p(cd, C.c_int) if len(cd) else None, len(cd), _p(cnt_out, C.c_uint32),
                          _p(min_den, C.c_double), _p(max_den, C.c_double), int(nthreads))

@@ -12,7 +12,7 @@ RT_OWNED, RT_ATOMIC_ABLATION, RT_PAPER_GROUPS = 0, 1, 2
 RT_J_IN, RT_J_TOTAL, RT_SUM_IN = 0, 1, 2
 
 EXPORTED_SYMBOLS = [
-    "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_sweep", "rt_combine", "rt_sweep_rates", "rt_segment_counts",
+    "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_set_inflow_faces", "rt_sweep", "rt_combine", "rt_sweep_rates", "rt_segment_counts",
     "rt_sum_ds", "rt_total_segments", "rt_direction_records", "rt_tune", "rt_last_launch_count",
     "rt_last_sweep_kernel_ms", "rt_destroy", "rt_strerror", "rt_last_cuda_error",
 ]
@@ -47,6 +47,8 @@ def load_library():
     L.rt_set_fields.restype = C.c_int
     L.rt_set_inflow.argtypes = [vp, fp]
     L.rt_set_inflow.restype = C.c_int
+    L.rt_set_inflow_faces.argtypes = [vp, fp]
+    L.rt_set_inflow_faces.restype = C.c_int
     L.rt_sweep.argtypes = [vp, vp, C.c_uint, vp]
     L.rt_sweep.restype = C.c_int
     L.rt_combine.argtypes = [vp, vp, C.c_longlong, C.c_uint, vp, vp]
@@ -133,6 +135,13 @@ def rt_set_inflow(h, Ibc):
     _check(load_library().rt_set_inflow(h, a.ctypes.data_as(C.POINTER(C.c_float))), "rt_set_inflow")
 
 
+def rt_set_inflow_faces(h, I_face, nbins):
+    a = np.ascontiguousarray(I_face, dtype=np.float32).reshape(-1)
+    if a.shape[0] != 6 * nbins:
+        raise ValueError("I_face must be [nbins][6]")
+    _check(load_library().rt_set_inflow_faces(h, a.ctypes.data_as(C.POINTER(C.c_float))), "rt_set_inflow_faces")
+
+
 def rt_sweep(h, J, numel, what=RT_J_IN, stream=None):
     import torch
     _check(load_library().rt_sweep(h, _dev_ptr(J, torch.float32, numel, "J"), int(what), _stream(stream)), "rt_sweep")
@@ -217,6 +226,9 @@ class RayTracer:
 
     def set_inflow(self, Ibc):
         rt_set_inflow(self.h, Ibc)
+
+    def set_inflow_faces(self, I_face):
+        rt_set_inflow_faces(self.h, I_face, self.nbins)
 
     def sweep(self, out=None, what=RT_J_IN, stream=None):
         import torch

@@ -216,7 +216,8 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
         if (h.refl[h.a]) { d.base += (long long)(h.Na - 1) * d.sk; d.sk = -d.sk; }
         if (h.refl[h.c]) { d.base += (long long)(h.Nc - 1) * d.sl; d.sl = -d.sl; }
         d.sj = h.refl[h.b] ? -1 : 1;           // st[h.b] == 1 by construction of the layouts
-        d.Na = h.Na; d.Nb = h.Nb; d.Nc = h.Nc; d.layout = h.layout;
+        d.Na = h.Na; d.Nb = h.Nb; d.Nc = h.Nc;
+        d.layout = h.layout | ((2 * h.a + h.refl[h.a]) << 8) | ((2 * h.b + h.refl[h.b]) << 12) | ((2 * h.c + h.refl[h.c]) << 16);
         d.prog_off = (int)prog_total;
         d.invL = (float)(1.0 / (h.L * cell_width * (double)r2));      // per cell and direction sum ds = r^2 L (pin P3)
         d.Mb = (int)h.Mb; d.Mc = (int)h.Mc; d.sub = h.sub;
@@ -270,10 +271,10 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     CKC(cudaMalloc(&c->d_L, sizeof(double) * nv));
     CKC(cudaMalloc(&c->d_prog, sizeof(SlabProg) * prog_total));
     CKC(cudaMalloc(&c->d_batch, sizeof(int) * 2 * nv));
-    CKC(cudaMalloc(&c->d_Ibc, sizeof(float) * nbins));
+    CKC(cudaMalloc(&c->d_Ibc, sizeof(float) * 6 * nbins));
     CKC(cudaMalloc(&c->d_red, sizeof(double) * 3));
     CKC(cudaMalloc(&c->d_u64, sizeof(unsigned long long)));
-    CKC(cudaMemset(c->d_Ibc, 0, sizeof(float) * nbins));
+    CKC(cudaMemset(c->d_Ibc, 0, sizeof(float) * 6 * nbins));
     CKC(cudaMemcpy(c->d_dirs, dd.data(), sizeof(DirDev) * nv, cudaMemcpyHostToDevice));
     CKC(cudaMemcpy(c->d_L, Lv.data(), sizeof(double) * nv, cudaMemcpyHostToDevice));
     {
@@ -386,8 +387,20 @@ extern "C" int rt_set_fields(rt_ctx *c, const float *kappa_dev, const float *S_d
 extern "C" int rt_set_inflow(rt_ctx *c, const float *I_bc_host)
 {
     if (!c || !I_bc_host) return RT_EINVAL;
-    for (int b = 0; b < c->nbins; ++b) if (!(I_bc_host[b] >= 0.0f) || !std::isfinite(I_bc_host[b])) return RT_EINVAL;
-    CK(cudaMemcpy(c->d_Ibc, I_bc_host, sizeof(float) * c->nbins, cudaMemcpyHostToDevice));
+    std::vector<float> six(6 * (size_t)c->nbins);
+    for (int b = 0; b < c->nbins; ++b) {
+        if (!(I_bc_host[b] >= 0.0f) || !std::isfinite(I_bc_host[b])) return RT_EINVAL;
+        for (int f = 0; f < 6; ++f) six[6 * (size_t)b + f] = I_bc_host[b];
+    }
+    CK(cudaMemcpy(c->d_Ibc, six.data(), sizeof(float) * six.size(), cudaMemcpyHostToDevice));
+    return RT_OK;
+}
+
+extern "C" int rt_set_inflow_faces(rt_ctx *c, const float *I_face_host)
+{
+    if (!c || !I_face_host) return RT_EINVAL;
+    for (int i = 0; i < 6 * c->nbins; ++i) if (!(I_face_host[i] >= 0.0f) || !std::isfinite(I_face_host[i])) return RT_EINVAL;
+    CK(cudaMemcpy(c->d_Ibc, I_face_host, sizeof(float) * 6 * c->nbins, cudaMemcpyHostToDevice));
     return RT_OK;
 }
 

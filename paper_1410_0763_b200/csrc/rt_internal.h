@@ -26,7 +26,8 @@ struct DirDev {
     long long sk, sl;    // signed element strides along canonical k (dominant axis) and l (transverse c)
     int sj;              // +1 / -1: rays move towards higher / lower memory columns
     int Na, Nb, Nc;      // extents along a, b (memory-contiguous axis of the layout), c
-    int layout;          // 0: native [z][y][x];  1: transposed [x][z][y] (x-dominant directions)
+    int layout;          // bits 0-3: 0 native [z][y][x], 1 transposed [x][z][y] (x-dominant directions); bits 8-10,
+                         // 12-14, 16-18: entry faces along a, b, c (face = 2 * axis + 1 if marching towards -axis)
     int prog_off;        // index of the first SlabProg of this direction
     float invL;          // 1 / (L * cell_width)
     int Mb, Mc;          // quantised slopes (generic kernel recomputes the traversal per ray)
@@ -55,7 +56,7 @@ struct SweepLaunch {
     int nslots;              // grid.y
     int nbins;               // grid.z
     long long ncell;
-    const float *Ibc;        // device [nbins]
+    const float *Ibc;        // device [nbins][6]: inflow per bin and entry face (-x, +x, -y, +y, -z, +z)
     int Nb, Nc;              // common to the batch (same layout => same Nb; Nc may differ per direction)
     int rows;                // rays rows per warp
     int mode;

@@ -211,8 +211,20 @@ k_sweep_generic(const SweepLaunch L, int np_max, int nq_max)
     const int rr = (D.sub >> 16) > 0 ? (D.sub >> 16) : 1;
     const float Lw = 1.0f / (D.invL * (float)(rr * rr));              // slab length L * cell_width (invL carries 1 / r^2)
     const bool rev = D.sj < 0;
-    float I = L.Ibc[bin];
     const long long U0 = (long long)p * ONE + sub_offset(D.sub, 0), V0 = (long long)q * ONE + sub_offset(D.sub, 1);
+    // inflow of the face the ray enters through = the face it crosses last: the a-face if it starts inside
+    // the transverse extent, else the side face whose plane it reaches later (both at once: c)
+    float I;
+    {
+        const int fa = (D.layout >> 8) & 7, fb = (D.layout >> 12) & 7, fc = (D.layout >> 16) & 7;
+        const bool inb = U0 >= 0, inc = V0 >= 0;
+        int f;
+        if (inb && inc) f = fa;
+        else if (inb) f = fc;
+        else if (inc) f = fb;
+        else f = ((-V0) * (long long)D.Mb >= (-U0) * (long long)D.Mc) ? fc : fb;
+        I = L.Ibc[6 * bin + f];
+    }
     for (int k = 0; k < D.Na; ++k) {
         const long long U = U0 + (long long)k * D.Mb, V = V0 + (long long)k * D.Mc;
         const long long j = U >> kF, l = V >> kF;

@@ -72,6 +72,11 @@ __device__ __forceinline__ void vshift_up(float2 &v, float in) { v.y = v.x; v.x 
 __device__ __forceinline__ void vshift_down(float &v, float in) { v = in; }
 __device__ __forceinline__ void vshift_down(float2 &v, float in) { v.x = v.y; v.y = in; }
 
+// per element: pad-column bit set ? alt : v   (bit 0 = memory element 0 of the chunk)
+__device__ __forceinline__ float  vpad(float v, float alt, unsigned m) { return (m & 1u) ? alt : v; }
+__device__ __forceinline__ float2 vpad(float2 v, float alt, unsigned m)
+{ return make_float2((m & 1u) ? alt : v.x, (m & 2u) ? alt : v.y); }
+
 __device__ __forceinline__ void unpack(const float2 &v, float &kap, float &src) { kap = v.x; src = v.y; }
 __device__ __forceinline__ void unpack(const float4 &v, float2 &kap, float2 &src)
 { kap = make_float2(v.x, v.y); src = make_float2(v.z, v.w); }     // pair-packed layout (rt_internal.h)
@@ -172,7 +177,8 @@ template <int CW, int G, int R, int MODE, int FLC, int V>
 __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>::T (&I)[R][G][(V == 2) ? 2 : 1],
                                           const unsigned char *__restrict__ sp, unsigned char *__restrict__ sa,
                                           const float len0, const float len1, const float len2,
-                                          const float Ibc, const float invL, const int lane, const int lwrap,
+                                          const float Ib0, const float Ib1, const float Ic, const float invL,
+                                          const int lane, const int lwrap, const unsigned padmask,
                                           float *const (&rowp)[R + 1], const Seam &seam)
 {
     using T = typename VT<CW>::T;
@@ -224,7 +230,7 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
                         // direction 0: hand every ray to the owner of the next column in canonical order
                         // (canonical lane + 1 is always the physical lane + 1); a new ray enters at
                         // canonical column 0.  Within a chunk, memory element 0 is upstream unless REV.
-                        float carry = Ibc;
+                        float carry = Ib0;               // inflow of the side face direction 0 enters through
 #pragma unroll
                         for (int g = 0; g < G; ++g) {
                             const float out = REV ? vfirst(Ir[g][0]) : vlast(Ir[g][0]);
@@ -236,7 +242,7 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
                         }
                         if (ND == 2) {
                             // mirrored direction: towards lower columns; a new ray enters the last column
-                            carry = Ibc;
+                            carry = Ib1;                 // the mirror image enters through the opposite face
 #pragma unroll
                             for (int g = G - 1; g >= 0; --g) {
                                 const float t = __shfl_sync(FULL, vfirst(Ir[g][ND - 1]), (lane + 1) & 31);
@@ -250,7 +256,8 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
 #pragma unroll
                         for (int g = 0; g < G; ++g)
 #pragma unroll
-                            for (int d = 0; d < ND; ++d) Ir[g][d] = vsplat<T>(Ibc);
+                            for (int d = 0; d < ND; ++d)           // pad columns hold rays that have yet to cross the b face
+                                Ir[g][d] = vpad(vsplat<T>(Ic), d == 0 ? Ib0 : Ib1, (padmask >> (g * CW)) & 3u);
                     }
                 }
                 if (fl & fsc) sel = true;
@@ -385,7 +392,10 @@ k_sweep_tma(const SweepLaunch L)
     const int q0 = q0c + wid * R;
     const int sk = (int)Dp->sk, sl = (int)Dp->sl;                // |offsets| < 2^31: checked by rt_create
     const float invL = (MODE == MODE_J) ? Dp->invL : 1.0f;
-    const float Ibc = L.Ibc[bin];
+    // inflow of the faces this slot's rays enter through (DirDev::layout carries the face indices)
+    const float *__restrict__ Ibin = L.Ibc + 6 * bin;
+    const int fcs = Dp->layout;
+    const float Ia = Ibin[(fcs >> 8) & 7], Ib0 = Ibin[(fcs >> 12) & 7], Ib1 = Ibin[((fcs >> 12) & 7) ^ 1], Ic = Ibin[(fcs >> 16) & 7];
     const SlabProg *__restrict__ prog = L.prog + Dp->prog_off;
 
     const long long foff = (long long)bin * L.ncell + Dp->base;
@@ -435,13 +445,22 @@ k_sweep_tma(const SweepLaunch L)
 #pragma unroll 1
     for (int kk = 0; kk < D && kk < Na; ++kk) produce(kk);
 
+    // Rows narrower than the template width are padded (rt_api.cu): a pad column carries a ray that has not yet
+    // crossed the b side face (it matters for rays moving towards lower columns, which cross the pad first), so
+    // it always holds that face's inflow: at the start and after a row wrap.
+    unsigned padmask = 0;
+#pragma unroll
+    for (int g = 0; g < G; ++g)
+#pragma unroll
+        for (int i = 0; i < CW; ++i)
+            if (CW * (REV ? 31 - lane : lane) + i + (REV ? (G - 1 - g) : g) * 32 * CW >= Dp->Nb) padmask |= 1u << (g * CW + i);
     T I[R][G][ND];
 #pragma unroll
     for (int r = 0; r < R; ++r)
 #pragma unroll
         for (int g = 0; g < G; ++g)
 #pragma unroll
-            for (int d = 0; d < ND; ++d) I[r][g][d] = vsplat<T>(Ibc);
+            for (int d = 0; d < ND; ++d) I[r][g][d] = vpad(vsplat<T>(Ia), d == 0 ? Ib0 : Ib1, (padmask >> (g * CW)) & 3u);
 
     // this lane's first memory column (canonical chunk 0 is memory chunk G-1 when REV)
     const int lcol = CW * (REV ? 31 - lane : lane);
@@ -487,7 +506,7 @@ k_sweep_tma(const SweepLaunch L)
             while (*landed_up < k + 1) { }
             mbar_wait(bars + SG::kWarpBytes + 8 * s, phase);     // acquire the copy's writes
         }
-        RT_DISPATCH_SLAB(fl, fl, I, sp, sa, len0, len1, len2, Ibc, invL, lane, lwrap, rowp, seam)
+        RT_DISPATCH_SLAB(fl, fl, I, sp, sa, len0, len1, len2, Ib0, Ib1, Ic, invL, lane, lwrap, padmask, rowp, seam)
         __syncwarp();                     // every lane is done with stage s
         if (k + D < Na) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");

@@ -76,8 +76,21 @@ def ray_intervals(dims, n, p, q, rays=1):
         idx[a] = Na - 1 - k if refl[a] else k
         idx[b] = Nb - 1 - j if refl[b] else j
         idx[c] = Nc - 1 - l if refl[c] else l
+        if not out:
+            # entry face: the boundary plane the entry point lies on (edge or corner of two side planes: c)
+            if s0 == 0:
+                ax = a
+            elif c0 + mc * s0 == 0:
+                ax = c
+            else:
+                assert b0 + mb * s0 == 0
+                ax = b
+            ENTRY_FACE[(tuple(n), p, q, rays)] = 2 * ax + (1 if refl[ax] else 0)
         out.append((tuple(idx), s1 - s0))
     return out, L
+
+
+ENTRY_FACE = {}
 
 
 def lattice(dims, n, rays=1):
@@ -92,7 +105,7 @@ def f_of(x):
     return 1.0 - 0.5 * x if x < 1e-8 else -math.expm1(-x) / x
 
 
-def sweep(kappa, S, dirs, Ibc=0.0, linear=False, rays=1):
+def sweep(kappa, S, dirs, Ibc=0.0, linear=False, rays=1, Ibc_faces=None):
     """kappa, S: nested [z][y][x] python/numpy arrays (single bin).  Returns dict of per-cell dicts.
 
     linear=True replaces eq. 7 by the optically thin limit I += kappa*S*ds and f by 1 (pin P6).
@@ -105,6 +118,8 @@ def sweep(kappa, S, dirs, Ibc=0.0, linear=False, rays=1):
         for (p, q) in lattice(dims, n, rays):
             iv, L = ray_intervals(dims, n, p, q, rays)
             I = float(Ibc)
+            if Ibc_faces is not None and iv:
+                I = float(Ibc_faces[ENTRY_FACE[(tuple(n), p, q, rays)]])
             chord = 0.0
             for (x, y, z), frac in iv:
                 ds = float(frac) * L

@@ -408,6 +408,33 @@ def test_rays_per_cell(orc, dims, rays, flags):
     assert rel_err(J, ref["J"]).max() <= J_TOL
 
 
+@pytest.mark.parametrize("dims,flags,rays", [((64, 32, 16), 0, 1), ((100, 60, 24), 0, 1), ((32, 64, 24), 0, 2), ((20, 12, 10), 2, 1), ((32, 32, 8), 1, 1)])
+def test_per_face_inflow(orc, dims, flags, rays):
+    """rt_set_inflow_faces (boundary illumination; reading A10): the ray chains of the owned
+    kernel (a-face at the start, b-face at the lane wrap - opposite faces for a mirror pair -, c-face at the
+    row wrap) and the per-ray rule of the generic kernel against the oracle; includes exact diagonals, where
+    a ray enters through an edge."""
+    import paper_1410_0763_b200 as rt
+    torch = _torch()
+    kap, S = _rand(dims, 37, nb=2)
+    kap *= 0.2                                           # thin enough that the inflow reaches every cell
+    dirs = np.concatenate([orc.healpix_dirs(2), np.array([[1, 1, 1], [-1, 1, -1], [1, -1, 0], [0, 0, -1], [0.5, 1, 0.5]], dtype=np.float64)])
+    faces = np.array([[0.1, 0.9, 0.3, 0.7, 0.5, 0.2], [1.5, 0.0, 0.0, 2.5, 0.25, 0.75]])
+    ref = orc.sweep(kap, S, dirs, Ibc_faces=faces, rays_per_cell=rays, want_counts=False)
+    tr = rt.RayTracer(dims, 2, dirs, flags=flags, rays_per_cell=rays)
+    try:
+        tr.set_inflow_faces(faces)
+        tr.set_fields(torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda())
+        Jin = tr.sweep(what=rt.RT_J_IN).cpu().numpy()
+        tr.set_inflow([0.4, 0.0])                        # back to one value per bin
+        Jin_u = tr.sweep(what=rt.RT_J_IN).cpu().numpy()
+    finally:
+        tr.close()
+    assert rel_err(Jin, ref["Jin"]).max() <= J_TOL
+    ref_u = orc.sweep(kap, S, dirs, Ibc=[0.4, 0.0], rays_per_cell=rays, want_counts=False)
+    assert rel_err(Jin_u, ref_u["Jin"]).max() <= J_TOL
+
+
 def test_degenerate_directions(orc):
     """Axis-aligned, exact diagonals, unit slopes, half slopes (crossings on slab planes), near-degenerate."""
     kap, S = _rand((32, 32, 32), 13)

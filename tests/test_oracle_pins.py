@@ -470,3 +470,33 @@ def test_p12_rays_per_cell_refines_the_same_quadrature(orc):
     assert abs(J[0] / J[3] - 1) < 0.05 and abs(J[2] / J[3] - 1) < 2e-3
     with pytest.raises(RuntimeError):
         orc.sweep(kap, S, dirs, rays_per_cell=3)
+
+
+# ---------------------------------------------------------------------------------------------
+# per-face inflow (A10)
+def test_p13_per_face_inflow_bruteforce_and_vacuum(orc):
+    """Inflow per entry face: (i) against the brute force, which finds the entry face from the exact
+    entry point (the boundary plane it lies on); (ii) in vacuum (kappa = 0, S = 0) every ray keeps its
+    inflow, so for one axis-aligned direction J_in is the inflow of the single upwind face everywhere;
+    (iii) six equal faces = the uniform inflow."""
+    dims = (5, 4, 3)
+    kap, S = rand_fields(dims, 41)
+    dirs = np.array([[0.37, 1, 0.81], [1, 0.5, 0.25], [-1, 1, 1], [0.2, -0.3, -1], [0, -1, 0], [-1, -0.999999, 0.5]], dtype=np.float64)
+    faces = [0.1, 0.9, 0.3, 0.7, 0.5, 0.2]
+    ref = bf.sweep(kap[0], S[0], [list(d) for d in dirs], Ibc_faces=faces)
+    r = orc.sweep(kap, S, dirs, Ibc_faces=[faces])
+    nx, ny, nz = dims
+    Jin = np.zeros((nz, ny, nx))
+    for (x, y, z), v in ref["Jin"].items():
+        Jin[z, y, x] = v
+    assert np.allclose(r["Jin"][0], Jin, rtol=1e-12, atol=1e-15)
+    vac = np.zeros((1, 3, 4, 5), dtype=np.float32)
+    for ax in range(3):
+        for sgn in (1, -1):
+            n = np.zeros((1, 3))
+            n[0, ax] = sgn
+            J = orc.sweep(vac, vac, n, Ibc_faces=[faces])["Jin"]
+            assert np.allclose(J, faces[2 * ax + (1 if sgn < 0 else 0)], rtol=1e-14)
+    a = orc.sweep(kap, S, dirs, Ibc=[0.6])["Jin"]
+    b = orc.sweep(kap, S, dirs, Ibc_faces=[[0.6] * 6])["Jin"]
+    assert np.allclose(a, b, rtol=1e-14, atol=0)            # (thread reduction order differs between runs)
