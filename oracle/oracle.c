@@ -547,3 +547,119 @@ int orc_num_threads(void)
     return 1;
 #endif
 }
+
+/* ================================================================================================
+ * Point radiation sources (section 2.1; Appendix 1) -- fp64.
+ *
+ * For every source alpha and every target cell one light-ray runs from the source to the centre of the
+ * cell (Fig. 1) and on through the cell.  tau = sum of kappa*ds over the cells crossed
+ * before the target cell (eq. 4's optical depth, up to the inner intersection r_in of Appendix 1),
+ * dtau = kappa_cell * (r_out - r_in).  Photon-conserving absorption rate per unit volume of the shell
+ * between r_in and r_out (eqs. A1-A3 divided by the shell volume; A5 is this divided by the species'
+ * number density):
+ *     Q[bin][cell] = sum_alpha  L[alpha][bin] * exp(-tau) * (1 - exp(-dtau)) / (4 pi/3 (r_out^3 - r_in^3))
+ * Readings: source positions are given in units of 1/256 cell (integers), so
+ * every decision of the traversal is exact integer arithmetic; a ray through an edge or corner steps all
+ * the axes involved at once (zero-length pieces dropped, as A3); the source's own cell has r_in = 0.
+ *   src_fix : int32 [nsrc][3] source positions in units of 1/256 cell width, inside the box
+ *   lum     : fp64 [nsrc][nbins]
+ *   Q       : fp64 [nbins][ncell] (may be NULL)
+ *   tau_out, dtau_out, rin_out, rout_out : fp64 [ncell] for source `diag_src` and bin `diag_bin` (may be NULL)
+ *   steps   : total number of positive-length segments marched (all sources, one bin)
+ */
+#define PS_FIX 256
+
+typedef struct { int64_t num, den; } ps_rat_t;      /* den > 0 */
+static int ps_less(ps_rat_t a, ps_rat_t b) { return (__int128)a.num * b.den < (__int128)b.num * a.den; }
+static int ps_equal(ps_rat_t a, ps_rat_t b) { return (__int128)a.num * b.den == (__int128)b.num * a.den; }
+
+int orc_point_sources(int nx, int ny, int nz, int nbins, const float *kappa, int nsrc, const int32_t *src_fix,
+                      const double *lum, double cell_width, double *Q, int diag_src, int diag_bin,
+                      double *tau_out, double *dtau_out, double *rin_out, double *rout_out,
+                      unsigned long long *steps, int nthreads)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || nbins < 1 || nbins > 16 || !kappa || nsrc < 1 || !src_fix || !lum) return -1;
+    const int dims[3] = {nx, ny, nz};
+    for (int a = 0; a < nsrc; ++a)
+        for (int i = 0; i < 3; ++i)
+            if (src_fix[3 * a + i] < 0 || src_fix[3 * a + i] > dims[i] * PS_FIX) return -1;
+    const size_t ncell = (size_t)nx * ny * nz;
+    const size_t stride[3] = {1, (size_t)nx, (size_t)nx * ny};
+    if (Q) memset(Q, 0, sizeof(double) * ncell * nbins);
+    unsigned long long nstep = 0;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+#pragma omp parallel for schedule(dynamic, 64) reduction(+ : nstep)
+    for (long long cidx = 0; cidx < (long long)ncell; ++cidx) {
+        int tgt[3] = {(int)(cidx % nx), (int)((cidx / nx) % ny), (int)(cidx / ((long long)nx * ny))};
+        for (int a = 0; a < nsrc; ++a) {
+            int64_t s[3], d[3];                                   /* source, and source -> cell centre, in 1/256 cells */
+            int cur[3], stp[3];
+            double len2 = 0.0;
+            for (int i = 0; i < 3; ++i) {
+                s[i] = src_fix[3 * a + i];
+                d[i] = ((int64_t)tgt[i] * PS_FIX + PS_FIX / 2) - s[i];
+                stp[i] = d[i] > 0 ? 1 : (d[i] < 0 ? -1 : 0);
+                len2 += (double)d[i] * (double)d[i];
+            }
+            const double len = sqrt(len2) / PS_FIX * cell_width;  /* |centre - source| */
+            /* cell containing the source, as seen from the ray: a source on a cell boundary belongs to the
+               cell the ray moves into (d[i] == 0 cannot happen on a boundary: centres are half-integers) */
+            for (int i = 0; i < 3; ++i) {
+                int64_t c = s[i] / PS_FIX;
+                if (s[i] % PS_FIX == 0 && stp[i] < 0) c -= 1;
+                cur[i] = (int)c;
+            }
+            double tau[16];
+            for (int b = 0; b < nbins; ++b) tau[b] = 0.0;
+            ps_rat_t u0 = {0, 1};                                  /* ray parameter: 0 at the source, 1 at the centre */
+            double r_in = 0.0, r_out = 0.0;
+            for (;;) {
+                /* next boundary crossing per axis: u_i = (plane_i - s_i) / d_i */
+                ps_rat_t un = {1, 0};                              /* +infinity */
+                int have = 0;
+                ps_rat_t ui[3];
+                for (int i = 0; i < 3; ++i) {
+                    if (stp[i] == 0) continue;
+                    int64_t plane = (int64_t)(cur[i] + (stp[i] > 0 ? 1 : 0)) * PS_FIX;
+                    ui[i].num = (plane - s[i]) * stp[i];
+                    ui[i].den = d[i] * stp[i];
+                    if (!have || ps_less(ui[i], un)) { un = ui[i]; have = 1; }
+                }
+                const int is_target = (cur[0] == tgt[0] && cur[1] == tgt[1] && cur[2] == tgt[2]);
+                const double t0 = (double)u0.num / (double)u0.den * len;
+                const double t1 = have ? (double)un.num / (double)un.den * len : t0;
+                const size_t cc = cur[0] * stride[0] + cur[1] * stride[1] + cur[2] * stride[2];
+                if (is_target) {
+                    r_in = t0; r_out = t1; nstep += 1;
+                    if (!have) { r_in = 0.0; r_out = 0.5 * cell_width; }   /* source at this cell's centre: inscribed sphere */
+                    break;
+                }
+                const double ds = t1 - t0;
+                if (ds > 0.0) {
+                    for (int b = 0; b < nbins; ++b) tau[b] += (double)kappa[(size_t)b * ncell + cc] * ds;
+                    nstep += 1;
+                }
+                for (int i = 0; i < 3; ++i)                        /* all axes that cross at u_next step together */
+                    if (stp[i] != 0 && ps_equal(ui[i], un)) cur[i] += stp[i];
+                u0 = un;
+            }
+            const double vol = 4.0 * 3.14159265358979323846 / 3.0 * (r_out * r_out * r_out - r_in * r_in * r_in);
+            for (int b = 0; b < nbins; ++b) {
+                const double dtau = (double)kappa[(size_t)b * ncell + cidx] * (r_out - r_in);
+                if (Q) Q[(size_t)b * ncell + cidx] += lum[(size_t)a * nbins + b] * exp(-tau[b]) * (-expm1(-dtau)) / vol;   /* A3 / V_shell */
+                if (a == diag_src && b == diag_bin) {
+                    if (tau_out) tau_out[cidx] = tau[b];
+                    if (dtau_out) dtau_out[cidx] = dtau;
+                }
+            }
+            if (a == diag_src) {
+                if (rin_out) rin_out[cidx] = r_in;
+                if (rout_out) rout_out[cidx] = r_out;
+            }
+        }
+    }
+    if (steps) *steps = nstep;
+    return 0;
+}

@@ -58,6 +58,9 @@ def lib():
         L.orc_sweep_cells.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, fp, fp, dp, C.c_int, dp, C.c_double,
                                       ip, C.c_int, dp, dp, up, C.c_int]
         L.orc_sweep_cells.restype = C.c_int
+        L.orc_point_sources.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, fp, C.c_int, ip, dp, C.c_double, dp, C.c_int, C.c_int,
+                                        dp, dp, dp, dp, C.POINTER(C.c_ulonglong), C.c_int]
+        L.orc_point_sources.restype = C.c_int
         L.orc_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -185,6 +188,31 @@ def rates(Jin, S, wG, lG, wH, lH):
         G += float(wG[b]) * Jin[b] + float(lG[b]) * S[b]
         H += float(wH[b]) * Jin[b] + float(lH[b]) * S[b]
     return G, H
+
+
+PS_FIX = 256        # source positions are given in units of 1/256 cell (exact integer traversal)
+
+
+def point_sources(kappa, src_fix, lum, cell_width: float = 1.0, diag=(0, 0), want_diag: bool = True, nthreads: int = 0) -> dict:
+    """Point radiation sources (PAPER.md:64-82 and Appendix 1): photon-conserving absorption rate per unit
+    shell volume Q [nbins][nz][ny][nx], and for source/bin `diag` the optical depth tau up to the target
+    cell, dtau across it and the radii r_in, r_out of Appendix 1.  src_fix: int [nsrc][3] in 1/256 cells."""
+    kappa = np.ascontiguousarray(kappa, dtype=np.float32)
+    if kappa.ndim == 3:
+        kappa = kappa[None]
+    nb, nz, ny, nx = kappa.shape
+    src = np.ascontiguousarray(src_fix, dtype=np.int32).reshape(-1, 3)
+    lum = np.ascontiguousarray(lum, dtype=np.float64).reshape(src.shape[0], nb)
+    Q = np.empty(kappa.shape, dtype=np.float64)
+    d = [np.empty((nz, ny, nx), dtype=np.float64) if want_diag else None for _ in range(4)]
+    steps = C.c_ulonglong(0)
+    rc = lib().orc_point_sources(nx, ny, nz, nb, _p(kappa, C.c_float), src.shape[0], _p(src, C.c_int), _p(lum, C.c_double),
+                                 float(cell_width), _p(Q, C.c_double), int(diag[0]), int(diag[1]),
+                                 _p(d[0], C.c_double), _p(d[1], C.c_double), _p(d[2], C.c_double), _p(d[3], C.c_double),
+                                 C.byref(steps), int(nthreads))
+    if rc != 0:
+        raise RuntimeError("orc_point_sources failed: %d" % rc)
+    return {"Q": Q, "tau": d[0], "dtau": d[1], "r_in": d[2], "r_out": d[3], "steps": int(steps.value)}
 
 
 def num_threads() -> int:

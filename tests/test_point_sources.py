@@ -1,0 +1,120 @@
+"""Point radiation sources (Appendix 1): pins of the oracle (CPU) and parity of the CUDA
+path against it (GPU)."""
+import math
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+FIX = 256
+
+
+def brute_ray(dims, kap, src_fix, tgt):
+    """Independent algorithm: all plane crossings of the line source -> cell centre (and beyond) as exact
+    rationals, sorted globally; every interval is classified by the cell its midpoint lies in.
+    Returns (tau up to the target cell, r_in, r_out) with lengths in cell widths."""
+    s = [Fraction(int(v), FIX) for v in src_fix]
+    c = [Fraction(2 * t + 1, 2) for t in tgt]
+    d = [ci - si for ci, si in zip(c, s)]
+    ln = math.sqrt(float(sum(x * x for x in d)))
+    if all(x == 0 for x in d):
+        return 0.0, 0.0, 0.5
+    ev = {Fraction(0)}
+    for i in range(3):
+        if d[i] != 0:
+            for plane in range(0, dims[i] + 1):
+                u = (Fraction(plane) - s[i]) / d[i]
+                if u > 0:
+                    ev.add(u)
+    ev = sorted(ev)
+    tau, r_in, r_out = 0.0, None, None
+    for u0, u1 in zip(ev[:-1], ev[1:]):
+        mid = (u0 + u1) / 2
+        cell = tuple(math.floor(s[i] + d[i] * mid) for i in range(3))
+        if cell == tuple(tgt):
+            if r_in is None:
+                r_in = float(u0) * ln
+            r_out = float(u1) * ln
+        elif r_in is None:
+            if all(0 <= cell[i] < dims[i] for i in range(3)):
+                tau += float(kap[cell[2], cell[1], cell[0]]) * float(u1 - u0) * ln
+        else:
+            break
+    return tau, r_in, r_out
+
+
+SOURCES = [[0, 0, 0], [5 * FIX, 4 * FIX, 3 * FIX], [2 * FIX + 128, 1 * FIX + 128, 1 * FIX + 128], [3 * FIX, 2 * FIX + 128, 77],
+           [1 * FIX + 10, 3 * FIX + 200, 2 * FIX + 31], [0, 2 * FIX, 3 * FIX]]
+
+
+def test_ps1_bruteforce_tau_and_radii(orc):
+    """tau, r_in, r_out of every (source, cell) pair against the global event sort with exact rationals;
+    sources at a box corner, the opposite corner, a cell centre, on a face, generic, on an edge."""
+    dims = (5, 4, 3)
+    rng = np.random.default_rng(51)
+    kap = rng.uniform(0.05, 2.0, (1, 3, 4, 5)).astype(np.float32)
+    for si, src in enumerate(SOURCES):
+        r = orc.point_sources(kap, SOURCES, np.ones((len(SOURCES), 1)), diag=(si, 0))
+        for z in range(3):
+            for y in range(4):
+                for x in range(5):
+                    tau, r_in, r_out = brute_ray(dims, kap[0], src, (x, y, z))
+                    assert abs(r["tau"][z, y, x] - tau) <= 1e-12 * max(1.0, tau)
+                    assert abs(r["r_in"][z, y, x] - r_in) <= 1e-12 and abs(r["r_out"][z, y, x] - r_out) <= 1e-12
+                    assert abs(r["dtau"][z, y, x] - float(kap[0, z, y, x]) * (r_out - r_in)) <= 1e-12
+
+
+def test_ps2_uniform_medium_closed_forms(orc):
+    """Uniform kappa: tau = kappa r_in exactly (eq. 4's optical depth of a straight path), and Q of a single
+    source is L e^{-kappa r_in} (1 - e^{-kappa (r_out - r_in)}) / (4 pi/3 (r_out^3 - r_in^3)) (eqs. A1-A3);
+    sources add linearly; cell_width scales lengths."""
+    kap = np.full((2, 6, 7, 8), 0.3, dtype=np.float32)
+    kap[1] = 1.7
+    src = [[0, 0, 0], [8 * FIX, 3 * FIX + 128, 100]]
+    lum = np.array([[2.0, 0.5], [1.0, 3.0]])
+    for cw in (1.0, 0.4):
+        ra = orc.point_sources(kap, src[:1], lum[:1], cell_width=cw)
+        rb = orc.point_sources(kap, src[1:], lum[1:], cell_width=cw)
+        rab = orc.point_sources(kap, src, lum, cell_width=cw, diag=(0, 1))
+        assert np.allclose(rab["Q"], ra["Q"] + rb["Q"], rtol=1e-13)
+        k1 = float(kap[1, 0, 0, 0])
+        assert np.allclose(rab["tau"], k1 * rab["r_in"], rtol=1e-12, atol=1e-14)
+        for b in range(2):
+            k = float(kap[b, 0, 0, 0])
+            q = lum[0, b] * np.exp(-k * ra["r_in"]) * (1 - np.exp(-k * (ra["r_out"] - ra["r_in"]))) / \
+                (4 * math.pi / 3 * (ra["r_out"] ** 3 - ra["r_in"] ** 3))
+            assert np.allclose(ra["Q"][b], q, rtol=1e-12)
+    # geometry: the ray to a cell centre passes the centre between r_in and r_out, at distance |c - s|
+    r = orc.point_sources(kap, src[:1], lum[:1])
+    z, y, x = np.meshgrid(np.arange(6), np.arange(7), np.arange(8), indexing="ij")
+    dist = np.sqrt((x + 0.5) ** 2 + (y + 0.5) ** 2 + (z + 0.5) ** 2)
+    assert np.all(r["r_in"] < dist) and np.all(dist < r["r_out"])
+
+
+def test_ps3_thin_limit_is_the_inverse_square_law(orc):
+    """kappa -> 0: Q / kappa -> L / (4 pi/3 (r_out^2 + r_out r_in + r_in^2)), i.e. L / (4 pi r^2) (eq. 4) to
+    O((dr/r)^2) far from the source."""
+    kap = np.full((1, 16, 16, 16), 1e-9, dtype=np.float32)
+    r = orc.point_sources(kap, [[0, 0, 0]], [[5.0]])
+    k = float(kap[0, 0, 0, 0])
+    exact = 5.0 / (4 * math.pi / 3 * (r["r_out"] ** 2 + r["r_out"] * r["r_in"] + r["r_in"] ** 2))
+    assert np.allclose(r["Q"][0] / k, exact, rtol=1e-7)
+    z, y, x = np.meshgrid(np.arange(16), np.arange(16), np.arange(16), indexing="ij")
+    d2 = (x + 0.5) ** 2 + (y + 0.5) ** 2 + (z + 0.5) ** 2
+    far = d2 > 100
+    assert np.abs(r["Q"][0][far] / k / (5.0 / (4 * math.pi * d2[far])) - 1).max() < 0.02
+
+
+def test_ps4_mirror_symmetry(orc):
+    """Mirroring the field and the source along an axis mirrors Q."""
+    rng = np.random.default_rng(52)
+    kap = rng.uniform(0.05, 1.0, (1, 4, 5, 6)).astype(np.float32)
+    src = np.array([[1 * FIX + 40, 2 * FIX, 3 * FIX + 128]])
+    q = orc.point_sources(kap, src, [[1.0]], want_diag=False)["Q"]
+    dims = (6, 5, 4)
+    for ax in range(3):
+        km = np.ascontiguousarray(np.flip(kap, axis=3 - ax))
+        sm = src.copy()
+        sm[0, ax] = dims[ax] * FIX - src[0, ax]
+        qm = orc.point_sources(km, sm, [[1.0]], want_diag=False)["Q"]
+        assert np.allclose(np.flip(qm, axis=3 - ax), q, rtol=1e-12)
