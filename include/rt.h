@@ -146,6 +146,28 @@ int rt_sweep_rates(rt_ctx *ctx, float *Gamma_dev, float *Heat_dev, const double 
                    const double *wH, const double *lH, void *cuda_stream);
 
 /*
+ * RT from point radiation sources (section 2.1) with the photon-conserving estimate of
+ * Appendix 1: one light-ray per (source, cell) from the source through the cell centre
+ * (long characteristics; cost N_m^(4/3) per source).  With tau the optical depth of the cells
+ * crossed before the target cell, r_in / r_out the distances at which the ray enters / leaves the target cell
+ * and dtau = kappa_cell (r_out - r_in), per cell and bin
+ *     Q = sum_alpha  L[alpha][bin] exp(-tau) (1 - exp(-dtau)) / (4 pi/3 (r_out^3 - r_in^3))       (eqs. A1-A3 / shell volume)
+ * i.e. the absorption rate per unit volume; eq. A5's rate of species i is Q (dtau_i/dtau) / (n_i h nu).
+ * Uses the kappa of the last rt_set_fields (S is not used).  Lengths are in units of cell_width.
+ *   src_fix_host : HOST, int32 [nsrc][3], source positions in units of 1/256 cell width (0 .. 256*dim), so that
+ *                  the traversal is exact; a source on a cell boundary belongs to the cell a ray moves into; the
+ *                  cell whose centre IS the source uses r_in = 0, r_out = cell_width/2
+ *   lum_host     : HOST, fp64 [nsrc][nbins] luminosities (>= 0, converted to fp32)
+ *   Q_dev        : DEVICE, fp32 [nbins][nz][ny][nx], fully overwritten
+ *   tau_dev      : DEVICE, fp32 [nz][ny][nx] or NULL: tau of source diag_src in bin diag_bin (diagnostic)
+ *   steps_host   : HOST or NULL: number of positive-length ray pieces marched per bin, all sources (integer
+ *                  traversal data for the parity gate)
+ * Mesh dimensions must be <= 1024 (RT_EINVAL).  Synchronises the stream before returning.
+ */
+int rt_point_sources(rt_ctx *ctx, const int *src_fix_host, const double *lum_host, int nsrc, float *Q_dev,
+                     int diag_src, int diag_bin, float *tau_dev, unsigned long long *steps_host, void *cuda_stream);
+
+/*
  * Diagnostics required by the parity gates (integer traversal data, summed ds).  They run the same
  * traversal kernel as rt_sweep with the transfer arithmetic replaced by counting.
  *

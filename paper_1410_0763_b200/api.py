@@ -12,7 +12,7 @@ RT_OWNED, RT_ATOMIC_ABLATION, RT_PAPER_GROUPS = 0, 1, 2
 RT_J_IN, RT_J_TOTAL, RT_SUM_IN = 0, 1, 2
 
 EXPORTED_SYMBOLS = [
-    "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_set_inflow_faces", "rt_sweep", "rt_combine", "rt_sweep_rates", "rt_segment_counts",
+    "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_set_inflow_faces", "rt_sweep", "rt_combine", "rt_sweep_rates", "rt_point_sources", "rt_segment_counts",
     "rt_sum_ds", "rt_total_segments", "rt_direction_records", "rt_tune", "rt_last_launch_count",
     "rt_last_sweep_kernel_ms", "rt_destroy", "rt_strerror", "rt_last_cuda_error",
 ]
@@ -55,6 +55,8 @@ def load_library():
     L.rt_combine.restype = C.c_int
     L.rt_sweep_rates.argtypes = [vp, vp, vp, dp, dp, dp, dp, vp]
     L.rt_sweep_rates.restype = C.c_int
+    L.rt_point_sources.argtypes = [vp, C.POINTER(C.c_int), dp, C.c_int, vp, C.c_int, C.c_int, vp, C.POINTER(C.c_ulonglong), vp]
+    L.rt_point_sources.restype = C.c_int
     L.rt_segment_counts.argtypes = [vp, C.c_int, vp, vp]
     L.rt_segment_counts.restype = C.c_int
     L.rt_sum_ds.argtypes = [vp, dp, dp, dp, vp]
@@ -164,6 +166,18 @@ def rt_sweep_rates(h, Gamma, Heat, ncell, nbins, wG, lG, wH, lH, stream=None):
                                          _stream(stream)), "rt_sweep_rates")
 
 
+def rt_point_sources(h, src_fix, lum, Q, numel, nbins, tau=None, diag=(0, 0), want_steps=False, stream=None):
+    import torch
+    src = np.ascontiguousarray(src_fix, dtype=np.int32).reshape(-1, 3)
+    lum = np.ascontiguousarray(lum, dtype=np.float64).reshape(src.shape[0], nbins)
+    steps = C.c_ulonglong(0)
+    _check(load_library().rt_point_sources(h, src.ctypes.data_as(C.POINTER(C.c_int)), lum.ctypes.data_as(C.POINTER(C.c_double)),
+                                           src.shape[0], _dev_ptr(Q, torch.float32, numel, "Q"), int(diag[0]), int(diag[1]),
+                                           None if tau is None else _dev_ptr(tau, torch.float32, numel // nbins, "tau"),
+                                           C.byref(steps) if want_steps else None, _stream(stream)), "rt_point_sources")
+    return int(steps.value)
+
+
 def rt_segment_counts(h, dir_index, counts, numel, stream=None):
     import torch
     _check(load_library().rt_segment_counts(h, int(dir_index), _dev_ptr(counts, torch.int32, numel, "counts"),
@@ -251,6 +265,14 @@ class RayTracer:
         H = torch.empty_like(G)
         rt_sweep_rates(self.h, G, H, self.nx * self.ny * self.nz, self.nbins, wG, lG, wH, lH, stream)
         return G, H
+
+    def point_sources(self, src_fix, lum, diag=None, want_steps=False, stream=None):
+        """rt_point_sources: Q [nbins][nz][ny][nx] (+ tau of (source, bin) = diag, + the step count)."""
+        import torch
+        Q = torch.empty(self.shape(), dtype=torch.float32, device="cuda")
+        tau = torch.empty((self.nz, self.ny, self.nx), dtype=torch.float32, device="cuda") if diag is not None else None
+        n = rt_point_sources(self.h, src_fix, lum, Q, self.numel, self.nbins, tau, diag or (0, 0), want_steps, stream)
+        return Q, tau, n
 
     def segment_counts(self, dir_index=-1, stream=None):
         import torch

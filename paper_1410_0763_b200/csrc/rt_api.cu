@@ -542,6 +542,45 @@ extern "C" int rt_sweep_rates(rt_ctx *c, float *Gamma_dev, float *Heat_dev, cons
     return RT_OK;
 }
 
+extern "C" int rt_point_sources(rt_ctx *c, const int *src_fix_host, const double *lum_host, int nsrc, float *Q_dev,
+                                int diag_src, int diag_bin, float *tau_dev, unsigned long long *steps_host, void *stream)
+{
+    if (!c || !src_fix_host || !lum_host || nsrc < 1 || nsrc > (1 << 20) || !Q_dev) return RT_EINVAL;
+    if (c->nx > 1024 || c->ny > 1024 || c->nz > 1024) return RT_EINVAL;       // 64-bit crossing parameters
+    if (tau_dev && (diag_src < 0 || diag_src >= nsrc || diag_bin < 0 || diag_bin >= c->nbins)) return RT_EINVAL;
+    if (!c->fields_set) return RT_ESTATE;
+    const int dims[3] = {c->nx, c->ny, c->nz};
+    std::vector<float> lum((size_t)nsrc * c->nbins);
+    for (int a = 0; a < nsrc; ++a) {
+        for (int i = 0; i < 3; ++i)
+            if (src_fix_host[3 * a + i] < 0 || src_fix_host[3 * a + i] > dims[i] * 256) return RT_EINVAL;
+        for (int b = 0; b < c->nbins; ++b) {
+            const double v = lum_host[(size_t)a * c->nbins + b];
+            if (!(v >= 0.0) || !std::isfinite(v)) return RT_EINVAL;
+            lum[(size_t)a * c->nbins + b] = (float)v;
+        }
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    int *d_src = nullptr;
+    float *d_lum = nullptr;
+    cudaError_t e = cudaMalloc(&d_src, sizeof(int) * 3 * (size_t)nsrc);
+    if (e == cudaSuccess) e = cudaMalloc(&d_lum, sizeof(float) * lum.size());
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_src, src_fix_host, sizeof(int) * 3 * (size_t)nsrc, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_lum, lum.data(), sizeof(float) * lum.size(), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && steps_host) e = cudaMemsetAsync(c->d_u64, 0, sizeof(unsigned long long), st);
+    if (e == cudaSuccess)
+        e = launch_point_sources(Q_dev, tau_dev, c->d_P[0], c->pp[0], c->nx, c->ny, c->nz, c->pitch[0], d_src, d_lum, nsrc,
+                                 c->nbins, (float)c->cell_width, diag_src, diag_bin, steps_host ? c->d_u64 : nullptr, st);
+    if (e == cudaSuccess && steps_host)
+        e = cudaMemcpyAsync(steps_host, c->d_u64, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
+    // the pageable host buffers above and the temporary device tables must outlive the enqueued work
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d_src); cudaFree(d_lum);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RT_ENOMEM : cuda_fail(e);
+    c->last_launches = 1;
+    return RT_OK;
+}
+
 extern "C" int rt_segment_counts(rt_ctx *c, int dir_index, unsigned int *counts_dev, void *stream)
 {
     if (!c || !counts_dev || dir_index < -1 || dir_index >= c->ndirs) return RT_EINVAL;

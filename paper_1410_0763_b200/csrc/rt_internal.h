@@ -95,6 +95,9 @@ cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN,
                          int nxp, int nyp, int nbins, float inv_nd, const float *w4, cudaStream_t st);
 cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int ppN, size_t n, int nx, int nxp,
                            float inv_nd, int add_S, cudaStream_t st);
+cudaError_t launch_point_sources(float *Q, float *tau_out, const float2 *Pnat, int ppN, int nx, int ny, int nz, int nxp,
+                                 const int *src_dev, const float *lum_dev, int nsrc, int nbins, float cell_width,
+                                 int diag_src, int diag_bin, unsigned long long *steps_dev, cudaStream_t st);
 cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const float *accNC, int slotsN,
                                    const float *accT, const float *accTC, int slotsT,
                                    int nx, int ny, int nz, int nxp, int nyp, cudaStream_t st);

@@ -443,6 +443,112 @@ cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int p
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------
+// Point radiation sources (section 2.1; Appendix 1 eqs. A1-A3): one thread per target
+// cell, one long characteristic per (source, cell) from the source through the cell centre.
+//   tau  = sum kappa ds over the cells before the target cell, dtau = kappa_cell (r_out - r_in)
+//   Q   += L exp(-tau) (1 - exp(-dtau)) / (4 pi/3 (r_out^3 - r_in^3))
+// Source positions are integers in units of 1/256 cell, so every traversal decision is exact: the
+// crossing parameters of the three axes are compared on the common denominator |dx dy dz| in 64-bit
+// integers (u_i = T_i / Dn, one add per step); axes that cross together step together and
+// zero-length pieces are dropped.  Threads of a warp hold 32 neighbouring cells of a row: their rays
+// from one source are nearly parallel, so the kappa gathers of a warp fall into a few cache lines.
+// ------------------------------------------------------------------------------------------------
+constexpr int kPsFix = 256;
+
+__global__ void __launch_bounds__(128)
+k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2 *__restrict__ Pnat, int ppN,
+                int nx, int ny, int nz, int nxp, const int *__restrict__ src, const float *__restrict__ lum, int nsrc,
+                int nbins, float cell_width, int diag_src, int diag_bin, unsigned long long *__restrict__ steps)
+{
+    const int bin = blockIdx.z;
+    const long long ncell = (long long)nx * ny * nz;
+    const long long cidx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = cidx < ncell;
+    const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
+    const size_t boffN = (size_t)bin * nxp * ny * nz;
+    const int dims[3] = {nx, ny, nz};
+    unsigned nstep = 0;
+    if (live) {
+        const int tgt[3] = {(int)(cidx % nx), (int)((cidx / nx) % ny), (int)(cidx / ((long long)nx * ny))};
+        const float kap_t = fN[field_index(boffN + ((size_t)tgt[2] * ny + tgt[1]) * nxp + tgt[0], ppN)];
+        double q = 0.0;
+        for (int a = 0; a < nsrc; ++a) {
+            long long s[3], d[3], ad[3], T[3], inc[3];
+            int cur[3], stp[3];
+            double len2 = 0.0;
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+                s[i] = src[3 * a + i];
+                d[i] = ((long long)tgt[i] * kPsFix + kPsFix / 2) - s[i];
+                stp[i] = d[i] > 0 ? 1 : (d[i] < 0 ? -1 : 0);
+                ad[i] = d[i] < 0 ? -d[i] : d[i];
+                len2 += (double)d[i] * (double)d[i];
+                int c = (int)(s[i] / kPsFix);
+                if (s[i] % kPsFix == 0 && stp[i] < 0) c -= 1;     // a source on a boundary belongs to the cell the ray moves into
+                cur[i] = c;
+            }
+            // common denominator over the moving axes; T_i = n_i * prod_{j != i} |d_j|
+            const long long f0 = ad[0] ? ad[0] : 1, f1 = ad[1] ? ad[1] : 1, f2 = ad[2] ? ad[2] : 1;
+            const long long W[3] = {f1 * f2, f0 * f2, f0 * f1};
+            const double Dn = (double)f0 * (double)f1 * (double)f2;
+            const double len = sqrt(len2) / kPsFix * (double)cell_width;
+            const double scale = len / Dn;                          // length per unit of T
+            const long long kInf = 0x7fffffffffffffffll;
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+                if (stp[i] == 0) { T[i] = kInf; inc[i] = 0; continue; }
+                const long long plane = (long long)(cur[i] + (stp[i] > 0 ? 1 : 0)) * kPsFix;
+                T[i] = (plane - s[i]) * stp[i] * W[i];
+                inc[i] = (long long)kPsFix * W[i];
+            }
+            double tau = 0.0;
+            long long T0 = 0;
+            double r_in = 0.0, r_out = 0.0, dr = 0.0;
+            for (;;) {
+                const long long Tn = min(T[0], min(T[1], T[2]));
+                if (cur[0] == tgt[0] && cur[1] == tgt[1] && cur[2] == tgt[2]) {
+                    if (Tn == kInf) { r_in = 0.0; dr = r_out = 0.5 * (double)cell_width; }   // source at this cell's centre
+                    else { r_in = (double)T0 * scale; dr = (double)(Tn - T0) * scale; r_out = r_in + dr; }
+                    nstep += 1;
+                    break;
+                }
+                if (Tn > T0) {
+                    const float kap = fN[field_index(boffN + ((size_t)cur[2] * ny + cur[1]) * nxp + cur[0], ppN)];
+                    tau += (double)kap * ((double)(Tn - T0) * scale);
+                    nstep += 1;
+                }
+#pragma unroll
+                for (int i = 0; i < 3; ++i)
+                    if (T[i] == Tn) { cur[i] += stp[i]; T[i] += inc[i]; }
+                T0 = Tn;
+            }
+            const double dtau = (double)kap_t * dr;
+            const double vol = 4.0 * 3.14159265358979323846 / 3.0 * dr * (r_out * r_out + r_out * r_in + r_in * r_in);
+            q += (double)lum[(size_t)a * nbins + bin] * exp(-tau) * (-expm1(-dtau)) / vol;
+            if (tau_out && a == diag_src && bin == diag_bin) tau_out[cidx] = (float)tau;
+        }
+        Q[(size_t)bin * ncell + cidx] = (float)q;
+    }
+    if (steps && bin == 0) {
+        unsigned n = nstep;
+        for (int o = 16; o > 0; o >>= 1) n += __shfl_xor_sync(0xffffffffu, n, o);
+        if ((threadIdx.x & 31) == 0 && n) atomicAdd(steps, (unsigned long long)n);
+    }
+    (void)dims;
+}
+
+cudaError_t launch_point_sources(float *Q, float *tau_out, const float2 *Pnat, int ppN, int nx, int ny, int nz, int nxp,
+                                 const int *src_dev, const float *lum_dev, int nsrc, int nbins, float cell_width,
+                                 int diag_src, int diag_bin, unsigned long long *steps_dev, cudaStream_t st)
+{
+    const long long ncell = (long long)nx * ny * nz;
+    dim3 grid((unsigned)((ncell + 127) / 128), 1, nbins);
+    k_point_sources<<<grid, 128, 0, st>>>(Q, tau_out, Pnat, ppN, nx, ny, nz, nxp, src_dev, lum_dev, nsrc, nbins, cell_width,
+                                          diag_src, diag_bin, steps_dev);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const float *accNC, int slotsN,
                                    const float *accT, const float *accTC, int slotsT,
                                    int nx, int ny, int nz, int nxp, int nyp, cudaStream_t st)

@@ -118,3 +118,66 @@ def test_ps4_mirror_symmetry(orc):
         sm[0, ax] = dims[ax] * FIX - src[0, ax]
         qm = orc.point_sources(km, sm, [[1.0]], want_diag=False)["Q"]
         assert np.allclose(np.flip(qm, axis=3 - ax), q, rtol=1e-12)
+
+
+# ---------------------------------------------------------------------------------------------
+# CUDA path against the oracle
+PS_TOL = 1e-5          # relative, with the A14 floor: fp32 output of fp64 path sums over fp32 kappa
+
+
+def _ps_rel(got, ref):
+    ref = np.asarray(ref, dtype=np.float64)
+    floor = max(1e-30 * np.abs(ref).max(), 1e-300)
+    return np.abs(np.asarray(got, dtype=np.float64) - ref) / np.maximum(np.abs(ref), floor)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dims,nb,cw", [((5, 4, 3), 1, 1.0), ((33, 20, 17), 2, 0.7), ((64, 64, 64), 1, 1.0), ((100, 30, 12), 3, 1.0)])
+def test_point_sources_parity(orc, dims, nb, cw):
+    """rt_point_sources against the oracle: step count bit-exact (integer traversal data), tau and Q within
+    1e-5 on every cell; sources on corners, faces, edges, cell centres and generic positions."""
+    import torch
+    import paper_1410_0763_b200 as rt
+    assert torch.cuda.is_available()
+    nx, ny, nz = dims
+    rng = np.random.default_rng(61)
+    kap = rng.uniform(0.02, 0.6, (nb, nz, ny, nx)).astype(np.float32)
+    kap[:, nz // 2:, : ny // 2, :] *= 8.0                      # an opaque block: exp(-tau) spans many decades
+    S = np.zeros_like(kap)
+    src = np.array([[0, 0, 0], [nx * FIX, ny * FIX, nz * FIX], [(nx // 2) * FIX + 128, (ny // 2) * FIX + 128, (nz // 2) * FIX + 128],
+                    [nx * FIX // 3, 0, nz * FIX // 2], [17, ny * FIX - 1, 3], [(nx // 2) * FIX, (ny // 2) * FIX, 77]], dtype=np.int32)
+    lum = rng.uniform(0.5, 2.0, (len(src), nb))
+    tr = rt.RayTracer(dims, nb, rt.healpix_dirs(1), cell_width=cw)
+    try:
+        tr.set_fields(torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda())
+        for diag in [(0, 0), (len(src) - 1, nb - 1), (2, 0)]:
+            Q, tau, steps = tr.point_sources(src, lum, diag=diag, want_steps=True)
+            ref = orc.point_sources(kap, src, lum, cell_width=cw, diag=diag)
+            assert steps == ref["steps"]
+            assert _ps_rel(tau.cpu().numpy(), ref["tau"]).max() <= PS_TOL
+            assert _ps_rel(Q.cpu().numpy(), ref["Q"]).max() <= PS_TOL
+        with pytest.raises(rt.RtError):
+            tr.point_sources([[nx * FIX + 1, 0, 0]], np.ones((1, nb)))
+    finally:
+        tr.close()
+
+
+@pytest.mark.gpu
+def test_point_sources_c3_sampled(orc):
+    """128^3 (config C3's mesh and kappa), 4 sources: full oracle comparison (the oracle takes seconds)."""
+    import torch
+    import paper_1410_0763_b200 as rt
+    from rt_inputs import make_fields
+    kap, S = make_fields("C3")
+    src = np.array([[0, 0, 0], [64 * FIX + 128, 64 * FIX + 128, 64 * FIX + 128], [128 * FIX, 40 * FIX, 77], [10 * FIX + 5, 100 * FIX + 200, 50 * FIX]], dtype=np.int32)
+    lum = np.array([[1.0], [2.0], [0.5], [1.5]])
+    tr = rt.RayTracer((128, 128, 128), 1, rt.healpix_dirs(1))
+    try:
+        tr.set_fields(torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda())
+        Q, tau, steps = tr.point_sources(src, lum, diag=(1, 0), want_steps=True)
+        ref = orc.point_sources(kap, src, lum, diag=(1, 0))
+    finally:
+        tr.close()
+    assert steps == ref["steps"]
+    assert _ps_rel(tau.cpu().numpy(), ref["tau"]).max() <= PS_TOL
+    assert _ps_rel(Q.cpu().numpy(), ref["Q"]).max() <= PS_TOL
