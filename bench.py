@@ -127,6 +127,60 @@ def run_reference(args):
     }))
 
 
+def run_point(args):
+    """--workload point: rt_point_sources on the config's mesh and kappa with seeded sources (one at a box corner,
+    one at the centre, the rest uniform in the box, positions in 1/256 cell).  One JSON line of its own."""
+    import torch
+    import paper_1410_0763_b200 as rt
+    from rt_inputs import make_fields, CONFIGS
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device; there is no CPU fallback"
+    spec = CONFIGS[args.config]
+    kap, S = make_fields(args.config)
+    nx, ny, nz = spec.dims
+    rng = np.random.default_rng(100 + spec.seed)
+    src = np.stack([rng.integers(0, 256 * nx + 1, args.sources), rng.integers(0, 256 * ny + 1, args.sources),
+                    rng.integers(0, 256 * nz + 1, args.sources)], 1).astype(np.int32)
+    src[0] = 0
+    if args.sources > 1:
+        src[1] = [128 * nx, 128 * ny, 128 * nz]
+    lum = rng.uniform(0.5, 2.0, (args.sources, spec.nbins))
+    tr = rt.RayTracer(spec.dims, spec.nbins, rt.healpix_dirs(1))
+    tr.set_fields(torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda())
+    _, _, steps = tr.point_sources(src, lum, want_steps=True)
+    for _ in range(max(args.warmup, 3)):
+        tr.point_sources(src, lum)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        Q, _, _ = tr.point_sources(src, lum)
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1) / args.steps
+    tr.close()
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import oracle
+        ns = min(args.sources, 2)
+        t0 = time.perf_counter()
+        r = oracle.point_sources(kap, src[:ns], lum[:ns], want_diag=False)
+        dt = time.perf_counter() - t0
+        cpu = {"value": r["steps"] * spec.nbins / dt, "unit": "ray steps/s", "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": "%d of %d sources, full mesh, %.1f s" % (ns, args.sources, dt)}
+    print(json.dumps({
+        "metric": "point_source_ray_steps_per_sec", "value": steps * spec.nbins / (ms * 1e-3), "unit": "ray steps/s",
+        "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64 path sums over f32 kappa", "data": "synthetic",
+        "config": {"workload": "point sources on " + workload_name(spec), "sources": args.sources,
+                   "ray_steps_per_step": steps * spec.nbins, "rays_per_step": args.sources * spec.ncell * spec.nbins},
+        "clocks": clocks, "gpu_launches": args.steps,
+        "roofline": None, "note": "gather along long characteristics: latency / integer-ALU bound, no roofline claimed",
+        "cpu_baseline": cpu}))
+
+
 def workload_name(spec):
     return "%s: %dx%dx%d mesh, Nside=%d (%d directions), %d bin(s), seed %d" % (
         spec.name, spec.dims[0], spec.dims[1], spec.dims[2], spec.nside, spec.ndirs, spec.nbins, spec.seed)
@@ -148,12 +202,18 @@ def main():
     ap.add_argument("--pair", type=int, default=None, help="0: switch the mirror-pair schedule off (ablation)")
     ap.add_argument("--tune", action="append", default=[], help="key=value passed to rt_tune (experiments)")
     ap.add_argument("--flags", type=int, default=0, help="0 owned, 1 atomic ablation, 2 paper's four groups")
+    ap.add_argument("--workload", default="diffuse", choices=["diffuse", "point"],
+                    help="diffuse: the ray sweep (BASELINE.json's metric, default); point: rt_point_sources, the paper's "
+                         "second workload (PAPER.md:64-82), SURVEY.md 8(f).4")
+    ap.add_argument("--sources", type=int, default=8, help="--workload point: number of seeded point sources")
     ap.add_argument("--shard", default="replicas", choices=["replicas", "directions"],
                     help="N > 1: independent replicas (default; north_star fixes one GPU) or the paper's direction "
                          "sharding with one all-reduce (PAPER.md:228-230)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload == "point":
+        return run_point(args)
 
     import torch
     import paper_1410_0763_b200 as rt
