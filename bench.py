@@ -29,7 +29,7 @@ UNIT = "updates/s"
 ALGO_BYTES_PER_CELL_DIR_BIN = 16.0     # read kappa,S (8 B) + read-modify-write J accumulator (8 B), SURVEY 8(d)
 # dram__bytes_read.sum + dram__bytes_write.sum per cell-direction-bin of the hot kernel, from the ncu --set full
 # capture named beside it (profiles/); multiplied by the cell-direction-bins of one launch to give `traffic`.
-NCU_DRAM_BYTES_PER_CELL_DIR_BIN = {"C4": (2.535e9 / (26 * 256 ** 3), "profiles/r1c_sweep_tma_full_c4.md")}
+NCU_DRAM_BYTES_PER_CELL_DIR_BIN = {"C4": (5.845, "profiles/r1d_sweep_tma_full_c4.md")}
 
 
 def measured_peaks():
@@ -194,7 +194,7 @@ def main():
     ap.add_argument("--config", default="C4")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-dirs", type=int, default=8, help="directions per step of the reference arm")
-    ap.add_argument("--cpu-dirs", type=int, default=48, help="directions of the cpu_baseline sample")
+    ap.add_argument("--cpu-dirs", type=int, default=96, help="directions of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--slots", type=int, default=None)
     ap.add_argument("--rows", type=int, default=None)
