@@ -199,8 +199,8 @@ int rt_direction_records(rt_ctx *ctx, long long *rec_host, double *L_host);
  *   "stages" : depth of the owned kernel's TMA shared-memory ring (2 or 3)
  *   "pair"   : 1 (default) = a direction and its mirror image along the memory-contiguous transverse axis
  *              are marched by the same warp (shared loads, stores and exponentials); 0 = one direction per warp
- *   "handoff": 1 = a warp's seam partial is handed to the next warp of its CTA through shared memory instead
- *              of the seam accumulator (less DRAM traffic, measured slower; default 0)
+ *   "handoff": 1 = a warp's seam partial is handed to the next warp of its CTA through a ring in shared memory
+ *              instead of the seam accumulator (15 % less DRAM traffic, measured 7 % slower; default 0)
  * Returns RT_EINVAL for unknown keys or unsupported values.  Must be called before rt_set_fields.
  */
 int rt_tune(rt_ctx *ctx, const char *key, int value);

@@ -13,9 +13,8 @@
 // memory row use the next row's data and add to the next row's partial, both held by the same
 // thread.  Only the partial of the row above the warp's last ray row (the "seam") has another
 // owner; it goes to the seam accumulator accC in global memory with plain stores (or, with the
-// "handoff" ablation, into the next warp's staged accumulator row in shared memory, announced
-// through an mbarrier; rows are processed top-down, so it is ready early in a slab and needed at
-// its end).  Every cell therefore has exactly one writer per accumulator array and launch: no
+// handoff, to the next warp of the CTA through a ring in shared memory, announced through an
+// mbarrier; rows are processed top-down, so it is ready early in a slab and needed at its end).  Every cell therefore has exactly one writer per accumulator array and launch: no
 // atomics on the data path, deterministic sums.
 //
 // Variants (template parameter V):
@@ -153,10 +152,11 @@ __device__ __forceinline__ void mbar_arrive(unsigned bar)
 struct Seam {
     bool first;          // first warp of the CTA: nobody hands a seam partial in (the CTA below wrote it to accC)
     bool last;           // last active warp of the CTA: the seam partial goes to accC in global memory
-    unsigned bar_out;    // mbarrier on which this warp announces its seam partial (if !last)
-    unsigned bar_in;     // mbarrier on which the warp below announces its seam partial (if !first)
-    unsigned par_in;     // parity to wait for on bar_in
-    unsigned char *up;   // this lane's position in the next warp's staged old-accumulator row 0 (if !last)
+    // handoff ring (template HO): two slots of one accumulator row per warp boundary, in the producer's block
+    unsigned full_out, empty_out, par_empty;   // producer side (if !last): barriers of the slot in use, parity to wait for
+    unsigned char *ring_out;                   // this lane's position in that slot
+    unsigned full_in, empty_in, par_full;      // consumer side (if !first): the warp below's barriers
+    const unsigned char *ring_in;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -280,14 +280,14 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
                     for (int g = 0; g < G; ++g)
                         *reinterpret_cast<T *>(rowp[R] + RT_MG(g)) = vfma(part_hi[g], invLv, RT_OLD(R, g));
                 } else {
-                    // row 0 of the next warp: add into its staged old-accumulator row and announce it
+                    // row 0 of the next warp: put the partial into the handoff ring and announce it (the slot is
+                    // free once that warp has taken the partial of two stepping slabs ago)
+                    mbar_wait(seam.empty_out, seam.par_empty);
 #pragma unroll
-                    for (int g = 0; g < G; ++g) {
-                        T *o = reinterpret_cast<T *>(seam.up + RT_MG(g) * (int)sizeof(float));
-                        *o = vfma(part_hi[g], invLv, *o);
-                    }
+                    for (int g = 0; g < G; ++g)
+                        *reinterpret_cast<T *>(seam.ring_out + RT_MG(g) * (int)sizeof(float)) = vmul(part_hi[g], invLv);
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(seam.bar_out);
+                    if (lane == 0) mbar_arrive(seam.full_out);
                 }
             }
         } else {
@@ -298,11 +298,20 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
 #pragma unroll
         for (int g = 0; g < G; ++g) part_hi[g] = part_lo[g];
     }
-    // memory row 0: own pieces + the seam partial the warp below added to the staged row
-    if (anySC && !seam.first) mbar_wait(seam.bar_in, seam.par_in);
+    // memory row 0: own pieces (+ with the handoff the seam partial of the warp below)
+    if (anySC && !seam.first) {
+        mbar_wait(seam.full_in, seam.par_full);
 #pragma unroll
-    for (int g = 0; g < G; ++g)
-        *reinterpret_cast<T *>(rowp[0] + RT_MG(g)) = vfma(part_hi[g], invLv, RT_OLD(0, g));
+        for (int g = 0; g < G; ++g)
+            *reinterpret_cast<T *>(rowp[0] + RT_MG(g)) =
+                vadd(vfma(part_hi[g], invLv, RT_OLD(0, g)), *reinterpret_cast<const T *>(seam.ring_in + RT_MG(g) * (int)sizeof(float)));
+        __syncwarp();
+        if (lane == 0) mbar_arrive(seam.empty_in);
+    } else {
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+            *reinterpret_cast<T *>(rowp[0] + RT_MG(g)) = vfma(part_hi[g], invLv, RT_OLD(0, g));
+    }
 #undef RT_OLD
 #undef RT_MG
 }
@@ -360,8 +369,8 @@ struct StageGeom {
     static constexpr int kRowA = kNb * (int)sizeof(float);
     static constexpr int kStage = (R + 1) * (kRowP + kRowA);
     static constexpr int kBarFull = D * kStage;               // D mbarriers: stage filled (transaction bytes)
-    static constexpr int kBarHand = kBarFull + 32;            // D mbarriers: this warp's seam partial of stage s added
-    static constexpr int kLanded = kBarHand + 32;             // int: 1 + last slab whose rows this warp has seen landed
+    static constexpr int kBarHand = kBarFull + 32;            // 2 mbarriers: handoff ring slot h holds this warp's seam partial
+    static constexpr int kBarEmpty = kBarHand + 32;           // 2 mbarriers: the next warp has taken slot h's partial
     static constexpr int kWarpBytes = D * kStage + 128;
     static_assert(D <= 4, "barrier block holds 4 stages");
 };
@@ -369,10 +378,11 @@ struct StageGeom {
 // Each warp owns a private ring of D stages; stage (k mod D) holds slab k's packed field rows and old
 // accumulator rows, copied by bulk async copies (SASS UBLKCP) issued by lane 0 D slabs ahead and
 // tracked by one mbarrier per stage (transaction-byte count).  No registers are spent on data in
-// flight, so the prefetch depth is set by shared memory.  With HO (rt_tune "handoff", a
-// measured ablation, off by default) warps meet on slabs with a step along c, where warp w adds its
-// seam partial into the staged row 0 of warp w + 1 instead of the seam accumulator: 17 % less DRAM
-// traffic, but the warps of a CTA are forced into near lock-step and the sweep gets slower.
+// flight, so the prefetch depth is set by shared memory.  With HO (rt_tune "handoff") warp w hands
+// the seam partial of a slab with a step along c to warp w + 1 through a two-slot ring in shared
+// memory (its own unused seam-accumulator rows) instead of the seam accumulator in global memory:
+// only the CTA's last warp still reads and writes accC.  The producer may run two stepping slabs
+// ahead of its consumer; the consumer never waits unless it has caught up.
 template <int CW, int G, int R, int MODE, int D, int V, int W, bool HO>
 __global__ void __launch_bounds__(32 * W)
 k_sweep_tma(const SweepLaunch L)
@@ -408,8 +418,9 @@ k_sweep_tma(const SweepLaunch L)
     const unsigned bars = wbase_s + SG::kBarFull;
     if (lane == 0) {
 #pragma unroll
-        for (int s = 0; s < D; ++s) { mbar_init(bars + 8 * s, 1); mbar_init(wbase_s + SG::kBarHand + 8 * s, 1); }
-        *reinterpret_cast<volatile int *>(wbase + SG::kLanded) = 0;
+        for (int s = 0; s < D; ++s) mbar_init(bars + 8 * s, 1);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) { mbar_init(wbase_s + SG::kBarHand + 8 * h, 1); mbar_init(wbase_s + SG::kBarEmpty + 8 * h, 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();                                             // every warp's barriers exist before a neighbour touches them
@@ -468,9 +479,7 @@ k_sweep_tma(const SweepLaunch L)
     unsigned char *lane_a = wbase + (R + 1) * SG::kRowP + lcol * (int)sizeof(float);
     float *const acc_l = acc + lcol;
     float *const accC_l = accC + lcol;
-    volatile int *const landed_own = reinterpret_cast<volatile int *>(wbase + SG::kLanded);
-    volatile int *const landed_up = reinterpret_cast<volatile int *>(wbase + SG::kWarpBytes + SG::kLanded);
-    unsigned hand_par = 0;               // bit s: parity of the next completion of the incoming barrier of stage s
+    unsigned hcnt = 0;                   // slabs with a step along c so far: handoff ring slot = hcnt & 1, use = hcnt >> 1
 
     RowState cs;
     cs.init(q0, sub_offset(Dp->sub, 1));
@@ -493,19 +502,20 @@ k_sweep_tma(const SweepLaunch L)
         const unsigned char *sp = lane_p + s * SG::kStage;
         unsigned char *sa = lane_a + s * SG::kStage;
         const bool anySC = (fl & (F_SC1 | F_SC2)) != 0;
-        seam.bar_out = wbase_s + SG::kBarHand + 8 * s;
-        seam.bar_in = wbase_s - SG::kWarpBytes + SG::kBarHand + 8 * s;
-        seam.par_in = (hand_par >> s) & 1u;
-        seam.up = sa + SG::kWarpBytes;
-        if (anySC && !seam.first) hand_par ^= (1u << s);
-        mbar_wait(bars + 8 * s, phase);
-        if (!seam.first && lane == 0) *landed_own = k + 1;
-        if (anySC && !seam.last) {
-            // the next warp's stage s must hold slab k before this warp adds its seam partial to it.  That
-            // warp cannot pass slab k without the partial, so "has seen slab k land" is exactly landed == k + 1.
-            while (*landed_up < k + 1) { }
-            mbar_wait(bars + SG::kWarpBytes + 8 * s, phase);     // acquire the copy's writes
+        if (HO && anySC) {
+            // ring slot of this stepping slab: the (unused) seam accumulator row of stage h in the producer's block
+            const unsigned h = hcnt & 1u, use = (hcnt >> 1) & 1u;
+            seam.full_out = wbase_s + SG::kBarHand + 8 * h;
+            seam.empty_out = wbase_s + SG::kBarEmpty + 8 * h;
+            seam.par_empty = use ^ 1u;                           // first use of a slot: passes at once
+            seam.ring_out = lane_a + h * SG::kStage + R * SG::kRowA;
+            seam.full_in = seam.full_out - SG::kWarpBytes;
+            seam.empty_in = seam.empty_out - SG::kWarpBytes;
+            seam.par_full = use;
+            seam.ring_in = seam.ring_out - SG::kWarpBytes;
+            ++hcnt;
         }
+        mbar_wait(bars + 8 * s, phase);
         RT_DISPATCH_SLAB(fl, fl, I, sp, sa, len0, len1, len2, Ib0, Ib1, Ic, invL, lane, lwrap, padmask, rowp, seam)
         __syncwarp();                     // every lane is done with stage s
         if (k + D < Na) {
