@@ -57,6 +57,7 @@ struct rt_ctx {
     bool pair_enable = true;
     int handoff = 0;
     int slots_pair[2] = {0, 0}, slots_single[2] = {0, 0};
+    int cap_pair[2] = {0, 0}, cap_single[2] = {0, 0};   // owned kernel: work items (CTAs per bin) of one full launch = one wave
     bool fast[2] = {false, false};   // owned kernel usable for the layout
     int pp[2] = {0, 0};              // packed field of the layout is pair-packed (rt_internal.h)
     int rows = 2;
@@ -336,14 +337,18 @@ static int ensure_buffers(rt_ctx *c)
                 for (int i : c->order[l]) Nc = std::min(Nc, c->hd[i].Nc);
                 const int rows = rows_for(c, l);
                 const int ctas_dir = ((Nc / rows + kOwnedWarpsPerCta - 1) / kOwnedWarpsPerCta) * c->nbins;
-                auto wave = [&](bool pair) {
+                // A launch is one wave of resident CTAs, whole wave: `cap` work items (entry, row tile), not
+                // rounded to whole entries; the entries of a launch cycle through cap / tiles + 2 slots.
+                auto wave = [&](bool pair, int *cap) {
                     int per_sm = c->fast[l] ? owned_ctas_per_sm(c->pitch[l], rows, c->stages, pair) : 0;
                     if (per_sm < 1) per_sm = 4;
                     const int resident = per_sm * c->sm_count;
-                    return std::max(1, std::min(nd, resident / std::max(1, ctas_dir)));
+                    *cap = std::max(1, resident / std::max(1, c->nbins));
+                    // (a wave that is a whole number of entries needs no spare slots: launches then end on entry boundaries)
+                    return std::max(1, std::min(nd, resident / std::max(1, ctas_dir) + ((resident % std::max(1, ctas_dir)) ? 2 : 0)));
                 };
-                c->slots_single[l] = wave(false);
-                c->slots_pair[l] = c->fast[l] ? wave(true) : 0;
+                c->slots_single[l] = wave(false, &c->cap_single[l]);
+                c->slots_pair[l] = c->fast[l] ? wave(true, &c->cap_pair[l]) : 0;
                 want = std::max(c->slots_single[l], c->slots_pair[l]);
                 if (!c->fast[l]) want = std::min(nd, 16);
             }
@@ -459,21 +464,46 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
                 auto eff_rev = [&](int d) { return c->hd[d].Mb == 0 ? 0 : c->hd[d].refl[c->hd[d].b]; };
                 const int a = c->hd[list[i]].a;
                 const int rev = eff_rev(list[i]);
+                // owned kernel, full sweep: the batch is the whole class; it is cut into launches of work items below
+                const bool whole = owned_l && only_dir < 0 && owned_supported(L.Nb, c->hd[list[i]].Nc, L.rows);
                 int n = 0;
-                while (i + n < nl && n < S && c->hd[list[i + n]].a == a && eff_rev(list[i + n]) == rev) ++n;
+                while (i + n < nl && (whole || n < S) && c->hd[list[i + n]].a == a && eff_rev(list[i + n]) == rev) ++n;
                 int first = i, count = n;
                 if (only_dir >= 0) {
                     if (c->hd[list[i]].parent != only_dir) { i += 1; continue; }      // all r^2 sub-lattices, one by one
                     count = 1;
                 }
-                used[l] = std::max(used[l], count);
+                used[l] = std::max(used[l], whole ? std::min(count, std::max(1, c->slots[l])) : count);
                 L.batch = c->d_batch + passes[ps].off + first;
                 L.nslots = count;
                 L.rev = rev;
                 L.Nc = c->hd[list[first]].Nc;
                 if (owned_l && owned_supported(L.Nb, L.Nc, L.rows)) {
-                    CK(launch_sweep_owned(L, st));
-                    ++*launches;
+                    const int tiles = (L.Nc + kOwnedWarpsPerCta * L.rows - 1) / (kOwnedWarpsPerCta * L.rows);
+                    L.tiles = tiles;
+                    if (only_dir >= 0) {
+                        L.nslots = 1; L.item0 = 0; L.nitems = tiles;
+                        CK(launch_sweep_owned(L, st));
+                        ++*launches;
+                    } else {
+                        // work items (entry, row tile) of the class, one resident wave per launch; a launch may
+                        // start and end inside an entry, and touches at most nslots entries
+                        const int nsl = std::max(1, c->slots[l]);
+                        int cap = L.pair ? c->cap_pair[l] : c->cap_single[l];
+                        if (c->slots_req > 0 || cap < 1) cap = nsl * tiles;            // whole entries per launch
+                        else if (cap % tiles == 0) cap = std::max(tiles, std::min(cap, nsl * tiles));
+                        else cap = std::max(tiles, std::min(cap, (nsl - 1) * tiles));
+                        if (nsl == 1) cap = tiles;
+                        L.nslots = nsl;
+                        const long long total = (long long)count * tiles;
+                        for (long long item0 = 0; item0 < total; item0 += cap) {
+                            L.item0 = (int)item0;
+                            L.nitems = (int)std::min<long long>(cap, total - item0);
+                            CK(launch_sweep_owned(L, st));
+                            ++*launches;
+                        }
+                        used[l] = std::max(used[l], std::min(nsl, count));
+                    }
                 } else if (c->flags == RT_ATOMIC_ABLATION) {
                     L.variant = 1;
                     CK(launch_sweep_generic(L, c->np_max[l], c->nq_max[l], st));

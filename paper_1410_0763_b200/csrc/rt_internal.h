@@ -53,7 +53,8 @@ struct SweepLaunch {
     const DirDev *dirs;      // device array of all direction records
     const SlabProg *prog;    // device array of all slab programs
     const int *batch;        // device array: direction index per slot of this launch
-    int nslots;              // grid.y
+    int nslots;              // generic kernel: grid.y = entries of the launch; owned kernel: slots the entries cycle through
+    int tiles, item0, nitems;// owned kernel: CTAs per entry; first work item and number of work items of this launch (grid.x)
     int nbins;               // grid.z
     long long ncell;
     const float *Ibc;        // device [nbins][6]: inflow per bin and entry face (-x, +x, -y, +y, -z, +z)

@@ -394,10 +394,15 @@ k_sweep_tma(const SweepLaunch L)
     extern __shared__ __align__(128) unsigned char smem_raw[];
 
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    const int slot = blockIdx.y, bin = blockIdx.z;
-    const DirDev *__restrict__ Dp = L.dirs + L.batch[slot];
+    // A launch is a range of work items (entry, row tile) of a list of entries (directions or mirror pairs)
+    // that need not end on an entry boundary, so that every launch fills all resident CTA slots.  An entry's
+    // accumulators are those of slot = entry mod nslots; nslots exceeds the entries a launch can touch.
+    const int item = (int)blockIdx.x + L.item0;
+    const int ent = item / L.tiles, tile = item - ent * L.tiles;
+    const int slot = ent % L.nslots, bin = blockIdx.z;
+    const DirDev *__restrict__ Dp = L.dirs + L.batch[ent];
     const int Nc = Dp->Nc, Na = Dp->Na, Mc = Dp->Mc;
-    const int q0c = blockIdx.x * (W * R);                        // first ray row of the CTA (grid.x covers Nc)
+    const int q0c = tile * (W * R);                              // first ray row of the CTA (L.tiles of them cover Nc)
     const int nact = min(W, (Nc - q0c) / R);                     // warps of this CTA that own rows (Nc % R == 0)
     const int q0 = q0c + wid * R;
     const int sk = (int)Dp->sk, sl = (int)Dp->sl;                // |offsets| < 2^31: checked by rt_create
@@ -569,7 +574,8 @@ static cudaError_t launch_variant(const SweepLaunch &L, dim3 grid, cudaStream_t 
 template <int CW, int G, int R>
 static cudaError_t launch_rows(const SweepLaunch &L, cudaStream_t st)
 {
-    const dim3 grid((L.Nc + kW * R - 1) / (kW * R), L.nslots, L.nbins);
+    if (L.tiles != (L.Nc + kW * R - 1) / (kW * R) || L.nitems < 1) return cudaErrorInvalidValue;
+    const dim3 grid(L.nitems, 1, L.nbins);
     if (L.mode == MODE_COUNT) return launch_variant<CW, G, R, MODE_COUNT, 2>(L, grid, st);   // diagnostics: depth 2
     if (L.mode == MODE_DS)    return launch_variant<CW, G, R, MODE_DS, 2>(L, grid, st);
     switch (L.stages) {
