@@ -135,7 +135,7 @@ int ctas_per_sm_nb256(int rows, int stages, bool pair);
 bool owned_supported(int Nb, int Nc, int rows)
 {
     if (!(Nb == 32 || Nb == 64 || Nb == 128 || Nb == 256)) return false;
-    if (!(rows == 1 || rows == 2)) return false;
+    if (!(rows == 1 || rows == 2 || (rows == 4 && Nb <= 128))) return false;
     return Nc % rows == 0;
 }
 

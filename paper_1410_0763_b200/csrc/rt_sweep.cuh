@@ -590,6 +590,7 @@ cudaError_t launch_sweep_nb(const SweepLaunch &L, cudaStream_t st)
     switch (L.rows) {
     case 1: return launch_rows<CW, G, 1>(L, st);
     case 2: return launch_rows<CW, G, 2>(L, st);
+    case 4: if constexpr (CW * G <= 4) return launch_rows<CW, G, 4>(L, st); else return cudaErrorInvalidValue;   // rows of <= 128 cells
     }
     return cudaErrorInvalidValue;
 }
@@ -624,6 +625,7 @@ int ctas_per_sm_nb(int rows, int stages, bool pair)
     switch (rows) {
     case 1: return ctas_per_sm_rows<CW, G, 1>(stages, pair);
     case 2: return ctas_per_sm_rows<CW, G, 2>(stages, pair);
+    case 4: if constexpr (CW * G <= 4) return ctas_per_sm_rows<CW, G, 4>(stages, pair); else return 0;
     }
     return 0;
 }

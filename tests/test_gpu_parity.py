@@ -273,7 +273,7 @@ def test_ablation_variants_pass_the_same_gates(orc, flags):
     check_full(orc, kap, S, dirs, out, ref)
 
 
-@pytest.mark.parametrize("rows,stages,pair", [(1, 2, 1), (2, 2, 0), (2, 2, 1), (1, 3, 0), (2, 3, 1), (1, 3, 1)])
+@pytest.mark.parametrize("rows,stages,pair", [(1, 2, 1), (2, 2, 0), (2, 2, 1), (1, 3, 0), (2, 3, 1), (1, 3, 1), (4, 2, 1), (4, 2, 0), (4, 3, 1)])
 def test_rows_per_warp_variants(orc, rows, stages, pair):
     kap, S = _rand((64, 32, 16), 9)
     dirs = orc.healpix_dirs(2)
