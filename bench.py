@@ -29,7 +29,7 @@ UNIT = "updates/s"
 ALGO_BYTES_PER_CELL_DIR_BIN = 16.0     # read kappa,S (8 B) + read-modify-write J accumulator (8 B), SURVEY 8(d)
 # dram__bytes_read.sum + dram__bytes_write.sum per cell-direction-bin of the hot kernel, from the ncu --set full
 # capture named beside it (profiles/); multiplied by the cell-direction-bins of one launch to give `traffic`.
-NCU_DRAM_BYTES_PER_CELL_DIR_BIN = {"C4": (5.845, "profiles/r1d_sweep_tma_full_c4.md")}
+NCU_DRAM_BYTES_PER_CELL_DIR_BIN = {"C4": (5.426, "profiles/r1e_sweep_tma_full_c4.md")}
 
 
 def measured_peaks():
