@@ -28,3 +28,37 @@ def test_gpu_arm_fails_loudly_without_a_device():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1", "--config", "C1"],
                          capture_output=True, text=True, timeout=300)
     assert out.returncode != 0 and "no CPU fallback" in (out.stderr + out.stdout)
+
+
+def _run_bench(*args):
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), *args], capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    return json.loads(out.stdout.strip().splitlines()[-1])
+
+
+import pytest  # noqa: E402
+
+
+@pytest.mark.gpu
+def test_gpu_arm_prints_the_contract_line():
+    """The line the driver parses: metric, whole-job value, e2e with host copies, roofline, cpu_baseline, clocks,
+    launch count (small config so that it runs in seconds)."""
+    d = _run_bench("--config", "C2", "--steps", "3", "--warmup", "3", "--cpu-dirs", "8")
+    assert d["metric"] == "ray_segment_updates_per_sec" and d["unit"] == "updates/s" and d["n_gpus"] == 1
+    assert d["steps"] == 3 and d["warmup"] >= 3 and d["higher_is_better"] is True and d["dtype"] == "f32"
+    assert d["value"] > 0 and d["ms_per_step"] > 0 and d["vs_baseline"] is None and d["data"] == "synthetic"
+    assert d["gpu_launches"] > 0 and "workload" in d["config"]
+    e = d["e2e"]
+    assert 0 < e["value"] <= d["value"] * 1.05 and e["h2d_bytes_per_step"] == 2 * 4 * 64 ** 3 and e["d2h_bytes_per_step"] == 4 * 64 ** 3
+    r = d["roofline"]
+    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and r["peak"] > 1000 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
+    assert 0.5 < r["kernel_share_of_step"] < 1.2
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["sample"]
+    assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+
+
+@pytest.mark.gpu
+def test_point_workload_line():
+    d = _run_bench("--workload", "point", "--config", "C2", "--steps", "2", "--sources", "3")
+    assert d["metric"] == "point_source_ray_steps_per_sec" and d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle"
