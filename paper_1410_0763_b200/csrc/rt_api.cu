@@ -60,7 +60,7 @@ struct rt_ctx {
     int cap_pair[2] = {0, 0}, cap_single[2] = {0, 0};   // owned kernel: work items (CTAs per bin) of one full launch = one wave
     bool fast[2] = {false, false};   // owned kernel usable for the layout
     int pp[2] = {0, 0};              // packed field of the layout is pair-packed (rt_internal.h)
-    int rows = 0;                    // rays rows per warp: 0 = by row width (4 for 128-cell rows, else 2)
+    int rows = 0;                    // rays rows per warp: 0 = by row width (1 up to 64 cells, 4 for 128, 2 for 256)
     int stages = 2;                  // depth of the owned kernel's TMA shared-memory ring (0 = register path)
     int slots_req = 0;               // user override
     int slots[2] = {0, 0};           // allocated slots per layout
@@ -311,7 +311,9 @@ extern "C" int rt_tune(rt_ctx *c, const char *key, int value)
 // rows per warp actually used for a layout (must divide every Nc of the layout's directions)
 static int rows_for(const rt_ctx *c, int layout)
 {
-    int r = c->rows > 0 ? c->rows : (c->pitch[layout] == 128 ? 4 : 2);
+    // by row width: short rows carry little work per warp and slab, so they want more warps (R = 1); 128-cell rows
+    // fit four ray rows in the registers two 256-cell rows take
+    int r = c->rows > 0 ? c->rows : (c->pitch[layout] == 128 ? 4 : (c->pitch[layout] <= 64 ? 1 : 2));
     if (r == 4 && c->pitch[layout] > 128) r = 2;            // four rows per warp only fit the registers for rows of <= 128 cells
     for (int i : c->order[layout])
         while (r > 1 && c->hd[i].Nc % r != 0) r >>= 1;
