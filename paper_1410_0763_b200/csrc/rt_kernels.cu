@@ -473,9 +473,11 @@ k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2
         const int tgt[3] = {(int)(cidx % nx), (int)((cidx / nx) % ny), (int)(cidx / ((long long)nx * ny))};
         const float kap_t = fN[field_index(boffN + ((size_t)tgt[2] * ny + tgt[1]) * nxp + tgt[0], ppN)];
         double q = 0.0;
+        // linear index of a cell in the packed native copy (row pitch nxp) and its change per step along an axis
+        const int idx_t = (tgt[2] * ny + tgt[1]) * nxp + tgt[0];
         for (int a = 0; a < nsrc; ++a) {
             long long s[3], d[3], ad[3], T[3], inc[3];
-            int cur[3], stp[3];
+            int stp[3], cur[3];
             double len2 = 0.0;
 #pragma unroll
             for (int i = 0; i < 3; ++i) {
@@ -488,6 +490,8 @@ k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2
                 if (s[i] % kPsFix == 0 && stp[i] < 0) c -= 1;     // a source on a boundary belongs to the cell the ray moves into
                 cur[i] = c;
             }
+            int idx = (cur[2] * ny + cur[1]) * nxp + cur[0];
+            const int didx[3] = {stp[0], stp[1] * nxp, stp[2] * nxp * ny};
             // common denominator over the moving axes; T_i = n_i * prod_{j != i} |d_j|
             const long long f0 = ad[0] ? ad[0] : 1, f1 = ad[1] ? ad[1] : 1, f2 = ad[2] ? ad[2] : 1;
             const long long W[3] = {f1 * f2, f0 * f2, f0 * f1};
@@ -507,20 +511,20 @@ k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2
             double r_in = 0.0, r_out = 0.0, dr = 0.0;
             for (;;) {
                 const long long Tn = min(T[0], min(T[1], T[2]));
-                if (cur[0] == tgt[0] && cur[1] == tgt[1] && cur[2] == tgt[2]) {
+                if (idx == idx_t) {                                 // (padded linear indices of distinct cells differ)
                     if (Tn == kInf) { r_in = 0.0; dr = r_out = 0.5 * (double)cell_width; }   // source at this cell's centre
                     else { r_in = (double)T0 * scale; dr = (double)(Tn - T0) * scale; r_out = r_in + dr; }
                     nstep += 1;
                     break;
                 }
                 if (Tn > T0) {
-                    const float kap = fN[field_index(boffN + ((size_t)cur[2] * ny + cur[1]) * nxp + cur[0], ppN)];
-                    tau += (double)kap * ((double)(Tn - T0) * scale);
+                    const float kap = fN[field_index(boffN + (size_t)idx, ppN)];
+                    tau = fma((double)kap, (double)(Tn - T0) * scale, tau);
                     nstep += 1;
                 }
 #pragma unroll
                 for (int i = 0; i < 3; ++i)
-                    if (T[i] == Tn) { cur[i] += stp[i]; T[i] += inc[i]; }
+                    if (T[i] == Tn) { idx += didx[i]; T[i] += inc[i]; }
                 T0 = Tn;
             }
             const double dtau = (double)kap_t * dr;
