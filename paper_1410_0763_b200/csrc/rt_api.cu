@@ -423,9 +423,11 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
         if (c->order[l].empty() || (only_dir >= 0 && c->hd[(size_t)only_dir * r2].layout != l)) continue;
         const int S = (only_dir >= 0) ? 1 : c->slots[l];
         const size_t acc_bytes = sizeof(float) * (size_t)c->ncell_l[l] * nbins;
-        CK(cudaMemsetAsync(c->d_acc[l], 0, acc_bytes * S, st));
+        // the seam accumulator is written sparsely, so it is always cleared; the slot accumulators are cleared
+        // below unless the first class of the layout initialises them itself (fresh entries)
         CK(cudaMemsetAsync(c->d_accC[l], 0, acc_bytes * S, st));
     }
+    bool acc_ready[2] = {false, false};
     if (mode == MODE_J) CK(cudaEventRecord(c->ev0, st));
     int off_all = 0;                 // position of the layout's list in d_batch: order[] region ...
     int off_j = c->nv;            // ... and pairs[]/singles[] region
@@ -477,6 +479,14 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
                     count = 1;
                 }
                 used[l] = std::max(used[l], whole ? std::min(count, std::max(1, c->slots[l])) : count);
+                if (!acc_ready[l]) {
+                    // first launches of the layout in this traversal
+                    const int S0 = (only_dir >= 0) ? 1 : c->slots[l];
+                    const bool self_init = whole && mode == MODE_J && !c->handoff && count >= std::max(1, c->slots[l]);
+                    if (!self_init) CK(cudaMemsetAsync(c->d_acc[l], 0, sizeof(float) * (size_t)c->ncell_l[l] * nbins * S0, st));
+                    L.fresh_below = self_init ? std::max(1, c->slots[l]) : 0;
+                    acc_ready[l] = true;
+                } else L.fresh_below = 0;
                 L.batch = c->d_batch + passes[ps].off + first;
                 L.nslots = count;
                 L.rev = rev;

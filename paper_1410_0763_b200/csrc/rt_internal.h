@@ -54,6 +54,7 @@ struct SweepLaunch {
     const SlabProg *prog;    // device array of all slab programs
     const int *batch;        // device array: direction index per slot of this launch
     int nslots;              // generic kernel: grid.y = entries of the launch; owned kernel: slots the entries cycle through
+    int fresh_below;         // owned kernel, MODE_J: entries below this index are the first users of their slots in the sweep
     int tiles, item0, nitems;// owned kernel: CTAs per entry; first work item and number of work items of this launch (grid.x)
     int nbins;               // grid.z
     long long ncell;

@@ -438,6 +438,16 @@ k_sweep_tma(const SweepLaunch L)
     // producer (lane 0): ask the TMA engine for the rows of the slab described by `ps` into stage s.
     // The seam row's old accumulator is needed only by the CTA's last warp (the others add their seam
     // partial into the next warp's stage).
+    // An entry that is the first user of its slot in this sweep starts from zero: its old accumulator rows are not
+    // copied (the slot was not cleared either, rt_api.cu); the staging rows are zeroed once instead.
+    const bool fresh = (MODE == MODE_J) && ent < L.fresh_below;
+    if (fresh) {
+#pragma unroll
+        for (int s = 0; s < D; ++s)
+            for (int i = lane; i < R * SG::kRowA / 16; i += 32)
+                *reinterpret_cast<float4 *>(wbase + s * SG::kStage + (R + 1) * SG::kRowP + 16 * i) = make_float4(0.f, 0.f, 0.f, 0.f);
+        __syncwarp();
+    }
     RowState ps;
     ps.init(q0, sub_offset(Dp->sub, 1));
     auto produce = [&](int s) {
@@ -445,15 +455,16 @@ k_sweep_tma(const SweepLaunch L)
             const unsigned st = wbase_s + s * SG::kStage, bar = bars + 8 * s;
             const bool stp = ps.steps(Mc);
             const int nP = (MODE == MODE_J) ? R + (stp ? 1 : 0) : 0;
-            const int nA = R + ((stp && seam.last) ? 1 : 0);
-            mbar_expect_tx(bar, (unsigned)(nP * SG::kRowP + nA * SG::kRowA));
+            const bool seamA = stp && seam.last;
+            mbar_expect_tx(bar, (unsigned)(nP * SG::kRowP + ((fresh ? 0 : R) + (seamA ? 1 : 0)) * SG::kRowA));
 #pragma unroll
             for (int r = 0; r <= R; ++r) {
                 int l = ps.lb + r; if (l >= Nc) l -= Nc;
                 const int o = ps.offk + l * sl;
                 // packed rows: 2 floats per cell in either packed layout, rows start at even cells
                 if (r < nP) bulk_g2s(st + r * SG::kRowP, P + o, SG::kRowP, bar);
-                if (r < nA) bulk_g2s(st + (R + 1) * SG::kRowP + r * SG::kRowA, (r < R ? acc : accC) + o, SG::kRowA, bar);
+                if (r < R ? !fresh : seamA)
+                    bulk_g2s(st + (R + 1) * SG::kRowP + r * SG::kRowA, (r < R ? acc : accC) + o, SG::kRowA, bar);
             }
         }
         ps.advance(Mc, Nc, sk);
