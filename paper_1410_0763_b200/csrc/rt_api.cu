@@ -42,7 +42,7 @@ struct rt_ctx {
     int rays = 1;                    // r rays per cell width: every direction is r^2 unit sub-lattices ("virtual directions")
     int nv = 0;                      // ndirs * r^2: hd, d_dirs, d_prog and the batch lists are indexed by virtual direction
     long long ncell = 0;
-    int pitch[2] = {0, 0};           // row pitch (cells) of the packed fields / accumulators of a layout: nx, ny padded to 32/64/128/256
+    int pitch[2] = {0, 0};           // row pitch (cells) of the packed fields / accumulators of a layout: nx, ny padded to 32/64/128/256/512
     long long ncell_l[2] = {0, 0};   // cells per bin of a layout including the pad columns
     double cell_width = 1.0;
     unsigned flags = 0;
@@ -161,15 +161,15 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     cudaGetDevice(&c->device);
     cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device);
     const int dims[3] = {nx, ny, nz};
-    // The owned kernel wants the memory-contiguous transverse extent to be 32/64/128/256: narrower or odd
+    // The owned kernel wants the memory-contiguous transverse extent to be 32/64/128/256/512: narrower or odd
     // rows are padded to the next such width (pad cells hold kappa = 0, S = 0: a ray crossing them keeps
     // its intensity and adds nothing, and a chain ray is replaced by the inflow where it wraps, after the pad).
     {
         const int NbL0[2] = {nx, ny};
         for (int l = 0; l < 2; ++l) {
             int p = NbL0[l];
-            if (flags == RT_OWNED && p <= 256) { p = 32; while (p < NbL0[l]) p *= 2; }
-            c->fast[l] = (flags == RT_OWNED) && NbL0[l] <= 256;
+            if (flags == RT_OWNED && p <= 512) { p = 32; while (p < NbL0[l]) p *= 2; }
+            c->fast[l] = (flags == RT_OWNED) && NbL0[l] <= 512;
             c->pitch[l] = p;
             c->pp[l] = (c->fast[l] && p >= 64) ? 1 : 0;          // two columns per chunk
         }
@@ -314,6 +314,7 @@ static int rows_for(const rt_ctx *c, int layout)
     // by row width: short rows carry little work per warp and slab, so they want more warps (R = 1); 128-cell rows
     // fit four ray rows in the registers two 256-cell rows take
     int r = c->rows > 0 ? c->rows : (c->pitch[layout] == 128 ? 4 : (c->pitch[layout] <= 64 ? 1 : 2));
+    if (c->pitch[layout] == 512) r = 1;                       // 512-cell rows: one ray row per warp fills the registers
     if (r == 4 && c->pitch[layout] > 128) r = 2;            // four rows per warp only fit the registers for rows of <= 128 cells
     for (int i : c->order[layout])
         while (r > 1 && c->hd[i].Nc % r != 0) r >>= 1;

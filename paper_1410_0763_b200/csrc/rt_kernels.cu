@@ -127,14 +127,17 @@ cudaError_t launch_sweep_nb32(const SweepLaunch &L, cudaStream_t st);
 cudaError_t launch_sweep_nb64(const SweepLaunch &L, cudaStream_t st);
 cudaError_t launch_sweep_nb128(const SweepLaunch &L, cudaStream_t st);
 cudaError_t launch_sweep_nb256(const SweepLaunch &L, cudaStream_t st);
+cudaError_t launch_sweep_nb512(const SweepLaunch &L, cudaStream_t st);
 int ctas_per_sm_nb32(int rows, int stages, bool pair);
 int ctas_per_sm_nb64(int rows, int stages, bool pair);
 int ctas_per_sm_nb128(int rows, int stages, bool pair);
 int ctas_per_sm_nb256(int rows, int stages, bool pair);
+int ctas_per_sm_nb512(int rows, int stages, bool pair);
 
 bool owned_supported(int Nb, int Nc, int rows)
 {
-    if (!(Nb == 32 || Nb == 64 || Nb == 128 || Nb == 256)) return false;
+    if (!(Nb == 32 || Nb == 64 || Nb == 128 || Nb == 256 || Nb == 512)) return false;
+    if (Nb == 512 && rows != 1) return false;
     if (!(rows == 1 || rows == 2 || (rows == 4 && Nb <= 128))) return false;
     return Nc % rows == 0;
 }
@@ -147,6 +150,7 @@ int owned_ctas_per_sm(int Nb, int rows, int stages, bool pair)
     case 64:  return ctas_per_sm_nb64(rows, stages, pair);
     case 128: return ctas_per_sm_nb128(rows, stages, pair);
     case 256: return ctas_per_sm_nb256(rows, stages, pair);
+    case 512: return ctas_per_sm_nb512(rows, stages, pair);
     }
     return 0;
 }
@@ -158,6 +162,7 @@ cudaError_t launch_sweep_owned(const SweepLaunch &L, cudaStream_t st)
     case 64:  return launch_sweep_nb64(L, st);
     case 128: return launch_sweep_nb128(L, st);
     case 256: return launch_sweep_nb256(L, st);
+    case 512: return launch_sweep_nb512(L, st);
     }
     return cudaErrorInvalidValue;
 }

@@ -595,12 +595,13 @@ static cudaError_t launch_rows(const SweepLaunch &L, cudaStream_t st)
     }
 }
 
-template <int CW, int G>
+// MAXR: largest number of ray rows per warp instantiated for this width (registers: R * G * CW intensities per direction)
+template <int CW, int G, int MAXR = 4>
 cudaError_t launch_sweep_nb(const SweepLaunch &L, cudaStream_t st)
 {
     switch (L.rows) {
     case 1: return launch_rows<CW, G, 1>(L, st);
-    case 2: return launch_rows<CW, G, 2>(L, st);
+    case 2: if constexpr (MAXR >= 2) return launch_rows<CW, G, 2>(L, st); else return cudaErrorInvalidValue;
     case 4: if constexpr (CW * G <= 4) return launch_rows<CW, G, 4>(L, st); else return cudaErrorInvalidValue;   // rows of <= 128 cells
     }
     return cudaErrorInvalidValue;
@@ -630,12 +631,12 @@ static int ctas_per_sm_rows(int stages, bool pair)
 }
 
 // resident CTAs (of kOwnedWarpsPerCta warps) per SM of the J-mode kernel; 0 if the configuration cannot launch
-template <int CW, int G>
+template <int CW, int G, int MAXR = 4>
 int ctas_per_sm_nb(int rows, int stages, bool pair)
 {
     switch (rows) {
     case 1: return ctas_per_sm_rows<CW, G, 1>(stages, pair);
-    case 2: return ctas_per_sm_rows<CW, G, 2>(stages, pair);
+    case 2: if constexpr (MAXR >= 2) return ctas_per_sm_rows<CW, G, 2>(stages, pair); else return 0;
     case 4: if constexpr (CW * G <= 4) return ctas_per_sm_rows<CW, G, 4>(stages, pair); else return 0;
     }
     return 0;

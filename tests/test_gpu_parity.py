@@ -243,11 +243,11 @@ def test_generic_fallback_dims(orc, dims):
     check_full(orc, kap, S, dirs, out, ref)
 
 
-@pytest.mark.parametrize("dims,nb", [((100, 60, 24), 1), ((130, 200, 8), 1), ((33, 7, 5), 2), ((250, 31, 9), 1), ((300, 16, 8), 1)])
+@pytest.mark.parametrize("dims,nb", [((100, 60, 24), 1), ((130, 200, 8), 1), ((33, 7, 5), 2), ((250, 31, 9), 1), ((300, 16, 8), 1), ((512, 24, 8), 1), ((40, 500, 6), 1), ((600, 8, 4), 1)])
 def test_padded_rows_take_the_owned_path(orc, dims, nb):
     """Row widths other than 32/64/128/256 are padded to the next such width (pad cells: kappa = 0, S = 0)
     and swept by the owned kernel (mirror pairs, reversed singles and counting modes all cross the pad);
-    nx > 256 still falls back to the generic kernel for the layout it affects.  Same gates, with inflow."""
+    rows wider than 512 cells still fall back to the generic kernel for the layout they affect.  Same gates, with inflow."""
     kap, S = _rand(dims, 29, nb=nb)
     dirs = np.concatenate([orc.healpix_dirs(2), np.array([[1, 1, 1], [-1, 0.5, 0.25], [0.3, -1, 0]], dtype=np.float64)])
     Ibc = [0.4, 0.1][:nb]
@@ -255,7 +255,7 @@ def test_padded_rows_take_the_owned_path(orc, dims, nb):
     out = gpu_run(kap, S, dirs, Ibc=Ibc, count_dirs=cd)
     ref = orc.sweep(kap, S, dirs, Ibc=Ibc, count_dirs=cd)
     check_records(orc, dirs, out)
-    layout_fast = {0: dims[0] <= 256, 1: dims[1] <= 256}
+    layout_fast = {0: dims[0] <= 512, 1: dims[1] <= 512}
     for i in range(len(dirs)):
         assert out["rec"][i, 4] == (0 if layout_fast[1 if out["rec"][i, 0] == 0 else 0] else 1)
     check_full(orc, kap, S, dirs, out, ref)
