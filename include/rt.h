@@ -196,7 +196,8 @@ int rt_direction_records(rt_ctx *ctx, long long *rec_host, double *L_host);
  * Tuning knobs (experiments and ablations; defaults are chosen by rt_create).
  *   "slots"  : concurrent direction slots per launch (each has private accumulators)
  *   "rows"   : rays rows per warp in the owned kernel (1, 2 or 4; 4 only for rows of <= 128 cells; default by row width:
- *              1 up to 64 cells, 4 for 128, 2 for 256)
+ *              1 up to 64 cells, 4 for 128, 2 for 256, 1 for 512; rows of nx (ny) cells are padded to the next of
+ *              32/64/128/256/512, wider ones run on the generic kernel)
  *   "stages" : depth of the owned kernel's TMA shared-memory ring (2 or 3)
  *   "pair"   : 1 (default) = a direction and its mirror image along the memory-contiguous transverse axis
  *              are marched by the same warp (shared loads, stores and exponentials); 0 = one direction per warp
