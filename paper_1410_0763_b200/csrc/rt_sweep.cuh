@@ -122,7 +122,6 @@ __device__ __forceinline__ void seg_update(T (&I)[ND], T kap, T src, float len, 
     }
 }
 
-constexpr int kWarpsPerCta = kOwnedWarpsPerCta;
 
 // The six slab patterns that occur away from exact boundary touches get straight-line code
 // (FLC = compile-time flags); anything else runs the same body with run-time flags (FLC < 0).
