@@ -133,6 +133,7 @@ typedef struct {
     double *den;                /* [ncell] */
     uint32_t *cnt;              /* [ncell] */
     const int32_t *slot;        /* NULL: accumulate everywhere; else accumulate only where slot[cell] >= 0 */
+    int kstop;                  /* > 0: march slabs 0 .. kstop-1 only (orc_sweep_cells: nothing is sampled further downstream) */
     /* optional per-ray outputs for a single direction */
     double *exitI;              /* [nq][np][nbins] */
     double *chord;              /* [nq][np] */
@@ -189,7 +190,8 @@ static void trace_ray(orc_work_t *w, const orc_dir_t *d, int64_t p, int64_t q)
     double chord = 0.0;
     size_t stride[3] = {1, (size_t)w->dims[0], (size_t)w->dims[0] * w->dims[1]};
 
-    for (int k = 0; k < Na; ++k) {
+    const int kend = (w->kstop > 0 && w->kstop < Na) ? w->kstop : Na;
+    for (int k = 0; k < kend; ++k) {
         int64_t U = U0 + (int64_t)k * d->Mb, V = V0 + (int64_t)k * d->Mc;
         int64_t j = U >> ORC_F, l = V >> ORC_F;                      /* floor */
         if (j < -1 || j >= Nb || l < -1 || l >= Nc) continue;        /* whole slab outside the box */
@@ -467,7 +469,14 @@ int orc_sweep_cells(int nx, int ny, int nz, int nbins,
         w.cnt = (uint32_t *)calloc(ncell, sizeof(uint32_t));
         double *Jloc = (double *)calloc((size_t)ncells * nbins, sizeof(double));
         uint32_t *cloc = (uint32_t *)calloc(ncells, sizeof(uint32_t));
-        if (!w.num || !w.den || !w.cnt || !Jloc || !cloc) {
+        /* the launch lattice of any direction has at most N + N_a + 2 rays along each transverse axis (O3) */
+        const size_t nmax = (size_t)(nx > ny ? (nx > nz ? nx : nz) : (ny > nz ? ny : nz));
+        int32_t *seen = (int32_t *)calloc((2 * nmax + 2) * (2 * nmax + 2), sizeof(int32_t));
+        int32_t *stamp = (int32_t *)calloc((2 * nmax + 2) * (2 * nmax + 2), sizeof(int32_t));
+        int32_t *cand_p = (int32_t *)malloc(sizeof(int32_t) * 4 * (size_t)ncells);
+        int32_t *cand_q = (int32_t *)malloc(sizeof(int32_t) * 4 * (size_t)ncells);
+        int32_t *cand_k = (int32_t *)malloc(sizeof(int32_t) * 4 * (size_t)ncells);
+        if (!w.num || !w.den || !w.cnt || !Jloc || !cloc || !seen || !stamp || !cand_p || !cand_q || !cand_k) {
 #pragma omp atomic write
             fail = 1;
         } else {
@@ -480,7 +489,12 @@ int orc_sweep_cells(int nx, int ny, int nz, int nbins,
                 lattice_range(w.dims, &d, &pmin, &qmin);
                 w.pmin = pmin; w.qmin = qmin; w.np = Nb - pmin; w.nq = Nc - qmin;
                 /* candidate rays: those whose entry cell in the sampled cell's slab is the cell itself or
-                   its (-1,0), (0,-1), (-1,-1) neighbour (a ray's footprint in a slab is a 2x2 block) */
+                   its (-1,0), (0,-1), (-1,-1) neighbour (a ray's footprint in a slab is a 2x2 block).
+                   A ray may be a candidate of several sampled cells; it is traced once per direction, from
+                   its start to the slab of the last sampled cell it can touch (nothing downstream of that
+                   slab is sampled): seen[(q - qmin) * np + (p - pmin)] = position + 1 in the candidate
+                   list of this direction, stamp[] = index + 1 of the direction that wrote it. */
+                int ncand = 0;
                 for (int s = 0; s < ncells; ++s) {
                     int idx[3] = {cells[3 * s], cells[3 * s + 1], cells[3 * s + 2]};
                     int k = d.refl[d.a] ? Na - 1 - idx[d.a] : idx[d.a];
@@ -492,22 +506,20 @@ int orc_sweep_cells(int nx, int ny, int nz, int nbins,
                     for (int dq = 0; dq <= 1; ++dq)
                         for (int dp = 0; dp <= 1; ++dp) {
                             int64_t p = j - dp - sb, q = l - dq - sc;
-                            /* a ray may be a candidate of several sampled cells; trace it once per direction */
-                            int dup = 0;
-                            for (int s2 = 0; s2 < s && !dup; ++s2) {
-                                int idx2[3] = {cells[3 * s2], cells[3 * s2 + 1], cells[3 * s2 + 2]};
-                                int k2 = d.refl[d.a] ? Na - 1 - idx2[d.a] : idx2[d.a];
-                                int j2 = d.refl[d.b] ? Nb - 1 - idx2[d.b] : idx2[d.b];
-                                int l2 = d.refl[d.c] ? Nc - 1 - idx2[d.c] : idx2[d.c];
-                                int64_t sb2 = (ORC_ONE / 2 + (int64_t)k2 * d.Mb) >> ORC_F;
-                                int64_t sc2 = (ORC_ONE / 2 + (int64_t)k2 * d.Mc) >> ORC_F;
-                                for (int e = 0; e < 4; ++e)
-                                    if (j2 - (e & 1) - sb2 == p && l2 - (e >> 1) - sc2 == q) dup = 1;
+                            if (p < pmin || q < qmin) continue;         /* not a lattice ray: it never meets the box (O3) */
+                            const size_t at = (size_t)(q - qmin) * w.np + (size_t)(p - pmin);
+                            if (stamp[at] == i + 1) {
+                                if (cand_k[seen[at]] < k) cand_k[seen[at]] = k;
+                                continue;
                             }
-                            for (int e = 0; e < dq * 2 + dp && !dup; ++e)       /* same cell, earlier candidate */
-                                if (j - (e & 1) - sb == p && l - (e >> 1) - sc == q) dup = 1;
-                            if (!dup) trace_ray(&w, &d, p, q);
+                            stamp[at] = i + 1; seen[at] = ncand;
+                            cand_p[ncand] = (int32_t)p; cand_q[ncand] = (int32_t)q; cand_k[ncand] = k;
+                            ++ncand;
                         }
+                }
+                for (int r = 0; r < ncand; ++r) {
+                    w.kstop = cand_k[r] + 1;
+                    trace_ray(&w, &d, cand_p[r], cand_q[r]);
                 }
                 const double wgt = 1.0 / (double)ndirs;
                 for (int s = 0; s < ncells; ++s) {
@@ -527,7 +539,7 @@ int orc_sweep_cells(int nx, int ny, int nz, int nbins,
                 if (cnt_out) for (int s = 0; s < ncells; ++s) cnt_out[s] += cloc[s];
             }
         }
-        free(w.num); free(w.den); free(w.cnt); free(Jloc); free(cloc);
+        free(w.num); free(w.den); free(w.cnt); free(Jloc); free(cloc); free(seen); free(stamp); free(cand_p); free(cand_q); free(cand_k);
     }
     if (!fail && J_out)
         for (int bin = 0; bin < nbins; ++bin)

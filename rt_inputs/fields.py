@@ -96,15 +96,16 @@ def _bubble_xhi(rng, dims, nbubbles):
     return xhi
 
 
-def make_fields(name: str, dims=None):
+def make_fields(name: str, dims=None, seed=None):
     """Return (kappa, S) as fp32 arrays [nbins][nz][ny][nx] for config `name` ("C1".."C5").
 
-    `dims` overrides the mesh size (same generator, same seed) for reduced-size parity cases.
+    `dims` overrides the mesh size (same generator, same seed) for reduced-size parity cases;
+    `seed` overrides the config's seed (further realisations of the same recipe).
     """
     spec = CONFIGS[name]
     dims = tuple(dims) if dims is not None else spec.dims
     nx, ny, nz = dims
-    rng = np.random.default_rng(spec.seed)
+    rng = np.random.default_rng(spec.seed if seed is None else seed)
     if spec.kind == "uniform":
         kappa = rng.uniform(0.05, 2.0, size=(nz, ny, nx))
         S = rng.uniform(0.0, 1.0, size=(nz, ny, nx))

@@ -14,11 +14,11 @@ from tests import bruteforce as bf
 GOLD = os.path.join(os.path.dirname(__file__), "golden", "worked_example.txt")
 
 
-def rand_fields(dims, seed, kmin=0.05, kmax=2.0):
+def rand_fields(dims, seed, kmin=0.05, kmax=2.0, nb=1):
     nx, ny, nz = dims
     rng = np.random.default_rng(seed)
-    kap = rng.uniform(kmin, kmax, size=(1, nz, ny, nx)).astype(np.float32)
-    S = rng.uniform(0.0, 1.0, size=(1, nz, ny, nx)).astype(np.float32)
+    kap = rng.uniform(kmin, kmax, size=(nb, nz, ny, nx)).astype(np.float32)
+    S = rng.uniform(0.0, 1.0, size=(nb, nz, ny, nx)).astype(np.float32)
     return kap, S
 
 
@@ -348,21 +348,34 @@ def test_multibin_bins_are_independent(orc):
     assert not np.allclose(both["Jin"][0], both["Jin"][1], rtol=1e-3)
 
 
-def test_sampled_cells_match_full_sweep(orc):
+@pytest.mark.parametrize("dims,nb,Ibc,nside,every", [
+    ((12, 10, 9), 1, None, 2, False),
+    ((12, 10, 9), 3, [0.4, 0.0, 1.5], 2, False),          # three bins, non-zero inflow
+    ((9, 14, 6), 2, [0.25, 2.0], 1, True),                # every cell sampled: all candidate rays shared
+    ((16, 5, 11), 3, [1.0, 0.5, 0.0], 2, True),
+])
+def test_sampled_cells_match_full_sweep(orc, dims, nb, Ibc, nside, every):
     """orc_sweep_cells (used for parity at full benchmark sizes) traces only the rays through the
-    sampled cells with the same trace_ray: must reproduce the full sweep there."""
-    dims = (12, 10, 9)
-    kap, S = rand_fields(dims, 71)
-    dirs = orc.healpix_dirs(2)
-    full = orc.sweep(kap, S, dirs)
-    rng = np.random.default_rng(0)
-    cells = np.stack([rng.integers(0, dims[0], 20), rng.integers(0, dims[1], 20), rng.integers(0, dims[2], 20)], 1)
-    cells = np.unique(cells, axis=0)
-    cells = np.concatenate([cells, [[0, 0, 0], [11, 9, 8], [0, 9, 0]]])
-    part = orc.sweep_cells(kap, S, dirs, cells)
-    for s, (x, y, z) in enumerate(cells):
-        assert abs(part["Jin"][0, s] - full["Jin"][0, z, y, x]) <= 1e-13 * full["Jin"][0, z, y, x]
-        assert part["cnt"][s] == full["cnt_sum"][z, y, x]
+    sampled cells with the same trace_ray: must reproduce the full sweep there (J_in, J and counts),
+    for several bins and non-zero inflow, and when neighbouring samples share their candidate rays
+    (axis lines, every cell)."""
+    kap, S = rand_fields(dims, 71, nb=nb)
+    dirs = np.concatenate([orc.healpix_dirs(nside), np.array([[1, 1, 1], [-1, 0.5, 0.25], [0, 0, -1]], dtype=np.float64)])
+    full = orc.sweep(kap, S, dirs, Ibc=Ibc)
+    if every:
+        cells = np.stack(np.meshgrid(np.arange(dims[0]), np.arange(dims[1]), np.arange(dims[2]), indexing="ij"), -1).reshape(-1, 3)
+    else:
+        rng = np.random.default_rng(0)
+        cells = np.stack([rng.integers(0, dims[0], 20), rng.integers(0, dims[1], 20), rng.integers(0, dims[2], 20)], 1)
+        line = np.stack([np.arange(dims[0]), np.full(dims[0], 3), np.full(dims[0], 4)], 1)       # a full axis line
+        cells = np.unique(np.concatenate([cells, line, [[0, 0, 0], [dims[0] - 1, dims[1] - 1, dims[2] - 1], [0, dims[1] - 1, 0]]]), axis=0)
+    part = orc.sweep_cells(kap, S, dirs, cells, Ibc=Ibc)
+    x, y, z = cells[:, 0], cells[:, 1], cells[:, 2]
+    assert np.array_equal(part["cnt"], full["cnt_sum"][z, y, x])
+    for b in range(nb):
+        assert np.abs(part["Jin"][b] - full["Jin"][b, z, y, x]).max() <= 1e-13 * full["Jin"][b].max()
+        assert np.all(np.abs(part["Jin"][b] - full["Jin"][b, z, y, x]) <= 1e-12 * full["Jin"][b, z, y, x] + 1e-300)
+        assert np.all(np.abs(part["J"][b] - full["J"][b, z, y, x]) <= 1e-12 * full["J"][b, z, y, x])
 
 
 def test_cell_width_scales_optical_depth(orc):
