@@ -20,7 +20,8 @@
  * Conventions
  *  - Every call returns RT_OK (0) or a negative RT_E* code; nothing throws, aborts or prints.
  *  - "host" / "device" is stated for every pointer.  Device pointers must belong to the CUDA
- *    device that was current when rt_create was called.
+ *    device that was current when rt_create was called; every call makes that device current for
+ *    its duration and restores the caller's.
  *  - Field arrays are fp32, C-contiguous [nbins][nz][ny][nx] (x fastest).
  *  - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All device
  *    work is enqueued on it; calls are asynchronous unless stated otherwise.
@@ -76,6 +77,8 @@ int rt_healpix_dirs(int nside, double *dirs_out);
  *                   sum ds = r^2 L, which the normalisation accounts for.  Cost and segment counts scale with r^2.
  *   cell_width    : mesh spacing dH (> 0); kappa is per unit length, so dtau = kappa * ds * dH
  *   flags         : RT_OWNED | RT_ATOMIC_ABLATION | RT_PAPER_GROUPS
+ * Limits (RT_EINVAL beyond): each dimension <= 2^20, nx*ny*nz < 2^31, 3 * ndirs * r^2 < 2^24 (per-cell segment
+ * counts stay exact in the fp32 accumulators).
  * Synchronises the device once (table build).  Returns RT_OK / RT_EINVAL / RT_ENOMEM / RT_ECUDA.
  */
 int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins,
@@ -92,6 +95,7 @@ int rt_set_fields(rt_ctx *ctx, const float *kappa_dev, const float *S_dev, void 
 /*
  * Boundary inflow intensity per bin (default 0; the diffuse field has no external source in the
  * paper's tests).   I_bc_host : HOST, fp32 [nbins].
+ * Synchronises the device (sweeps in flight on any stream keep the old values), then copies.
  */
 int rt_set_inflow(rt_ctx *ctx, const float *I_bc_host);
 
@@ -101,7 +105,7 @@ int rt_set_inflow(rt_ctx *ctx, const float *I_bc_host);
  * A ray starts with the value of the face through which it enters the box, i.e. the face it crosses last: a
  * ray marching towards +x that starts inside the transverse extent enters through -x; one that comes in from
  * the side enters through that side face; through an edge (both side planes at once): the c-axis face
- * (reading A10).  rt_set_inflow(v) is the same as all six faces = v.  Synchronous copy.
+ * (reading A10).  rt_set_inflow(v) is the same as all six faces = v.  Synchronises the device, then copies.
  */
 int rt_set_inflow_faces(rt_ctx *ctx, const float *I_face_host);
 
@@ -162,7 +166,9 @@ int rt_sweep_rates(rt_ctx *ctx, float *Gamma_dev, float *Heat_dev, const double 
  *   tau_dev      : DEVICE, fp32 [nz][ny][nx] or NULL: tau of source diag_src in bin diag_bin (diagnostic)
  *   steps_host   : HOST or NULL: number of positive-length ray pieces marched per bin, all sources (integer
  *                  traversal data for the parity gate)
- * Mesh dimensions must be <= 1024 (RT_EINVAL).  Synchronises the stream before returning.
+ * Mesh dimensions must be <= 1024 (RT_EINVAL).  Asynchronous on `cuda_stream`: the source tables are copied into
+ * context-owned device tables through a pinned staging buffer (only when they differ from the previous call's), the
+ * host arrays may be reused as soon as the call returns.  Only a call with steps_host != NULL synchronises the stream.
  */
 int rt_point_sources(rt_ctx *ctx, const int *src_fix_host, const double *lum_host, int nsrc, float *Q_dev,
                      int diag_src, int diag_bin, float *tau_dev, unsigned long long *steps_host, void *cuda_stream);
@@ -178,11 +184,28 @@ int rt_point_sources(rt_ctx *ctx, const int *src_fix_host, const double *lum_hos
  *   sum_ds_host : HOST, fp64 [ndirs].  Synchronises the stream.
  *   min_ds_host, max_ds_host : HOST, fp64 [ndirs] or NULL: min / max over cells of the per-cell sum of ds.
  * rt_total_segments: exact total over directions and cells (numerator of the throughput metric,
- *   per bin).  n_host : HOST.  Synchronises the stream.
+ *   per bin).  n_host : HOST.  The first call runs a counting traversal and synchronises the stream; the
+ *   geometry of a context never changes, so later calls return the cached value.
  */
 int rt_segment_counts(rt_ctx *ctx, int dir_index, unsigned int *counts_dev, void *cuda_stream);
 int rt_sum_ds(rt_ctx *ctx, double *sum_ds_host, double *min_ds_host, double *max_ds_host, void *cuda_stream);
 int rt_total_segments(rt_ctx *ctx, unsigned long long *n_host, void *cuda_stream);
+
+/*
+ * Writer-count check of the ownership scheme that replaces the paper's ray groups (section 3.1:
+ * "light-rays in each group do not traverse any mesh grid more than once").  Runs the launches of rt_sweep (same
+ * work-item ranges, slots, mirror pairs, rows per warp, handoff) with every accumulator store replaced by an atomic
+ * increment of the element it would have written, one launch at a time, and reads the counts back.
+ *   out_host : HOST, unsigned long long [8] =
+ *     [0] largest number of stores any element of a slot accumulator received within one launch (must be 1)
+ *     [1] stores to the slot accumulators, all launches     [2], [3] the same for the seam accumulators ([2] <= 1)
+ *     [4] launches checked                                  [5] launches that start or end inside an entry
+ *     [6] (entries) x (cells of the entry's padded layout) x nbins: every such element is stored exactly once per
+ *         entry, so [1] must equal [6]                      [7] entries (directions or mirror pairs) swept
+ * RT_EINVAL unless the context was created with RT_OWNED and every layout runs on the owned kernel.
+ * Diagnostic: slow (clears and reduces all slot accumulators around every launch); synchronises the stream.
+ */
+int rt_debug_writer_counts(rt_ctx *ctx, unsigned long long *out_host, void *cuda_stream);
 
 /*
  * Per-direction record as quantised by the library (for cross-checks against the oracle).
@@ -198,7 +221,13 @@ int rt_direction_records(rt_ctx *ctx, long long *rec_host, double *L_host);
  *   "rows"   : rays rows per warp in the owned kernel (1, 2 or 4; 4 only for rows of <= 128 cells; default by row width:
  *              1 up to 64 cells, 4 for 128, 2 for 256, 1 for 512; rows of nx (ny) cells are padded to the next of
  *              32/64/128/256/512, wider ones run on the generic kernel)
- *   "stages" : depth of the owned kernel's TMA shared-memory ring (2 or 3)
+ *   "stages" : depth of the owned kernel's TMA shared-memory ring (2 or 3; 4 for rows of <= 64 cells)
+ *   "overlap": 1 = every class of directions (layout, dominant axis, pairs / singles, march sense) gets its own slot
+ *              range and runs on an internal stream of its own, forked from and joined into the caller's stream, so that
+ *              consecutive classes overlap; 0 = one launch after the other; default: 1 when the packed fields fit in
+ *              half the L2 (32^3 ... 128^3), else 0
+ *   "graph"  : 1 = from its second use on, a (J buffer, what) combination of rt_sweep is replayed as one CUDA graph;
+ *              default: only for sweeps of at most two waves of CTAs (launch-latency bound, e.g. 32^3 x 48)
  *   "pair"   : 1 (default) = a direction and its mirror image along the memory-contiguous transverse axis
  *              are marched by the same warp (shared loads, stores and exponentials); 0 = one direction per warp
  *   "handoff": 1 = a warp's seam partial is handed to the next warp of its CTA through a ring in shared memory
@@ -206,6 +235,25 @@ int rt_direction_records(rt_ctx *ctx, long long *rec_host, double *L_host);
  * Returns RT_EINVAL for unknown keys or unsupported values.  Must be called before rt_set_fields.
  */
 int rt_tune(rt_ctx *ctx, const char *key, int value);
+
+/*
+ * Device memory the sweep streams through: packed fields of both layouts + slot and seam accumulators (allocates
+ * them if that has not happened yet).  bytes_host : HOST.  Used to say whether a workload is L2-resident.
+ */
+int rt_working_set_bytes(rt_ctx *ctx, unsigned long long *bytes_host);
+
+/*
+ * Streaming bandwidth probe of the current device: the denominators of the memory-side roofline that
+ * MEASURED_PEAKS.json does not carry ("L2 peak ... the builder must measure it").  One kernel of
+ * 8 CTAs per SM x 512 threads streams a zeroed scratch buffer of `bytes` with 16-byte cache-global accesses (about
+ * 8 GB of them per timed launch, i.e. many passes over a small buffer):
+ *   mode 0 : read only;  mode 1 : read-modify-write of every element (bytes counted twice: read + write)
+ * A buffer well below the L2 capacity (<= 64 MB of 126 MB) measures L2, one of >= 1 GB measures HBM.
+ *   bytes    : 2^20 .. 2^36;  iters : timed repetitions after two warm-up passes (best is reported)
+ *   gbs_host : HOST, GB/s (1e9 bytes per second)
+ * Allocates and frees its scratch buffer; synchronises the stream.  Needs no context.
+ */
+int rt_probe_bandwidth(unsigned long long bytes, int mode, int iters, double *gbs_host, void *cuda_stream);
 
 /* Number of kernel launches issued by the last rt_sweep of this context. */
 int rt_last_launch_count(rt_ctx *ctx);

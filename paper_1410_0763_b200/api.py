@@ -13,7 +13,7 @@ RT_J_IN, RT_J_TOTAL, RT_SUM_IN = 0, 1, 2
 
 EXPORTED_SYMBOLS = [
     "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_set_inflow_faces", "rt_sweep", "rt_combine", "rt_sweep_rates", "rt_point_sources", "rt_segment_counts",
-    "rt_sum_ds", "rt_total_segments", "rt_direction_records", "rt_tune", "rt_last_launch_count",
+    "rt_sum_ds", "rt_total_segments", "rt_debug_writer_counts", "rt_working_set_bytes", "rt_probe_bandwidth", "rt_direction_records", "rt_tune", "rt_last_launch_count",
     "rt_last_sweep_kernel_ms", "rt_destroy", "rt_strerror", "rt_last_cuda_error",
 ]
 
@@ -63,6 +63,12 @@ def load_library():
     L.rt_sum_ds.restype = C.c_int
     L.rt_total_segments.argtypes = [vp, C.POINTER(C.c_ulonglong), vp]
     L.rt_total_segments.restype = C.c_int
+    L.rt_debug_writer_counts.argtypes = [vp, C.POINTER(C.c_ulonglong), vp]
+    L.rt_debug_writer_counts.restype = C.c_int
+    L.rt_working_set_bytes.argtypes = [vp, C.POINTER(C.c_ulonglong)]
+    L.rt_working_set_bytes.restype = C.c_int
+    L.rt_probe_bandwidth.argtypes = [C.c_ulonglong, C.c_int, C.c_int, dp, vp]
+    L.rt_probe_bandwidth.restype = C.c_int
     L.rt_direction_records.argtypes = [vp, C.POINTER(C.c_longlong), dp]
     L.rt_direction_records.restype = C.c_int
     L.rt_tune.argtypes = [vp, C.c_char_p, C.c_int]
@@ -197,6 +203,26 @@ def rt_total_segments(h, stream=None) -> int:
     return int(n.value)
 
 
+def rt_debug_writer_counts(h, stream=None) -> dict:
+    out = (C.c_ulonglong * 8)()
+    _check(load_library().rt_debug_writer_counts(h, out, _stream(stream)), "rt_debug_writer_counts")
+    keys = ("max_writers", "stores", "max_seam_writers", "seam_stores", "launches", "partial_launches", "expected_stores", "entries")
+    return dict(zip(keys, (int(v) for v in out)))
+
+
+def rt_working_set_bytes(h) -> int:
+    n = C.c_ulonglong(0)
+    _check(load_library().rt_working_set_bytes(h, C.byref(n)), "rt_working_set_bytes")
+    return int(n.value)
+
+
+def rt_probe_bandwidth(nbytes: int, mode: int = 0, iters: int = 5, stream=None) -> float:
+    """GB/s of the streaming probe over a scratch buffer of nbytes (mode 0 read, 1 read-modify-write)."""
+    g = C.c_double(0.0)
+    _check(load_library().rt_probe_bandwidth(int(nbytes), int(mode), int(iters), C.byref(g), _stream(stream)), "rt_probe_bandwidth")
+    return float(g.value)
+
+
 def rt_direction_records(h, ndirs):
     rec = np.empty((ndirs, 6), dtype=np.int64)
     L = np.empty(ndirs, dtype=np.float64)
@@ -285,6 +311,12 @@ class RayTracer:
 
     def total_segments(self, stream=None) -> int:
         return rt_total_segments(self.h, stream)
+
+    def debug_writer_counts(self, stream=None) -> dict:
+        return rt_debug_writer_counts(self.h, stream)
+
+    def working_set_bytes(self) -> int:
+        return rt_working_set_bytes(self.h)
 
     def direction_records(self):
         return rt_direction_records(self.h, self.ndirs)

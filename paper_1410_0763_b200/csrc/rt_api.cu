@@ -25,6 +25,20 @@ static int cuda_fail(cudaError_t e)
 }
 #define CK(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(e__); } while (0)
 
+// Every entry point that takes a context makes the context's device current for the duration of the call (a
+// process that drives several GPUs may have switched devices since rt_create) and restores the caller's.
+struct DevGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DevGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = (cudaSetDevice(dev) == cudaSuccess);
+    }
+    ~DevGuard() { if (switched) cudaSetDevice(prev); }
+    DevGuard(const DevGuard &) = delete;
+    DevGuard &operator=(const DevGuard &) = delete;
+};
+
 struct HostDir {
     int a, b, c;          // axes
     int refl[3];
@@ -61,7 +75,7 @@ struct rt_ctx {
     bool fast[2] = {false, false};   // owned kernel usable for the layout
     int pp[2] = {0, 0};              // packed field of the layout is pair-packed (rt_internal.h)
     int rows = 0;                    // rays rows per warp: 0 = by row width (1 up to 64 cells, 4 for 128, 2 for 256)
-    int stages = 2;                  // depth of the owned kernel's TMA shared-memory ring (0 = register path)
+    int stages = 0;                  // depth of the owned kernel's TMA shared-memory ring: 0 = by row width (stages_for)
     int slots_req = 0;               // user override
     int slots[2] = {0, 0};           // allocated slots per layout
     bool fields_set = false;
@@ -82,6 +96,28 @@ struct rt_ctx {
     int last_launches = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool ev_valid = false;
+    // overlapped schedule (small meshes): every class of directions (layout, dominant axis, pairs / singles, march
+    // sense along b) has its own slot range and runs on its own internal stream ("lane"), so that the classes of a
+    // sweep that does not fill the machine run side by side instead of one short launch after the other
+    struct ClassPlan { int l, pair, off, count, rev, Nc, tiles, slot_base, nslots; };
+    std::vector<ClassPlan> plan;
+    int overlap = -1;                // rt_tune "overlap": -1 = automatic, 0 = off, 1 = on
+    bool overlap_on = false;
+    bool tiny = false;               // the whole sweep is at most two waves of resident CTAs: launch-latency bound, replayed as a CUDA graph
+    int graph = -1;                  // rt_tune "graph": -1 = automatic (with the overlapped schedule), 0 = off, 1 = on
+    static constexpr int kLanes = 8;
+    cudaStream_t lane[kLanes] = {};
+    cudaEvent_t ev_fork = nullptr, ev_join[kLanes] = {};
+    cudaStream_t cap_stream = nullptr;   // origin stream of the graph captures (the caller's stream may be the legacy one)
+    struct SweepGraph { float *J; unsigned what; int seen; cudaGraph_t graph; cudaGraphExec_t exec; };
+    std::vector<SweepGraph> graphs;
+    unsigned char *d_src = nullptr, *src_stage = nullptr;     // rt_point_sources: device tables {int src[n][3], float lum[n][nbins]} and pinned staging
+    size_t src_cap = 0;
+    int src_n = 0;
+    bool src_valid = false, src_copy_pending = false;
+    cudaEvent_t ev_src = nullptr;
+    long long seg_total = -1;        // rt_total_segments: the geometry never changes, so the count is taken once
+    unsigned long long *d_own = nullptr;   // [4] rt_debug_writer_counts: {max, sum} of acc, {max, sum} of accC
 };
 
 extern "C" const char *rt_strerror(int code)
@@ -130,9 +166,20 @@ static void free_device(rt_ctx *c)
 {
     cudaFree(c->d_dirs); cudaFree(c->d_L); cudaFree(c->d_prog);
     for (int l = 0; l < 2; ++l) { cudaFree(c->d_P[l]); cudaFree(c->d_acc[l]); cudaFree(c->d_accC[l]); }
-    cudaFree(c->d_batch); cudaFree(c->d_Ibc); cudaFree(c->d_red); cudaFree(c->d_u64); cudaFree(c->d_cnt);
+    cudaFree(c->d_batch); cudaFree(c->d_Ibc); cudaFree(c->d_red); cudaFree(c->d_u64); cudaFree(c->d_cnt); cudaFree(c->d_own);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    for (auto &g : c->graphs) { if (g.exec) cudaGraphExecDestroy(g.exec); if (g.graph) cudaGraphDestroy(g.graph); }
+    c->graphs.clear();
+    for (int i = 0; i < rt_ctx::kLanes; ++i) {
+        if (c->lane[i]) cudaStreamDestroy(c->lane[i]);
+        if (c->ev_join[i]) cudaEventDestroy(c->ev_join[i]);
+    }
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    cudaFree(c->d_src);
+    if (c->src_stage) cudaFreeHost(c->src_stage);
+    if (c->ev_src) cudaEventDestroy(c->ev_src);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
 }
 
 extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const double *dirs, int ndirs,
@@ -142,7 +189,9 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
     *out = nullptr;
     if (nx < 1 || ny < 1 || nz < 1 || nbins < 1 || nbins > 16 || !dirs || ndirs < 1) return RT_EINVAL;
     if (rays_per_cell < 1 || rays_per_cell > 16 || (rays_per_cell & (rays_per_cell - 1)) != 0) return RT_EINVAL;
-    if ((long long)ndirs * rays_per_cell * rays_per_cell > (1ll << 24)) return RT_EINVAL;
+    // per-cell segment counts (up to 3 per direction and sub-lattice) are tallied in fp32 accumulators: keep them exact
+    if (3ll * ndirs * rays_per_cell * rays_per_cell >= (1ll << 24)) return RT_EINVAL;
+    if (nx > (1 << 20) || ny > (1 << 20) || nz > (1 << 20)) return RT_EINVAL;
     if (!(cell_width > 0.0) || !std::isfinite(cell_width)) return RT_EINVAL;
     if (flags > 2u) return RT_EINVAL;
     if ((long long)nx * ny * nz >= (1ll << 31) || (long long)nx * ny * nz * nbins >= (1ll << 40)) return RT_EINVAL;
@@ -287,7 +336,7 @@ extern "C" int rt_create(rt_ctx **out, int nx, int ny, int nz, int nbins, const 
         }
         CKC(cudaMemcpy(c->d_batch, batch.data(), sizeof(int) * batch.size(), cudaMemcpyHostToDevice));
     }
-    CKC(launch_build_programs(c->d_dirs, nv, c->d_prog, cell_width, c->d_L, 0));
+    CKC(launch_build_programs(c->d_dirs, nv, std::max(nx, std::max(ny, nz)), c->d_prog, cell_width, c->d_L, 0));
     CKC(cudaEventCreate(&c->ev0));
     CKC(cudaEventCreate(&c->ev1));
     CKC(cudaDeviceSynchronize());
@@ -301,9 +350,11 @@ extern "C" int rt_tune(rt_ctx *c, const char *key, int value)
     if (!c || !key) return RT_EINVAL;
     if (c->buffers_ready) return RT_ESTATE;
     if (!strcmp(key, "slots")) { if (value < 1 || value > 4096) return RT_EINVAL; c->slots_req = value; return RT_OK; }
-    if (!strcmp(key, "stages")) { if (!(value >= 2 && value <= 3) || (c->handoff && value != 2)) return RT_EINVAL; c->stages = value; return RT_OK; }
-    if (!strcmp(key, "handoff")) { if ((value != 0 && value != 1) || (value && c->stages != 2)) return RT_EINVAL; c->handoff = value; return RT_OK; }
+    if (!strcmp(key, "stages")) { if (!(value >= 2 && value <= 4) || (c->handoff && value != 2)) return RT_EINVAL; c->stages = value; return RT_OK; }
+    if (!strcmp(key, "handoff")) { if ((value != 0 && value != 1) || (value && c->stages != 2 && c->stages != 0)) return RT_EINVAL; c->handoff = value; if (value) c->stages = 2; return RT_OK; }
     if (!strcmp(key, "pair")) { if (value != 0 && value != 1) return RT_EINVAL; c->pair_enable = value != 0; return RT_OK; }
+    if (!strcmp(key, "overlap")) { if (value < -1 || value > 1) return RT_EINVAL; c->overlap = value; return RT_OK; }
+    if (!strcmp(key, "graph")) { if (value < -1 || value > 1) return RT_EINVAL; c->graph = value; return RT_OK; }
     if (!strcmp(key, "rows")) { if (!(value == 1 || value == 2 || value == 4)) return RT_EINVAL; c->rows = value; return RT_OK; }
     return RT_EINVAL;
 }
@@ -319,6 +370,66 @@ static int rows_for(const rt_ctx *c, int layout)
     for (int i : c->order[layout])
         while (r > 1 && c->hd[i].Nc % r != 0) r >>= 1;
     return r;
+}
+
+// depth of the TMA ring used for a layout: rt_tune "stages", else by row width (a slab of a short row is little work
+// per warp, so the copies of more slabs have to be in flight to cover their latency)
+static int stages_for(const rt_ctx *c, int layout)
+{
+    if (c->stages > 0) return c->stages;
+    return c->pitch[layout] <= 64 ? kShortRowStages : 2;
+}
+
+// Classes of a full J sweep in launch order, each with a slot range of its own (overlapped schedule).  The
+// enumeration is the one run_traversal walks: per layout the mirror pairs, then the singles, cut where the dominant
+// axis or the march sense along b changes.  false if some class cannot run on the owned kernel.
+static bool build_overlap_plan(const rt_ctx *c, std::vector<rt_ctx::ClassPlan> &plan, int need[2], long long *items)
+{
+    plan.clear();
+    need[0] = need[1] = 0;
+    *items = 0;
+    int off_all = 0, off_j = c->nv;
+    for (int l = 0; l < 2; ++l) {
+        const int nd = (int)c->order[l].size();
+        const int my_all = off_all, my_j = off_j;
+        off_all += nd;
+        off_j += (int)(c->pairs[l].size() + c->singles[l].size());
+        if (nd == 0) continue;
+        if (!c->fast[l]) return false;
+        const int rows = rows_for(c, l);
+        const bool use_pairs = c->pair_enable && !c->pairs[l].empty();
+        struct Pass { const std::vector<int> *list; int off; int S; int pair; };
+        Pass passes[2];
+        int npass = 0;
+        if (use_pairs) {
+            passes[npass++] = Pass{&c->pairs[l], my_j, c->slots_pair[l], 1};
+            passes[npass++] = Pass{&c->singles[l], my_j + (int)c->pairs[l].size(), c->slots_single[l], 0};
+        } else {
+            passes[npass++] = Pass{&c->order[l], my_all, c->slots_single[l], 0};
+        }
+        for (int ps = 0; ps < npass; ++ps) {
+            const std::vector<int> &list = *passes[ps].list;
+            const int nl = (int)list.size();
+            auto eff_rev = [&](int d) { return c->hd[d].Mb == 0 ? 0 : c->hd[d].refl[c->hd[d].b]; };
+            int i = 0;
+            while (i < nl) {
+                const int a = c->hd[list[i]].a, rev = eff_rev(list[i]), Nc = c->hd[list[i]].Nc;
+                if (!owned_supported(c->pitch[l], Nc, rows)) return false;
+                int n = 0;
+                while (i + n < nl && c->hd[list[i + n]].a == a && eff_rev(list[i + n]) == rev) ++n;
+                rt_ctx::ClassPlan p;
+                p.l = l; p.pair = passes[ps].pair; p.off = passes[ps].off + i; p.count = n; p.rev = rev; p.Nc = Nc;
+                p.tiles = (Nc + kOwnedWarpsPerCta * rows - 1) / (kOwnedWarpsPerCta * rows);
+                p.slot_base = need[l];
+                p.nslots = std::max(1, std::min(n, passes[ps].S));
+                need[l] += p.nslots;
+                *items += (long long)n * p.tiles * c->nbins;
+                plan.push_back(p);
+                i += n;
+            }
+        }
+    }
+    return !plan.empty();
 }
 
 static int ensure_buffers(rt_ctx *c)
@@ -344,7 +455,7 @@ static int ensure_buffers(rt_ctx *c)
                 // A launch is one wave of resident CTAs, whole wave: `cap` work items (entry, row tile), not
                 // rounded to whole entries; the entries of a launch cycle through cap / tiles + 2 slots.
                 auto wave = [&](bool pair, int *cap) {
-                    int per_sm = c->fast[l] ? owned_ctas_per_sm(c->pitch[l], rows, c->stages, pair) : 0;
+                    int per_sm = c->fast[l] ? owned_ctas_per_sm(c->pitch[l], rows, stages_for(c, l), pair) : 0;
                     if (per_sm < 1) per_sm = 4;
                     const int resident = per_sm * c->sm_count;
                     *cap = std::max(1, resident / std::max(1, c->nbins));
@@ -366,17 +477,62 @@ static int ensure_buffers(rt_ctx *c)
         c->slots_single[l] = (c->slots_req > 0 || !c->fast[l]) ? want : std::min(want, c->slots_single[l]);
         c->slots_pair[l] = (c->slots_req > 0) ? want : std::min(want, c->slots_pair[l]);
     }
+    // overlapped schedule: on by rt_tune, or by itself for meshes whose packed fields are L2-resident
+    c->overlap_on = false;
+    if (c->flags == RT_OWNED && c->overlap != 0 && c->slots_req == 0 && !c->handoff) {
+        std::vector<rt_ctx::ClassPlan> plan;
+        int need[2];
+        long long items = 0;
+        if (build_overlap_plan(c, plan, need, &items)) {
+            long long capacity = 0;
+            for (int l = 0; l < 2; ++l) capacity = std::max<long long>(capacity, (long long)std::max(c->cap_pair[l], c->cap_single[l]) * c->nbins);
+            const size_t budget = freeb / 3, need_fixed = field_bytes_l[0] + field_bytes_l[1];
+            const size_t need_acc = 2 * (need[0] * acc_bytes_l[0] + need[1] * acc_bytes_l[1]);
+            const bool fits = budget > need_fixed && need_acc <= budget - need_fixed;
+            // by itself when the packed fields of both layouts stay in L2 next to the accumulator rows in flight (the
+            // classes then need not march the same slabs to share them): measured C1 0.19 -> 0.07 ms, C2 0.74 -> 0.57 ms,
+            // C3 7.31 -> 7.14 ms
+            int l2_bytes = 0;
+            cudaDeviceGetAttribute(&l2_bytes, cudaDevAttrL2CacheSize, c->device);
+            const bool resident = need_fixed <= (size_t)l2_bytes / 2;
+            c->tiny = items <= 2 * capacity;
+            if ((c->overlap == 1 || (c->overlap == -1 && resident)) && fits) {
+                c->plan.swap(plan);
+                c->overlap_on = true;
+                for (int l = 0; l < 2; ++l) c->slots[l] = std::max(c->slots[l], need[l]);
+            }
+        }
+    }
+    // on failure nothing stays allocated, so that a later call starts from scratch instead of leaking
+    auto fail = [&](cudaError_t e) {
+        for (int l = 0; l < 2; ++l) {
+            cudaFree(c->d_P[l]); cudaFree(c->d_acc[l]); cudaFree(c->d_accC[l]);
+            c->d_P[l] = nullptr; c->d_acc[l] = c->d_accC[l] = nullptr;
+        }
+        if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return (int)RT_ENOMEM; }
+        return cuda_fail(e);
+    };
     for (int l = 0; l < 2; ++l) {
         {   // both packed copies are always kept (the pack kernel writes both in one pass)
             cudaError_t e = cudaMalloc(&c->d_P[l], field_bytes_l[l]);
             if (e == cudaSuccess) e = cudaMemset(c->d_P[l], 0, field_bytes_l[l]);      // pad cells stay zero
-            if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RT_ENOMEM : cuda_fail(e);
+            if (e != cudaSuccess) return fail(e);
         }
         if (c->slots[l] > 0) {
             cudaError_t e = cudaMalloc(&c->d_acc[l], acc_bytes_l[l] * c->slots[l]);
             if (e == cudaSuccess) e = cudaMalloc(&c->d_accC[l], acc_bytes_l[l] * c->slots[l]);
-            if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RT_ENOMEM : cuda_fail(e);
+            if (e != cudaSuccess) return fail(e);
         }
+    }
+    if (c->overlap_on) {
+        cudaError_t e = cudaSuccess;
+        for (int i = 0; i < rt_ctx::kLanes && e == cudaSuccess; ++i) {
+            if (!c->lane[i]) e = cudaStreamCreateWithFlags(&c->lane[i], cudaStreamNonBlocking);
+            if (e == cudaSuccess && !c->ev_join[i]) e = cudaEventCreateWithFlags(&c->ev_join[i], cudaEventDisableTiming);
+        }
+        if (e == cudaSuccess && !c->ev_fork) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
+        if (e == cudaSuccess && !c->cap_stream) e = cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) return fail(e);
     }
     c->buffers_ready = true;
     return RT_OK;
@@ -385,6 +541,7 @@ static int ensure_buffers(rt_ctx *c)
 extern "C" int rt_set_fields(rt_ctx *c, const float *kappa_dev, const float *S_dev, void *stream)
 {
     if (!c || !kappa_dev || !S_dev) return RT_EINVAL;
+    DevGuard dev_guard(c->device);
     int rc = ensure_buffers(c);
     if (rc != RT_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
@@ -396,11 +553,13 @@ extern "C" int rt_set_fields(rt_ctx *c, const float *kappa_dev, const float *S_d
 extern "C" int rt_set_inflow(rt_ctx *c, const float *I_bc_host)
 {
     if (!c || !I_bc_host) return RT_EINVAL;
+    DevGuard dev_guard(c->device);
     std::vector<float> six(6 * (size_t)c->nbins);
     for (int b = 0; b < c->nbins; ++b) {
         if (!(I_bc_host[b] >= 0.0f) || !std::isfinite(I_bc_host[b])) return RT_EINVAL;
         for (int f = 0; f < 6; ++f) six[6 * (size_t)b + f] = I_bc_host[b];
     }
+    CK(cudaDeviceSynchronize());        // sweeps in flight on any stream still read the old values
     CK(cudaMemcpy(c->d_Ibc, six.data(), sizeof(float) * six.size(), cudaMemcpyHostToDevice));
     return RT_OK;
 }
@@ -408,7 +567,9 @@ extern "C" int rt_set_inflow(rt_ctx *c, const float *I_bc_host)
 extern "C" int rt_set_inflow_faces(rt_ctx *c, const float *I_face_host)
 {
     if (!c || !I_face_host) return RT_EINVAL;
+    DevGuard dev_guard(c->device);
     for (int i = 0; i < 6 * c->nbins; ++i) if (!(I_face_host[i] >= 0.0f) || !std::isfinite(I_face_host[i])) return RT_EINVAL;
+    CK(cudaDeviceSynchronize());        // sweeps in flight on any stream still read the old values
     CK(cudaMemcpy(c->d_Ibc, I_face_host, sizeof(float) * 6 * c->nbins, cudaMemcpyHostToDevice));
     return RT_OK;
 }
@@ -416,7 +577,10 @@ extern "C" int rt_set_inflow_faces(rt_ctx *c, const float *I_face_host)
 // Enqueue the traversal in `mode` of all directions (only_dir < 0) or of one direction (slot 0 of
 // its layout).  The slot accumulators that will be used are zeroed first; used[l] receives the
 // number of slots of layout l that hold results afterwards.
-static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStream_t st, int *launches, int used[2])
+struct OwnerStats { unsigned long long launches = 0, partial = 0, expected = 0, entries = 0; };
+
+static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStream_t st, int *launches, int used[2],
+                         OwnerStats *own = nullptr, bool record_events = true)
 {
     const int r2 = c->rays * c->rays;
     used[0] = used[1] = 0;
@@ -429,7 +593,7 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
         CK(cudaMemsetAsync(c->d_accC[l], 0, acc_bytes * S, st));
     }
     bool acc_ready[2] = {false, false};
-    if (mode == MODE_J) CK(cudaEventRecord(c->ev0, st));
+    if (mode == MODE_J && record_events) CK(cudaEventRecord(c->ev0, st));
     int off_all = 0;                 // position of the layout's list in d_batch: order[] region ...
     int off_j = c->nv;            // ... and pairs[]/singles[] region
     for (int l = 0; l < 2; ++l) {
@@ -443,14 +607,14 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
         memset(&L, 0, sizeof(L));
         L.P = c->d_P[l]; L.acc = c->d_acc[l]; L.accC = c->d_accC[l];
         L.dirs = c->d_dirs; L.prog = c->d_prog; L.nbins = nbins; L.ncell = c->ncell_l[l]; L.Ibc = c->d_Ibc;
-        L.rows = rows_for(c, l); L.mode = mode; L.stages = c->stages; L.handoff = c->handoff;
+        L.rows = rows_for(c, l); L.mode = mode; L.stages = stages_for(c, l); L.handoff = c->handoff;
         L.Nb = c->pitch[l]; L.pp = c->pp[l];
         const bool owned_l = c->fast[l];
         // the lists this traversal walks: (direction list, position in d_batch, slots per launch, paired)
         struct Pass { const std::vector<int> *list; int off; int S; int pair; };
         Pass passes[2];
         int npass = 0;
-        const bool use_pairs = (mode == MODE_J) && only_dir < 0 && c->pair_enable && owned_l &&
+        const bool use_pairs = (mode == MODE_J || mode == MODE_OWNERS) && only_dir < 0 && c->pair_enable && owned_l &&
                                !c->pairs[l].empty();
         if (use_pairs) {
             passes[npass++] = Pass{&c->pairs[l], my_j, c->slots_pair[l], 1};
@@ -513,11 +677,28 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
                         for (long long item0 = 0; item0 < total; item0 += cap) {
                             L.item0 = (int)item0;
                             L.nitems = (int)std::min<long long>(cap, total - item0);
+                            const size_t nacc = (size_t)c->ncell_l[l] * nbins * nsl;
+                            if (mode == MODE_OWNERS) {       // writer counts of this launch alone
+                                CK(cudaMemsetAsync(c->d_acc[l], 0, sizeof(float) * nacc, st));
+                                CK(cudaMemsetAsync(c->d_accC[l], 0, sizeof(float) * nacc, st));
+                            }
                             CK(launch_sweep_owned(L, st));
                             ++*launches;
+                            if (mode == MODE_OWNERS) {
+                                CK(launch_owner_reduce(c->d_own, c->d_acc[l], (long long)nacc, st));
+                                CK(launch_owner_reduce(c->d_own + 2, c->d_accC[l], (long long)nacc, st));
+                                own->launches += 1;
+                                if (L.item0 % tiles != 0 || (L.item0 + L.nitems) % tiles != 0) own->partial += 1;
+                            }
+                        }
+                        if (mode == MODE_OWNERS) {
+                            own->entries += (unsigned long long)count;
+                            own->expected += (unsigned long long)count * (unsigned long long)c->ncell_l[l] * (unsigned long long)nbins;
                         }
                         used[l] = std::max(used[l], std::min(nsl, count));
                     }
+                } else if (mode == MODE_OWNERS) {
+                    return RT_EINVAL;                 // the writer-count check is for the owned kernel's ownership scheme
                 } else if (c->flags == RT_ATOMIC_ABLATION) {
                     L.variant = 1;
                     CK(launch_sweep_generic(L, c->np_max[l], c->nq_max[l], st));
@@ -534,18 +715,70 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
             }
         }
     }
-    if (mode == MODE_J) { CK(cudaEventRecord(c->ev1, st)); c->ev_valid = true; }
+    if (mode == MODE_J && record_events) { CK(cudaEventRecord(c->ev1, st)); c->ev_valid = true; }
     return RT_OK;
 }
 
-extern "C" int rt_sweep(rt_ctx *c, float *J_dev, unsigned what, void *stream)
+// Overlapped J sweep (ensure_buffers decided c->overlap_on): the classes run on the context's lanes, forked from
+// and joined back into `st` with events.  Every class owns its slot range and its first nslots entries start from
+// zero ("fresh"), so no slot accumulator is cleared; the sparsely written seam accumulators are.
+static int run_overlapped(rt_ctx *c, cudaStream_t st, int *launches, int used[2], bool record_events)
 {
-    if (!c || !J_dev || what > 2u) return RT_EINVAL;
-    if (!c->fields_set) return RT_ESTATE;
-    cudaStream_t st = (cudaStream_t)stream;
+    const int nbins = c->nbins;
+    for (int l = 0; l < 2; ++l) {
+        used[l] = 0;
+        for (const auto &p : c->plan) if (p.l == l) used[l] = std::max(used[l], p.slot_base + p.nslots);
+        if (used[l] > 0) CK(cudaMemsetAsync(c->d_accC[l], 0, sizeof(float) * (size_t)c->ncell_l[l] * nbins * used[l], st));
+    }
+    if (record_events) CK(cudaEventRecord(c->ev0, st));
+    CK(cudaEventRecord(c->ev_fork, st));
+    bool lane_used[rt_ctx::kLanes] = {};
+    int idx = 0;
+    for (const auto &p : c->plan) {
+        const int ln = idx++ % rt_ctx::kLanes;
+        cudaStream_t ls = c->lane[ln];
+        if (!lane_used[ln]) { CK(cudaStreamWaitEvent(ls, c->ev_fork, 0)); lane_used[ln] = true; }
+        const int l = p.l;
+        SweepLaunch L;
+        memset(&L, 0, sizeof(L));
+        const size_t slot_stride = (size_t)c->ncell_l[l] * nbins;
+        L.P = c->d_P[l]; L.acc = c->d_acc[l] + slot_stride * p.slot_base; L.accC = c->d_accC[l] + slot_stride * p.slot_base;
+        L.dirs = c->d_dirs; L.prog = c->d_prog; L.nbins = nbins; L.ncell = c->ncell_l[l]; L.Ibc = c->d_Ibc;
+        L.rows = rows_for(c, l); L.mode = MODE_J; L.stages = stages_for(c, l); L.handoff = 0;
+        L.Nb = c->pitch[l]; L.pp = c->pp[l]; L.pair = p.pair; L.rev = p.rev; L.Nc = p.Nc; L.tiles = p.tiles;
+        L.batch = c->d_batch + p.off;
+        L.nslots = p.nslots;
+        L.fresh_below = p.nslots;
+        int cap = p.pair ? c->cap_pair[l] : c->cap_single[l];
+        if (cap < 1) cap = p.nslots * p.tiles;
+        else if (cap % p.tiles == 0) cap = std::max(p.tiles, std::min(cap, p.nslots * p.tiles));
+        else cap = std::max(p.tiles, std::min(cap, (p.nslots - 1) * p.tiles));
+        if (p.nslots == 1) cap = p.tiles;
+        if (p.nslots >= p.count) cap = p.count * p.tiles;           // every entry has its own slot: one launch
+        const long long total = (long long)p.count * p.tiles;
+        for (long long item0 = 0; item0 < total; item0 += cap) {
+            L.item0 = (int)item0;
+            L.nitems = (int)std::min<long long>(cap, total - item0);
+            CK(launch_sweep_owned(L, ls));
+            ++*launches;
+        }
+    }
+    for (int ln = 0; ln < rt_ctx::kLanes; ++ln)
+        if (lane_used[ln]) {
+            CK(cudaEventRecord(c->ev_join[ln], c->lane[ln]));
+            CK(cudaStreamWaitEvent(st, c->ev_join[ln], 0));
+        }
+    if (record_events) { CK(cudaEventRecord(c->ev1, st)); c->ev_valid = true; }
+    return RT_OK;
+}
+
+// traversal + normalisation of one rt_sweep, enqueued on st
+static int enqueue_sweep(rt_ctx *c, float *J_dev, unsigned what, cudaStream_t st, bool record_events)
+{
     int launches = 0;
     int used[2];
-    int rc = run_traversal(c, MODE_J, -1, c->nbins, st, &launches, used);
+    int rc = c->overlap_on ? run_overlapped(c, st, &launches, used, record_events)
+                           : run_traversal(c, MODE_J, -1, c->nbins, st, &launches, used, nullptr, record_events);
     if (rc != RT_OK) return rc;
     CK(launch_normalise(J_dev, c->d_P[0], c->pp[0], c->d_acc[0], c->d_accC[0], used[0], c->d_acc[1], c->d_accC[1], used[1],
                         c->nx, c->ny, c->nz, c->pitch[0], c->pitch[1], c->nbins, what == RT_SUM_IN ? 1.0f : (float)(1.0 / (double)c->ndirs),
@@ -554,9 +787,57 @@ extern "C" int rt_sweep(rt_ctx *c, float *J_dev, unsigned what, void *stream)
     return RT_OK;
 }
 
+extern "C" int rt_sweep(rt_ctx *c, float *J_dev, unsigned what, void *stream)
+{
+    if (!c || !J_dev || what > 2u) return RT_EINVAL;
+    DevGuard dev_guard(c->device);
+    if (!c->fields_set) return RT_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    // A sweep of a few short launches is bound by launch latency: from its second use on, a (J buffer, what)
+    // combination is replayed as one CUDA graph (captured on an internal stream, launched into the caller's).
+    const bool want_graph = c->graph == 1 || (c->graph == -1 && c->overlap_on && c->tiny);
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (want_graph && st != nullptr && st != cudaStreamLegacy && st != cudaStreamPerThread) CK(cudaStreamIsCapturing(st, &cap));
+    if (want_graph && cap == cudaStreamCaptureStatusNone) {
+        if (!c->cap_stream) CK(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+        rt_ctx::SweepGraph *g = nullptr;
+        for (auto &e : c->graphs) if (e.J == J_dev && e.what == what) g = &e;
+        if (!g) {
+            if (c->graphs.size() >= 8) {                          // forget the oldest combination
+                if (c->graphs[0].exec) cudaGraphExecDestroy(c->graphs[0].exec);
+                if (c->graphs[0].graph) cudaGraphDestroy(c->graphs[0].graph);
+                c->graphs.erase(c->graphs.begin());
+            }
+            c->graphs.push_back(rt_ctx::SweepGraph{J_dev, what, 0, nullptr, nullptr});
+            g = &c->graphs.back();
+        }
+        if (g->seen >= 1 && !g->exec) {
+            CK(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+            int rc = enqueue_sweep(c, J_dev, what, c->cap_stream, false);
+            cudaGraph_t graph = nullptr;
+            cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
+            if (rc != RT_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+            if (e != cudaSuccess) return cuda_fail(e);
+            e = cudaGraphInstantiate(&g->exec, graph, 0);
+            if (e != cudaSuccess) { cudaGraphDestroy(graph); g->exec = nullptr; return cuda_fail(e); }
+            g->graph = graph;
+        }
+        g->seen += 1;
+        if (g->exec) {
+            CK(cudaEventRecord(c->ev0, st));
+            CK(cudaGraphLaunch(g->exec, st));
+            CK(cudaEventRecord(c->ev1, st));
+            c->ev_valid = true;                                   // here the events bracket the whole sweep, normalisation included
+            return RT_OK;
+        }
+    }
+    return enqueue_sweep(c, J_dev, what, st, true);
+}
+
 extern "C" int rt_combine(rt_ctx *c, const float *sum_dev, long long ndirs_total, unsigned what, float *J_dev, void *stream)
 {
     if (!c || !sum_dev || !J_dev || ndirs_total < 1 || what > 1u) return RT_EINVAL;
+    DevGuard dev_guard(c->device);
     if (!c->fields_set) return RT_ESTATE;
     CK(launch_combine(J_dev, sum_dev, c->d_P[0], c->pp[0], (size_t)c->ncell * c->nbins, c->nx, c->pitch[0], (float)(1.0 / (double)ndirs_total),
                       what == RT_J_TOTAL ? 1 : 0, (cudaStream_t)stream));
@@ -567,6 +848,7 @@ extern "C" int rt_sweep_rates(rt_ctx *c, float *Gamma_dev, float *Heat_dev, cons
                               const double *wH, const double *lH, void *stream)
 {
     if (!c || !Gamma_dev || !Heat_dev || !wG || !lG || !wH || !lH) return RT_EINVAL;
+    DevGuard dev_guard(c->device);
     if (!c->fields_set) return RT_ESTATE;
     std::vector<float> w4(4 * (size_t)c->nbins);
     const double *src[4] = {wG, lG, wH, lH};
@@ -586,11 +868,43 @@ extern "C" int rt_sweep_rates(rt_ctx *c, float *Gamma_dev, float *Heat_dev, cons
     return RT_OK;
 }
 
+// Source tables of rt_point_sources: persistent device copies, refilled only when the caller's tables change, through a
+// context-owned pinned staging buffer, so that the call only enqueues (no allocation, no synchronisation).
+static int upload_sources(rt_ctx *c, const int *src_fix_host, const float *lum, int nsrc, cudaStream_t st)
+{
+    const size_t nsrc3 = 3 * (size_t)nsrc, nlum = (size_t)nsrc * c->nbins;
+    const size_t bytes = sizeof(int) * nsrc3 + sizeof(float) * nlum;
+    if (c->src_valid && c->src_n == nsrc && !memcmp(c->src_stage, src_fix_host, sizeof(int) * nsrc3) &&
+        !memcmp(c->src_stage + sizeof(int) * nsrc3, lum, sizeof(float) * nlum))
+        return RT_OK;                                            // same sources as last time: the device tables stand
+    if (c->src_copy_pending) { CK(cudaEventSynchronize(c->ev_src)); c->src_copy_pending = false; }   // staging buffer still being read
+    if (bytes > c->src_cap) {
+        CK(cudaDeviceSynchronize());                             // kernels in flight may still read the old tables
+        cudaFree(c->d_src); c->d_src = nullptr;
+        if (c->src_stage) cudaFreeHost(c->src_stage);
+        c->src_stage = nullptr; c->src_cap = 0; c->src_valid = false;
+        const size_t cap = std::max<size_t>(2 * bytes, 4096);
+        cudaError_t e = cudaMalloc(&c->d_src, cap);
+        if (e == cudaSuccess) e = cudaMallocHost(&c->src_stage, cap);
+        if (e != cudaSuccess) { cudaFree(c->d_src); c->d_src = nullptr; return e == cudaErrorMemoryAllocation ? RT_ENOMEM : cuda_fail(e); }
+        c->src_cap = cap;
+        if (!c->ev_src) CK(cudaEventCreateWithFlags(&c->ev_src, cudaEventDisableTiming));
+    }
+    memcpy(c->src_stage, src_fix_host, sizeof(int) * nsrc3);
+    memcpy(c->src_stage + sizeof(int) * nsrc3, lum, sizeof(float) * nlum);
+    CK(cudaMemcpyAsync(c->d_src, c->src_stage, bytes, cudaMemcpyHostToDevice, st));
+    CK(cudaEventRecord(c->ev_src, st));
+    c->src_copy_pending = true;
+    c->src_n = nsrc; c->src_valid = true;
+    return RT_OK;
+}
+
 extern "C" int rt_point_sources(rt_ctx *c, const int *src_fix_host, const double *lum_host, int nsrc, float *Q_dev,
                                 int diag_src, int diag_bin, float *tau_dev, unsigned long long *steps_host, void *stream)
 {
     if (!c || !src_fix_host || !lum_host || nsrc < 1 || nsrc > (1 << 20) || !Q_dev) return RT_EINVAL;
-    if (c->nx > 1024 || c->ny > 1024 || c->nz > 1024) return RT_EINVAL;       // 64-bit crossing parameters
+    DevGuard dev_guard(c->device);
+    if (c->nx > 1024 || c->ny > 1024 || c->nz > 1024) return RT_EINVAL;       // crossing parameters below 2^54
     if (tau_dev && (diag_src < 0 || diag_src >= nsrc || diag_bin < 0 || diag_bin >= c->nbins)) return RT_EINVAL;
     if (!c->fields_set) return RT_ESTATE;
     const int dims[3] = {c->nx, c->ny, c->nz};
@@ -605,29 +919,25 @@ extern "C" int rt_point_sources(rt_ctx *c, const int *src_fix_host, const double
         }
     }
     cudaStream_t st = (cudaStream_t)stream;
-    int *d_src = nullptr;
-    float *d_lum = nullptr;
-    cudaError_t e = cudaMalloc(&d_src, sizeof(int) * 3 * (size_t)nsrc);
-    if (e == cudaSuccess) e = cudaMalloc(&d_lum, sizeof(float) * lum.size());
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_src, src_fix_host, sizeof(int) * 3 * (size_t)nsrc, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_lum, lum.data(), sizeof(float) * lum.size(), cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess && steps_host) e = cudaMemsetAsync(c->d_u64, 0, sizeof(unsigned long long), st);
-    if (e == cudaSuccess)
-        e = launch_point_sources(Q_dev, tau_dev, c->d_P[0], c->pp[0], c->nx, c->ny, c->nz, c->pitch[0], d_src, d_lum, nsrc,
-                                 c->nbins, (float)c->cell_width, diag_src, diag_bin, steps_host ? c->d_u64 : nullptr, st);
-    if (e == cudaSuccess && steps_host)
-        e = cudaMemcpyAsync(steps_host, c->d_u64, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st);
-    // the pageable host buffers above and the temporary device tables must outlive the enqueued work
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cudaFree(d_src); cudaFree(d_lum);
-    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RT_ENOMEM : cuda_fail(e);
+    int rc = upload_sources(c, src_fix_host, lum.data(), nsrc, st);
+    if (rc != RT_OK) return rc;
+    const int *d_src = reinterpret_cast<const int *>(c->d_src);
+    const float *d_lum = reinterpret_cast<const float *>(c->d_src + sizeof(int) * 3 * (size_t)nsrc);
+    if (steps_host) CK(cudaMemsetAsync(c->d_u64, 0, sizeof(unsigned long long), st));
+    CK(launch_point_sources(Q_dev, tau_dev, c->d_P[0], c->pp[0], c->nx, c->ny, c->nz, c->pitch[0], d_src, d_lum, nsrc,
+                            c->nbins, (float)c->cell_width, diag_src, diag_bin, steps_host ? c->d_u64 : nullptr, st));
     c->last_launches = 1;
+    if (steps_host) {                                            // the one synchronising variant: the count comes back to the host
+        CK(cudaMemcpyAsync(steps_host, c->d_u64, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
     return RT_OK;
 }
 
 extern "C" int rt_segment_counts(rt_ctx *c, int dir_index, unsigned int *counts_dev, void *stream)
 {
     if (!c || !counts_dev || dir_index < -1 || dir_index >= c->ndirs) return RT_EINVAL;
+    DevGuard dev_guard(c->device);
     int rc = ensure_buffers(c);
     if (rc != RT_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
@@ -640,9 +950,38 @@ extern "C" int rt_segment_counts(rt_ctx *c, int dir_index, unsigned int *counts_
     return RT_OK;
 }
 
+extern "C" int rt_debug_writer_counts(rt_ctx *c, unsigned long long *out_host, void *stream)
+{
+    if (!c || !out_host) return RT_EINVAL;
+    if (c->flags != RT_OWNED) return RT_EINVAL;
+    DevGuard dev_guard(c->device);
+    int rc = ensure_buffers(c);
+    if (rc != RT_OK) return rc;
+    for (int l = 0; l < 2; ++l)           // every layout must run on the owned kernel (rows <= 512 cells)
+        if (!c->order[l].empty() && !c->fast[l]) return RT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!c->d_own) {
+        cudaError_t e = cudaMalloc(&c->d_own, sizeof(unsigned long long) * 4);
+        if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RT_ENOMEM : cuda_fail(e);
+    }
+    CK(cudaMemsetAsync(c->d_own, 0, sizeof(unsigned long long) * 4, st));
+    OwnerStats own;
+    int launches = 0, used[2];
+    rc = run_traversal(c, MODE_OWNERS, -1, c->nbins, st, &launches, used, &own);
+    if (rc != RT_OK) return rc;
+    unsigned long long dev[4];
+    CK(cudaMemcpyAsync(dev, c->d_own, sizeof(dev), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    out_host[0] = dev[0]; out_host[1] = dev[1]; out_host[2] = dev[2]; out_host[3] = dev[3];
+    out_host[4] = own.launches; out_host[5] = own.partial; out_host[6] = own.expected; out_host[7] = own.entries;
+    return RT_OK;
+}
+
 extern "C" int rt_total_segments(rt_ctx *c, unsigned long long *n_host, void *stream)
 {
     if (!c || !n_host) return RT_EINVAL;
+    if (c->seg_total >= 0) { *n_host = (unsigned long long)c->seg_total; return RT_OK; }
+    DevGuard dev_guard(c->device);
     cudaStream_t st = (cudaStream_t)stream;
     if (!c->d_cnt) {
         cudaError_t e = cudaMalloc(&c->d_cnt, sizeof(unsigned) * (size_t)c->ncell);
@@ -654,12 +993,16 @@ extern "C" int rt_total_segments(rt_ctx *c, unsigned long long *n_host, void *st
     CK(launch_sum_u32(c->d_u64, c->d_cnt, c->ncell, st));
     CK(cudaMemcpyAsync(n_host, c->d_u64, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    c->seg_total = (long long)*n_host;
+    cudaFree(c->d_cnt);                  // the scratch is not needed again
+    c->d_cnt = nullptr;
     return RT_OK;
 }
 
 extern "C" int rt_sum_ds(rt_ctx *c, double *sum_host, double *min_host, double *max_host, void *stream)
 {
     if (!c || !sum_host) return RT_EINVAL;
+    DevGuard dev_guard(c->device);
     int rc = ensure_buffers(c);
     if (rc != RT_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
@@ -710,11 +1053,63 @@ extern "C" int rt_direction_records(rt_ctx *c, long long *rec, double *L_host)
     return RT_OK;
 }
 
+extern "C" int rt_working_set_bytes(rt_ctx *c, unsigned long long *bytes_host)
+{
+    if (!c || !bytes_host) return RT_EINVAL;
+    DevGuard dev_guard(c->device);
+    int rc = ensure_buffers(c);
+    if (rc != RT_OK) return rc;
+    unsigned long long b = 0;
+    for (int l = 0; l < 2; ++l) {
+        b += sizeof(float2) * (unsigned long long)c->ncell_l[l] * c->nbins;                        // packed fields
+        b += 2ull * sizeof(float) * (unsigned long long)c->ncell_l[l] * c->nbins * c->slots[l];   // slot + seam accumulators
+    }
+    *bytes_host = b;
+    return RT_OK;
+}
+
+extern "C" int rt_probe_bandwidth(unsigned long long bytes, int mode, int iters, double *gbs_host, void *stream)
+{
+    if (bytes < (1ull << 20) || bytes > (1ull << 36) || (mode != 0 && mode != 1) || iters < 1 || iters > 1000 || !gbs_host) return RT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 148;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const size_t n4 = (size_t)(bytes / 16);
+    float4 *buf = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaError_t e = cudaMalloc(&buf, n4 * 16);
+    if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? RT_ENOMEM : cuda_fail(e);
+    if (e == cudaSuccess) e = cudaMemsetAsync(buf, 0, n4 * 16, st);
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    double best = 0.0;
+    // enough passes per launch that it lasts of the order of a millisecond (about 8 GB of accesses)
+    const int reps = (int)std::max<unsigned long long>(1, std::min<unsigned long long>(512, (8ull << 30) / (n4 * 16)));
+    for (int w = 0; w < 2 && e == cudaSuccess; ++w) e = launch_probe(buf, n4, mode, 1, sms, st);   // warm-up: fills L2 if it fits
+    for (int i = 0; i < iters && e == cudaSuccess; ++i) {
+        e = cudaEventRecord(e0, st);
+        if (e == cudaSuccess) e = launch_probe(buf, n4, mode, reps, sms, st);
+        if (e == cudaSuccess) e = cudaEventRecord(e1, st);
+        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+        float ms = 0.0f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (e == cudaSuccess && ms > 0.0f) best = std::max(best, (double)(n4 * 16) * reps * (mode ? 2.0 : 1.0) / (ms * 1e-3) / 1e9);
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(buf);
+    if (e != cudaSuccess) return cuda_fail(e);
+    *gbs_host = best;
+    return RT_OK;
+}
+
 extern "C" int rt_last_launch_count(rt_ctx *c) { return c ? c->last_launches : RT_EINVAL; }
 
 extern "C" float rt_last_sweep_kernel_ms(rt_ctx *c)
 {
     if (!c || !c->ev_valid) return -1.0f;
+    DevGuard dev_guard(c->device);
     if (cudaEventSynchronize(c->ev1) != cudaSuccess) return -1.0f;
     float ms = -1.0f;
     if (cudaEventElapsedTime(&ms, c->ev0, c->ev1) != cudaSuccess) return -1.0f;
@@ -724,6 +1119,7 @@ extern "C" float rt_last_sweep_kernel_ms(rt_ctx *c)
 extern "C" int rt_destroy(rt_ctx *c)
 {
     if (!c) return RT_OK;
+    DevGuard dev_guard(c->device);
     cudaDeviceSynchronize();
     free_device(c);
     delete c;

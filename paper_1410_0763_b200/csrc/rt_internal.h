@@ -44,7 +44,9 @@ __host__ __device__ __forceinline__ int sub_offset(int sub, int which)
     return (2 * idx + 1) * (int)(kOne / (2 * r));
 }
 
-enum Mode : int { MODE_J = 0, MODE_COUNT = 1, MODE_DS = 2 };
+// MODE_OWNERS (rt_debug_writer_counts): the J-mode schedule with every accumulator store replaced by an atomic
+// increment of the stored-to element, so that the number of writers per cell, accumulator array and launch can be read back
+enum Mode : int { MODE_J = 0, MODE_COUNT = 1, MODE_DS = 2, MODE_OWNERS = 3 };
 
 struct SweepLaunch {
     const float2 *P;         // packed (kappa, S) field of the batch's layout, [nbins][cells]
@@ -80,13 +82,14 @@ __host__ __device__ __forceinline__ size_t field_index(size_t o, int pp) { retur
 __host__ __device__ __forceinline__ int field_s_offset(int pp) { return pp ? 2 : 1; }
 
 // launchers (rt_kernels.cu); all return cudaError_t of the launch
-cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, SlabProg *prog, double cell_width,
+cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, int max_na, SlabProg *prog, double cell_width,
                                   const double *Lvals, cudaStream_t st);
 cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat, float2 *PT, int ppN, int ppT,
                                int nx, int ny, int nz, int nxp, int nyp, int nbins, cudaStream_t st);
 bool owned_supported(int Nb, int Nc, int rows);
 int owned_ctas_per_sm(int Nb, int rows, int stages, bool pair);
 constexpr int kOwnedWarpsPerCta = 4;
+constexpr int kShortRowStages = 2;             // TMA ring depth for rows of <= 64 cells (rt_api.cu stages_for)
 cudaError_t launch_sweep_owned(const SweepLaunch &L, cudaStream_t st);
 cudaError_t launch_sweep_generic(const SweepLaunch &L, int max_lattice_b, int max_lattice_c, cudaStream_t st);
 cudaError_t launch_normalise(float *J, const float2 *Pnat, int ppN, const float *accN, const float *accNC, int slotsN,
@@ -107,5 +110,10 @@ cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const fl
 cudaError_t launch_ds_reduce(double *out3, const float *acc, const float *accC, long long ncell, int pitch, int width,
                              cudaStream_t st);
 cudaError_t launch_sum_u32(unsigned long long *out, const unsigned *counts, long long n, cudaStream_t st);
+// writer counts of one launch in MODE_OWNERS: out2[0] = max(out2[0], max_i w[i]), out2[1] += sum_i w[i] over n floats
+cudaError_t launch_owner_reduce(unsigned long long *out2, const float *w, long long n, cudaStream_t st);
+
+// `reps` passes of the streaming probe over n4 float4 in one launch (rmw = 0: read, 1: read-modify-write)
+cudaError_t launch_probe(float4 *buf, size_t n4, int rmw, int reps, int sm_count, cudaStream_t st);
 
 }  // namespace rt

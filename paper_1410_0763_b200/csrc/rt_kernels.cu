@@ -12,7 +12,12 @@
 // See DESIGN.md for the data layout and why the ownership scheme replaces the four ray groups.
 #include "rt_internal.h"
 
+#include <algorithm>
+#include <type_traits>
+
 namespace rt {
+
+constexpr long long kMaxGridZ = 65535;       // planes (bin, z) per launch of the per-plane kernels; taller stacks loop
 
 // ------------------------------------------------------------------------------------------------
 // Slab programs
@@ -60,13 +65,13 @@ __global__ void k_build_programs(const DirDev *__restrict__ dirs, int ndirs, Sla
     prog[D.prog_off + k] = s;
 }
 
-cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, SlabProg *prog, double cell_width,
+cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, int max_na, SlabProg *prog, double cell_width,
                                   const double *Lvals, cudaStream_t st)
 {
-    // Na <= max dim; launch enough threads for the largest (bounded by 65535 blocks in y: loop)
+    // one thread per (direction, slab): grid.x covers the longest march, grid.y the directions (65535 at most: loop)
     for (int d0 = 0; d0 < ndirs; d0 += 32768) {
         int nd = ndirs - d0 < 32768 ? ndirs - d0 : 32768;
-        dim3 grid(64, nd);     // 64*256 = 16384 slabs max
+        dim3 grid((max_na + 255) / 256, nd);
         k_build_programs<<<grid, 256, 0, st>>>(dirs + d0, nd, prog, cell_width, Lvals + d0);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
@@ -79,12 +84,13 @@ cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, SlabProg *prog,
 // ------------------------------------------------------------------------------------------------
 __global__ void k_pack_fields(const float *__restrict__ kappa, const float *__restrict__ S,
                               float2 *__restrict__ Pnat, float2 *__restrict__ PT, int ppN, int ppT, int nx, int ny, int nz,
-                              int nxp, int nyp)
+                              int nxp, int nyp, int zb0)
 {
     float *__restrict__ fN = reinterpret_cast<float *>(Pnat);
     float *__restrict__ fT = reinterpret_cast<float *>(PT);
     __shared__ float2 tile[32][33];
-    const int bin = blockIdx.z / nz, z = blockIdx.z % nz;
+    const int zb = (int)blockIdx.z + zb0;                  // (bin, z) planes; grid.z holds at most 65535 of them per launch
+    const int bin = zb / nz, z = zb % nz;
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
     const size_t ncell = (size_t)nx * ny * nz;
     const size_t boff = (size_t)bin * ncell;
@@ -115,9 +121,14 @@ __global__ void k_pack_fields(const float *__restrict__ kappa, const float *__re
 cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat, float2 *PT, int ppN, int ppT,
                                int nx, int ny, int nz, int nxp, int nyp, int nbins, cudaStream_t st)
 {
-    dim3 grid((nx + 31) / 32, (ny + 31) / 32, nz * nbins), block(32, 8);
-    k_pack_fields<<<grid, block, 0, st>>>(kappa, S, Pnat, PT, ppN, ppT, nx, ny, nz, nxp, nyp);
-    return cudaGetLastError();
+    const long long planes = (long long)nz * nbins;
+    for (long long zb0 = 0; zb0 < planes; zb0 += kMaxGridZ) {
+        dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, planes - zb0)), block(32, 8);
+        k_pack_fields<<<grid, block, 0, st>>>(kappa, S, Pnat, PT, ppN, ppT, nx, ny, nz, nxp, nyp, (int)zb0);
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -295,25 +306,34 @@ cudaError_t launch_sweep_generic(const SweepLaunch &L, int np_max, int nq_max, c
 // Sums the slot and seam accumulators of the native layout and, through a shared-memory tile
 // transpose, of the transposed layout.
 // ------------------------------------------------------------------------------------------------
+template <bool COUNTS> __device__ __forceinline__ typename std::conditional<COUNTS, unsigned long long, double>::type widen(float v);
+template <> __device__ __forceinline__ unsigned long long widen<true>(float v) { return (unsigned long long)__float2uint_rn(v); }
+template <> __device__ __forceinline__ double widen<false>(float v) { return (double)v; }
+
 template <bool COUNTS>
 __global__ void k_finalise(float *__restrict__ J, unsigned *__restrict__ counts, const float2 *__restrict__ Pnat, int ppN,
                            const float *__restrict__ accN, const float *__restrict__ accNC, int slotsN,
                            const float *__restrict__ accT, const float *__restrict__ accTC, int slotsT,
-                           int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, int add_S)
+                           int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, int add_S, int zb0)
 {
-    __shared__ float tile[32][33];
-    const int bin = blockIdx.z / nz, z = blockIdx.z % nz;
+    using SumT = typename std::conditional<COUNTS, unsigned long long, double>::type;
+    __shared__ SumT tile[32][33];
+    const int zb = (int)blockIdx.z + zb0;
+    const int bin = zb / nz, z = zb % nz;
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
     const size_t ncell = (size_t)nx * ny * nz;
     const size_t ncellN = (size_t)nxp * ny * nz, ncellT = (size_t)nyp * nz * nx;      // padded row pitch per layout
     const size_t strideN = ncellN * nbins, strideT = ncellT * nbins;
+    // The slot partials are summed in fp64 (J) or as integers (counts: every slot partial is an exact integer below
+    // 2^24, rt_create bounds 3 N_d r^2): the kernel is bound by its loads, and the sum over up to a few hundred slot
+    // and seam partials then adds no rounding of its own to J.
     // transposed layout [x][z][y]: coalesced along y
     for (int dx = threadIdx.y; dx < 32; dx += blockDim.y) {
         const int x = x0 + dx, y = y0 + threadIdx.x;
-        float s = 0.0f;
+        SumT s = 0;
         if (x < nx && y < ny) {
             const size_t i = (size_t)bin * ncellT + ((size_t)x * nz + z) * nyp + y;
-            for (int sl = 0; sl < slotsT; ++sl) s += accT[sl * strideT + i] + accTC[sl * strideT + i];
+            for (int sl = 0; sl < slotsT; ++sl) s += widen<COUNTS>(accT[sl * strideT + i]) + widen<COUNTS>(accTC[sl * strideT + i]);
         }
         tile[dx][threadIdx.x] = s;
     }
@@ -323,15 +343,15 @@ __global__ void k_finalise(float *__restrict__ J, unsigned *__restrict__ counts,
         if (x < nx && y < ny) {
             const size_t i = (size_t)bin * ncell + ((size_t)z * ny + y) * nx + x;
             const size_t ip = (size_t)bin * ncellN + ((size_t)z * ny + y) * nxp + x;
-            float s = tile[threadIdx.x][dy];
-            for (int sl = 0; sl < slotsN; ++sl) s += accN[sl * strideN + ip] + accNC[sl * strideN + ip];
+            SumT s = tile[threadIdx.x][dy];
+            for (int sl = 0; sl < slotsN; ++sl) s += widen<COUNTS>(accN[sl * strideN + ip]) + widen<COUNTS>(accNC[sl * strideN + ip]);
             if (COUNTS) {
-                counts[i] = (unsigned)__float2uint_rn(s);
+                counts[i] = (unsigned)s;
             } else {
                 const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
                 const size_t o = field_index(ip, ppN);
                 const float2 ks = make_float2(fN[o], fN[o + field_s_offset(ppN)]);
-                const float jin = s * inv_nd / ks.x;
+                const float jin = (float)(s * (double)inv_nd) / ks.x;
                 J[i] = add_S ? jin + ks.y : jin;
             }
         }
@@ -342,10 +362,15 @@ cudaError_t launch_normalise(float *J, const float2 *Pnat, int ppN, const float 
                              const float *accT, const float *accTC, int slotsT,
                              int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, int add_S, cudaStream_t st)
 {
-    dim3 grid((nx + 31) / 32, (ny + 31) / 32, nz * nbins), block(32, 8);
-    k_finalise<false><<<grid, block, 0, st>>>(J, nullptr, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT,
-                                              nx, ny, nz, nxp, nyp, nbins, inv_nd, add_S);
-    return cudaGetLastError();
+    const long long planes = (long long)nz * nbins;
+    for (long long zb0 = 0; zb0 < planes; zb0 += kMaxGridZ) {
+        dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, planes - zb0)), block(32, 8);
+        k_finalise<false><<<grid, block, 0, st>>>(J, nullptr, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT,
+                                                  nx, ny, nz, nxp, nyp, nbins, inv_nd, add_S, (int)zb0);
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -358,10 +383,10 @@ struct RateWeights { float wG[16], lG[16], wH[16], lH[16]; };
 __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, const float2 *__restrict__ Pnat, int ppN,
                         const float *__restrict__ accN, const float *__restrict__ accNC, int slotsN,
                         const float *__restrict__ accT, const float *__restrict__ accTC, int slotsT,
-                        int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, const RateWeights W)
+                        int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, const RateWeights W, int z0)
 {
-    __shared__ float tile[32][33];
-    const int z = blockIdx.z;
+    __shared__ double tile[32][33];
+    const int z = (int)blockIdx.z + z0;
     const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 32;
     const size_t ncellN = (size_t)nxp * ny * nz, ncellT = (size_t)nyp * nz * nx;
     const size_t strideN = ncellN * nbins, strideT = ncellT * nbins;
@@ -371,10 +396,10 @@ __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, con
         // transposed layout [x][z][y]: coalesced along y
         for (int dx = threadIdx.y; dx < 32; dx += blockDim.y) {
             const int x = x0 + dx, y = y0 + threadIdx.x;
-            float s = 0.0f;
+            double s = 0.0;
             if (x < nx && y < ny) {
                 const size_t i = (size_t)bin * ncellT + ((size_t)x * nz + z) * nyp + y;
-                for (int sl = 0; sl < slotsT; ++sl) s += accT[sl * strideT + i] + accTC[sl * strideT + i];
+                for (int sl = 0; sl < slotsT; ++sl) s += (double)accT[sl * strideT + i] + (double)accTC[sl * strideT + i];
             }
             tile[dx][threadIdx.x] = s;
         }
@@ -384,11 +409,11 @@ __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, con
             const int x = x0 + threadIdx.x, y = y0 + dy;
             if (x < nx && y < ny) {
                 const size_t i = (size_t)bin * ncellN + ((size_t)z * ny + y) * nxp + x;
-                float s = tile[threadIdx.x][dy];
-                for (int sl = 0; sl < slotsN; ++sl) s += accN[sl * strideN + i] + accNC[sl * strideN + i];
+                double s = tile[threadIdx.x][dy];
+                for (int sl = 0; sl < slotsN; ++sl) s += (double)accN[sl * strideN + i] + (double)accNC[sl * strideN + i];
                 const size_t o = field_index(i, ppN);
                 const float kap = fN[o], src = fN[o + field_s_offset(ppN)];
-                const float jin = s * inv_nd / kap;
+                const float jin = (float)(s * (double)inv_nd) / kap;
                 g[j] = fmaf(W.wG[bin], jin, fmaf(W.lG[bin], src, g[j]));
                 h[j] = fmaf(W.wH[bin], jin, fmaf(W.lH[bin], src, h[j]));
             }
@@ -417,10 +442,14 @@ cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN,
         W.wG[b] = in ? w4[b] : 0.0f;             W.lG[b] = in ? w4[nbins + b] : 0.0f;
         W.wH[b] = in ? w4[2 * nbins + b] : 0.0f; W.lH[b] = in ? w4[3 * nbins + b] : 0.0f;
     }
-    dim3 grid((nx + 31) / 32, (ny + 31) / 32, nz), block(32, 8);
-    k_rates<<<grid, block, 0, st>>>(Gamma, Heat, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT, nx, ny, nz, nxp, nyp,
-                                   nbins, inv_nd, W);
-    return cudaGetLastError();
+    for (long long z0 = 0; z0 < nz; z0 += kMaxGridZ) {
+        dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, nz - z0)), block(32, 8);
+        k_rates<<<grid, block, 0, st>>>(Gamma, Heat, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT, nx, ny, nz, nxp, nyp,
+                                       nbins, inv_nd, W, (int)z0);
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -461,6 +490,29 @@ cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int p
 // ------------------------------------------------------------------------------------------------
 constexpr int kPsFix = 256;
 
+// Crossing parameters T_i (position along the ray in units of 1 / |dx dy dz|) are exact integers below 2^54.  For
+// meshes up to 512 cells per axis they stay below 2^52 and are held in fp64 (TT = double): every add, compare and
+// difference is exact there too, and costs one instruction instead of the two to three a 64-bit integer takes on
+// the 32-bit ALU.  Larger meshes (up to 1024) use 64-bit integers.
+template <class TT> struct PsInf;
+template <> struct PsInf<double> { static __device__ __forceinline__ double v() { return 1.0e300; } };
+template <> struct PsInf<long long> { static __device__ __forceinline__ long long v() { return 0x7fffffffffffffffll; } };
+
+// plain minimum (no NaN handling: the operands are exact integers or the "never" marker)
+template <class TT> __device__ __forceinline__ TT ps_min(TT a, TT b) { return a < b ? a : b; }
+// one axis of a ray step: if this axis' next plane is the one reached (T == Tn), move to the next cell along it and
+// schedule its next plane.  Predicated adds instead of selects: three instructions per axis.
+__device__ __forceinline__ void ps_advance(double &T, int &idx, double Tn, double inc, int didx)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.eq.f64 p, %0, %2;\n\t@p add.f64 %0, %0, %3;\n\t@p add.s32 %1, %1, %4;\n\t}"
+        : "+d"(T), "+r"(idx) : "d"(Tn), "d"(inc), "r"(didx));
+}
+__device__ __forceinline__ void ps_advance(long long &T, int &idx, long long Tn, long long inc, int didx)
+{
+    if (T == Tn) { idx += didx; T += inc; }
+}
+
+template <class TT>
 __global__ void __launch_bounds__(128)
 k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2 *__restrict__ Pnat, int ppN,
                 int nx, int ny, int nz, int nxp, const int *__restrict__ src, const float *__restrict__ lum, int nsrc,
@@ -472,16 +524,18 @@ k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2
     const bool live = cidx < ncell;
     const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
     const size_t boffN = (size_t)bin * nxp * ny * nz;
-    const int dims[3] = {nx, ny, nz};
     unsigned nstep = 0;
     if (live) {
         const int tgt[3] = {(int)(cidx % nx), (int)((cidx / nx) % ny), (int)(cidx / ((long long)nx * ny))};
         const float kap_t = fN[field_index(boffN + ((size_t)tgt[2] * ny + tgt[1]) * nxp + tgt[0], ppN)];
+        const float *__restrict__ fbin = fN + 2 * boffN;          // this bin's plane of the packed copy (boffN is even: nxp is)
         double q = 0.0;
         // linear index of a cell in the packed native copy (row pitch nxp) and its change per step along an axis
         const int idx_t = (tgt[2] * ny + tgt[1]) * nxp + tgt[0];
+        const TT kInf = PsInf<TT>::v();
         for (int a = 0; a < nsrc; ++a) {
-            long long s[3], d[3], ad[3], T[3], inc[3];
+            long long s[3], d[3], ad[3];
+            TT T[3], inc[3];
             int stp[3], cur[3];
             double len2 = 0.0;
 #pragma unroll
@@ -503,35 +557,38 @@ k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2
             const double Dn = (double)f0 * (double)f1 * (double)f2;
             const double len = sqrt(len2) / kPsFix * (double)cell_width;
             const double scale = len / Dn;                          // length per unit of T
-            const long long kInf = 0x7fffffffffffffffll;
 #pragma unroll
             for (int i = 0; i < 3; ++i) {
-                if (stp[i] == 0) { T[i] = kInf; inc[i] = 0; continue; }
+                if (stp[i] == 0) { T[i] = kInf; inc[i] = (TT)0; continue; }
                 const long long plane = (long long)(cur[i] + (stp[i] > 0 ? 1 : 0)) * kPsFix;
-                T[i] = (plane - s[i]) * stp[i] * W[i];
-                inc[i] = (long long)kPsFix * W[i];
+                T[i] = (TT)((plane - s[i]) * stp[i] * W[i]);
+                inc[i] = (TT)((long long)kPsFix * W[i]);
             }
-            double tau = 0.0;
-            long long T0 = 0;
+            // Every piece has positive length: T_i > 0 at the start (a source on a boundary belongs to the cell the ray
+            // moves into) and all axes that reach Tn step together, so the next Tn is larger.  tau is summed in units
+            // of T and scaled once.
+            double tauT = 0.0;
+            TT T0 = (TT)0;
             double r_in = 0.0, r_out = 0.0, dr = 0.0;
             for (;;) {
-                const long long Tn = min(T[0], min(T[1], T[2]));
+                const TT Tn = ps_min(T[0], ps_min(T[1], T[2]));
                 if (idx == idx_t) {                                 // (padded linear indices of distinct cells differ)
                     if (Tn == kInf) { r_in = 0.0; dr = r_out = 0.5 * (double)cell_width; }   // source at this cell's centre
                     else { r_in = (double)T0 * scale; dr = (double)(Tn - T0) * scale; r_out = r_in + dr; }
                     nstep += 1;
                     break;
                 }
-                if (Tn > T0) {
-                    const float kap = fN[field_index(boffN + (size_t)idx, ppN)];
-                    tau = fma((double)kap, (double)(Tn - T0) * scale, tau);
-                    nstep += 1;
-                }
-#pragma unroll
-                for (int i = 0; i < 3; ++i)
-                    if (T[i] == Tn) { idx += didx[i]; T[i] += inc[i]; }
+                // kappa of cell idx in the packed native copy: float index 2 o - (o & 1) if pair-packed, else 2 o
+                // (rt_internal.h field_index; the bin offset is even)
+                const float kap = fbin[2 * idx - (idx & ppN)];
+                tauT = fma((double)kap, (double)(Tn - T0), tauT);
+                nstep += 1;
+                ps_advance(T[0], idx, Tn, inc[0], didx[0]);
+                ps_advance(T[1], idx, Tn, inc[1], didx[1]);
+                ps_advance(T[2], idx, Tn, inc[2], didx[2]);
                 T0 = Tn;
             }
+            const double tau = tauT * scale;
             const double dtau = (double)kap_t * dr;
             const double vol = 4.0 * 3.14159265358979323846 / 3.0 * dr * (r_out * r_out + r_out * r_in + r_in * r_in);
             q += (double)lum[(size_t)a * nbins + bin] * exp(-tau) * (-expm1(-dtau)) / vol;
@@ -544,7 +601,6 @@ k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2
         for (int o = 16; o > 0; o >>= 1) n += __shfl_xor_sync(0xffffffffu, n, o);
         if ((threadIdx.x & 31) == 0 && n) atomicAdd(steps, (unsigned long long)n);
     }
-    (void)dims;
 }
 
 cudaError_t launch_point_sources(float *Q, float *tau_out, const float2 *Pnat, int ppN, int nx, int ny, int nz, int nxp,
@@ -553,8 +609,12 @@ cudaError_t launch_point_sources(float *Q, float *tau_out, const float2 *Pnat, i
 {
     const long long ncell = (long long)nx * ny * nz;
     dim3 grid((unsigned)((ncell + 127) / 128), 1, nbins);
-    k_point_sources<<<grid, 128, 0, st>>>(Q, tau_out, Pnat, ppN, nx, ny, nz, nxp, src_dev, lum_dev, nsrc, nbins, cell_width,
-                                          diag_src, diag_bin, steps_dev);
+    if (nx <= 512 && ny <= 512 && nz <= 512)
+        k_point_sources<double><<<grid, 128, 0, st>>>(Q, tau_out, Pnat, ppN, nx, ny, nz, nxp, src_dev, lum_dev, nsrc, nbins, cell_width,
+                                                      diag_src, diag_bin, steps_dev);
+    else
+        k_point_sources<long long><<<grid, 128, 0, st>>>(Q, tau_out, Pnat, ppN, nx, ny, nz, nxp, src_dev, lum_dev, nsrc, nbins, cell_width,
+                                                         diag_src, diag_bin, steps_dev);
     return cudaGetLastError();
 }
 
@@ -562,10 +622,14 @@ cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const fl
                                    const float *accT, const float *accTC, int slotsT,
                                    int nx, int ny, int nz, int nxp, int nyp, cudaStream_t st)
 {
-    dim3 grid((nx + 31) / 32, (ny + 31) / 32, nz), block(32, 8);
-    k_finalise<true><<<grid, block, 0, st>>>(nullptr, counts, nullptr, 0, accN, accNC, slotsN, accT, accTC, slotsT,
-                                             nx, ny, nz, nxp, nyp, 1, 1.0f, 0);
-    return cudaGetLastError();
+    for (long long zb0 = 0; zb0 < nz; zb0 += kMaxGridZ) {
+        dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, nz - zb0)), block(32, 8);
+        k_finalise<true><<<grid, block, 0, st>>>(nullptr, counts, nullptr, 0, accN, accNC, slotsN, accT, accTC, slotsT,
+                                                 nx, ny, nz, nxp, nyp, 1, 1.0f, 0, (int)zb0);
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 __device__ __forceinline__ double warp_sum(double v)
@@ -608,6 +672,34 @@ cudaError_t launch_ds_reduce(double *out3, const float *acc, const float *accC, 
     return cudaGetLastError();
 }
 
+// MODE_OWNERS: every element of w holds the number of stores it received in one launch (an exact small integer)
+__global__ void k_owner_reduce(unsigned long long *out2, const float *__restrict__ w, long long n)
+{
+    unsigned mx = 0;
+    unsigned long long s = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const unsigned v = __float2uint_rn(w[i]);
+        mx = max(mx, v);
+        s += v;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        s += __shfl_xor_sync(0xffffffffu, s, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicMax(&out2[0], (unsigned long long)mx);
+        atomicAdd(&out2[1], s);
+    }
+}
+
+cudaError_t launch_owner_reduce(unsigned long long *out2, const float *w, long long n, cudaStream_t st)
+{
+    int blocks = (int)((n + 1023) / 1024);
+    if (blocks > 1184) blocks = 1184;
+    k_owner_reduce<<<blocks, 256, 0, st>>>(out2, w, n);
+    return cudaGetLastError();
+}
+
 __global__ void k_sum_u32(unsigned long long *out, const unsigned *__restrict__ c, long long n)
 {
     unsigned long long s = 0;
@@ -621,6 +713,47 @@ cudaError_t launch_sum_u32(unsigned long long *out, const unsigned *counts, long
     int blocks = (int)((n + 1023) / 1024);
     if (blocks > 592) blocks = 592;
     k_sum_u32<<<blocks, 256, 0, st>>>(out, counts, n);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// Streaming bandwidth probe (rt_probe_bandwidth): the roofline denominators of the memory levels that
+// MEASURED_PEAKS.json does not carry (L2), measured with the same instruction mix the sweep's memory side has:
+// 16-byte cache-global loads, and a read-modify-write of every element.
+// ------------------------------------------------------------------------------------------------
+template <int RMW>
+__global__ void __launch_bounds__(512) k_probe(float4 *__restrict__ buf, size_t n4, int reps, float4 *__restrict__ sink)
+{
+    // `reps` passes over the buffer inside one launch (a single pass over an L2-sized buffer lasts a few microseconds,
+    // less than a launch); four independent 16-byte accesses per thread and iteration
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int r = 0; r < reps; ++r) {
+        size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+        for (; i + 3 * stride < n4; i += 4 * stride) {
+            float4 v0 = __ldcg(buf + i), v1 = __ldcg(buf + i + stride), v2 = __ldcg(buf + i + 2 * stride), v3 = __ldcg(buf + i + 3 * stride);
+            if (RMW) {
+                v0.x += 1.0f; v1.x += 1.0f; v2.x += 1.0f; v3.x += 1.0f;
+                __stcg(buf + i, v0); __stcg(buf + i + stride, v1); __stcg(buf + i + 2 * stride, v2); __stcg(buf + i + 3 * stride, v3);
+            } else {
+                acc.x += v0.x + v1.x + v2.x + v3.x; acc.y += v0.y + v1.y + v2.y + v3.y;
+                acc.z += v0.z + v1.z + v2.z + v3.z; acc.w += v0.w + v1.w + v2.w + v3.w;
+            }
+        }
+        for (; i < n4; i += stride) {
+            float4 v = __ldcg(buf + i);
+            if (RMW) { v.x += 1.0f; __stcg(buf + i, v); }
+            else { acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w; }
+        }
+    }
+    if (!RMW && acc.x + acc.y + acc.z + acc.w == -1.0f) *sink = acc;      // never true for the zeroed buffer: keeps the loads
+}
+
+cudaError_t launch_probe(float4 *buf, size_t n4, int rmw, int reps, int sm_count, cudaStream_t st)
+{
+    const int blocks = 8 * sm_count;
+    if (rmw) k_probe<1><<<blocks, 512, 0, st>>>(buf, n4, reps, buf);
+    else     k_probe<0><<<blocks, 512, 0, st>>>(buf, n4, reps, buf);
     return cudaGetLastError();
 }
 

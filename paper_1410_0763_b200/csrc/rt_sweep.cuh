@@ -90,17 +90,60 @@ __device__ __forceinline__ void unpack(const float4 &v, float2 &kap, float2 &src
 //   A = x (c0 + c1 x + c2 x^2 + c3 x^3)  (fitted on [0, 1/4], rel. error 3.4e-7)
 //     = t (d0 + d1 t + d2 t^2 + d3 t^3),  d_k = c_k (-ln 2)^(k+1).
 // ------------------------------------------------------------------------------------------------
+#ifndef RT_EXPVAR
+#define RT_EXPVAR 0
+#endif
+__device__ __forceinline__ float  vexact_e(float t) { return exp2f(t); }
+__device__ __forceinline__ float2 vexact_e(float2 t) { return make_float2(exp2f(t.x), exp2f(t.y)); }
+__device__ __forceinline__ float  vexact_A(float t) { return -expm1f(t * 0.6931471805599453f); }
+__device__ __forceinline__ float2 vexact_A(float2 t) { return make_float2(-expm1f(t.x * 0.6931471805599453f), -expm1f(t.y * 0.6931471805599453f)); }
 template <class T>
 __device__ __forceinline__ T one_minus_exp(T kap, T ctv, T &e)
 {
     const T t = vmul(kap, ctv);
+#if RT_EXPVAR & 8
+    e = vexact_e(t);
+    return vexact_A(t);
+#else
     e = vex2(t);
+#if RT_EXPVAR & 4
+    constexpr float thr = -0.7213475204444817f;
+    T p = vfma(t, vsplat<T>(-0.0010833843844011426f), vsplat<T>(-0.009464533999562263f));
+    p = vfma(t, p, vsplat<T>(-0.05546464025974274f));
+    p = vfma(t, p, vsplat<T>(-0.24022290110588074f));
+    p = vfma(t, p, vsplat<T>(-0.6931471228599548f));
+#elif RT_EXPVAR & 2
+    constexpr float thr = -0.36067376022224085f;
+    T p = vfma(t, vsplat<T>(-0.0012016557157039642f), vsplat<T>(-0.009577106684446335f));
+    p = vfma(t, p, vsplat<T>(-0.05549883097410202f));
+    p = vfma(t, p, vsplat<T>(-0.24022626876831055f));
+    p = vfma(t, p, vsplat<T>(-0.6931471824645996f));
+#else
+    constexpr float thr = -0.36067376022224085f;
     T p = vfma(t, vsplat<T>(-0.00871029682457447f), vsplat<T>(-0.055303432047367096f));
     p = vfma(t, p, vsplat<T>(-0.24021217226982117f));
     p = vfma(t, p, vsplat<T>(-0.6931470036506653f));
+#endif
     const T As = vmul(t, p);
     const T Ab = vfma(e, vsplat<T>(-1.0f), vsplat<T>(1.0f));       // 1 - e, one rounding
-    return vsel_gt(t, -0.36067376022224085f, As, Ab);              // x < 1/4
+#if RT_EXPVAR & 1
+    e = vsel_gt(t, thr, vfma(As, vsplat<T>(-1.0f), vsplat<T>(1.0f)), e);
+#endif
+    return vsel_gt(t, thr, As, Ab);
+#endif
+}
+
+// Store of a finished accumulator chunk: the one writer of these cells in this launch and array.  In MODE_OWNERS
+// (rt_debug_writer_counts) the store becomes an atomic increment of every element it would have written, so that
+// "one writer per cell, accumulator array and launch" can be read back instead of assumed.
+template <int MODE> __device__ __forceinline__ void acc_store(float *p, float v)
+{
+    if (MODE == MODE_OWNERS) atomicAdd(p, 1.0f); else *p = v;
+}
+template <int MODE> __device__ __forceinline__ void acc_store(float *p, float2 v)
+{
+    if (MODE == MODE_OWNERS) { atomicAdd(p, 1.0f); atomicAdd(p + 1, 1.0f); }
+    else *reinterpret_cast<float2 *>(p) = v;
 }
 
 // ND intensities (1, or 2 for a mirror pair) cross the same cell piece: e, A and S*A are shared.
@@ -117,7 +160,7 @@ __device__ __forceinline__ void seg_update(T (&I)[ND], T kap, T src, float len, 
         for (int d = 0; d < ND; ++d) I[d] = vfma(I[d], e, SA);   // eq. 7
     } else if (MODE == MODE_COUNT) {
         part = vadd(part, vsplat<T>((float)ND));
-    } else {
+    } else if (MODE == MODE_DS) {
         part = vadd(part, vsplat<T>((float)ND * len));
     }
 }
@@ -277,7 +320,7 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
                     // the row above the CTA's tile has another owner: seam accumulator, plain stores
 #pragma unroll
                     for (int g = 0; g < G; ++g)
-                        *reinterpret_cast<T *>(rowp[R] + RT_MG(g)) = vfma(part_hi[g], invLv, RT_OLD(R, g));
+                        acc_store<MODE>(rowp[R] + RT_MG(g), vfma(part_hi[g], invLv, RT_OLD(R, g)));
                 } else {
                     // row 0 of the next warp: put the partial into the handoff ring and announce it (the slot is
                     // free once that warp has taken the partial of two stepping slabs ago)
@@ -292,7 +335,7 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
         } else {
 #pragma unroll
             for (int g = 0; g < G; ++g)
-                *reinterpret_cast<T *>(rowp[r + 1] + RT_MG(g)) = vfma(part_hi[g], invLv, RT_OLD(r + 1, g));
+                acc_store<MODE>(rowp[r + 1] + RT_MG(g), vfma(part_hi[g], invLv, RT_OLD(r + 1, g)));
         }
 #pragma unroll
         for (int g = 0; g < G; ++g) part_hi[g] = part_lo[g];
@@ -302,14 +345,14 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
         mbar_wait(seam.full_in, seam.par_full);
 #pragma unroll
         for (int g = 0; g < G; ++g)
-            *reinterpret_cast<T *>(rowp[0] + RT_MG(g)) =
-                vadd(vfma(part_hi[g], invLv, RT_OLD(0, g)), *reinterpret_cast<const T *>(seam.ring_in + RT_MG(g) * (int)sizeof(float)));
+            acc_store<MODE>(rowp[0] + RT_MG(g),
+                            vadd(vfma(part_hi[g], invLv, RT_OLD(0, g)), *reinterpret_cast<const T *>(seam.ring_in + RT_MG(g) * (int)sizeof(float))));
         __syncwarp();
         if (lane == 0) mbar_arrive(seam.empty_in);
     } else {
 #pragma unroll
         for (int g = 0; g < G; ++g)
-            *reinterpret_cast<T *>(rowp[0] + RT_MG(g)) = vfma(part_hi[g], invLv, RT_OLD(0, g));
+            acc_store<MODE>(rowp[0] + RT_MG(g), vfma(part_hi[g], invLv, RT_OLD(0, g)));
     }
 #undef RT_OLD
 #undef RT_MG
@@ -553,8 +596,16 @@ static cudaError_t launch_tma_ho(const SweepLaunch &L, dim3 grid, cudaStream_t s
     constexpr int smem = kW * StageGeom<CW, G, R, D>::kWarpBytes;
     if (smem > 227 * 1024) return cudaErrorInvalidValue;
     auto kern = k_sweep_tma<CW, G, R, MODE, D, V, kW, HO>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    // the shared-memory opt-in is per kernel and device: set once, not on every launch
+    static bool opted_in[64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || !opted_in[dev]) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < 64) opted_in[dev] = true;
+    }
     kern<<<grid, dim3(32 * kW), smem, st>>>(L);
     return cudaGetLastError();
 }
@@ -573,7 +624,7 @@ static cudaError_t launch_tma(const SweepLaunch &L, dim3 grid, cudaStream_t st)
 template <int CW, int G, int R, int MODE, int D>
 static cudaError_t launch_variant(const SweepLaunch &L, dim3 grid, cudaStream_t st)
 {
-    if constexpr (MODE == MODE_J) {
+    if constexpr (MODE == MODE_J || MODE == MODE_OWNERS) {
         if (L.pair) return launch_tma<CW, G, R, MODE, D, 2>(L, grid, st);
     } else {
         if (L.pair) return cudaErrorInvalidValue;
@@ -588,7 +639,9 @@ static cudaError_t launch_rows(const SweepLaunch &L, cudaStream_t st)
     const dim3 grid(L.nitems, 1, L.nbins);
     if (L.mode == MODE_COUNT) return launch_variant<CW, G, R, MODE_COUNT, 2>(L, grid, st);   // diagnostics: depth 2
     if (L.mode == MODE_DS)    return launch_variant<CW, G, R, MODE_DS, 2>(L, grid, st);
+    if (L.mode == MODE_OWNERS) return launch_variant<CW, G, R, MODE_OWNERS, 2>(L, grid, st);
     switch (L.stages) {
+    case 4:  if constexpr (CW * G <= 2) return launch_variant<CW, G, R, MODE_J, 4>(L, grid, st); else return cudaErrorInvalidValue;   // rows of <= 64 cells
     case 3:  return launch_variant<CW, G, R, MODE_J, 3>(L, grid, st);
     default: return launch_variant<CW, G, R, MODE_J, 2>(L, grid, st);
     }
@@ -624,6 +677,7 @@ template <int CW, int G, int R>
 static int ctas_per_sm_rows(int stages, bool pair)
 {
     switch (stages) {
+    case 4:  if constexpr (CW * G <= 2) return ctas_per_sm_one<CW, G, R, 4>(pair); else return 0;
     case 3:  return ctas_per_sm_one<CW, G, R, 3>(pair);
     default: return ctas_per_sm_one<CW, G, R, 2>(pair);
     }

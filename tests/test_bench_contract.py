@@ -43,19 +43,52 @@ import pytest  # noqa: E402
 def test_gpu_arm_prints_the_contract_line():
     """The line the driver parses: metric, whole-job value, e2e with host copies, roofline, cpu_baseline, clocks,
     launch count (small config so that it runs in seconds)."""
-    d = _run_bench("--config", "C2", "--steps", "3", "--warmup", "3", "--cpu-dirs", "8")
+    d = _run_bench("--config", "C2", "--steps", "3", "--warmup", "3", "--cpu-dirs", "24", "--no-all-configs")
     assert d["metric"] == "ray_segment_updates_per_sec" and d["unit"] == "updates/s" and d["n_gpus"] == 1
     assert d["steps"] == 3 and d["warmup"] >= 3 and d["higher_is_better"] is True and d["dtype"] == "f32"
     assert d["value"] > 0 and d["ms_per_step"] > 0 and d["vs_baseline"] is None and d["data"] == "synthetic"
-    assert d["gpu_launches"] > 0 and "workload" in d["config"]
+    assert d["gpu_launches"] > 0 and "workload" in d["config"] and "configs" not in d
+    assert "flushed" in d["config"]["l2"] or "larger than L2" in d["config"]["l2"]      # the bench says how it timed it
     e = d["e2e"]
     assert 0 < e["value"] <= d["value"] * 1.05 and e["h2d_bytes_per_step"] == 2 * 4 * 64 ** 3 and e["d2h_bytes_per_step"] == 4 * 64 ** 3
+    assert e["h2d_ms"] > 0 and e["pack_ms"] > 0 and e["sweep_ms"] > 0 and e["d2h_ms"] > 0 and e["kernel_ms"] > 0
+    assert abs(e["h2d_ms"] + e["pack_ms"] + e["sweep_ms"] + e["d2h_ms"] - e["ms_per_step"]) < 0.05 * e["ms_per_step"]
     r = d["roofline"]
-    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and r["peak"] > 1000 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
+    assert r["bound"] == "l2" and r["unit"] == "GB/s" and r["peak"] > 5000 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
     assert 0.5 < r["kernel_share_of_step"] < 1.2
+    assert d["peaks"]["l2_read_gbs"] > d["peaks"]["hbm_gbs"] > 1000
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["sample"]
+    assert c["single_thread"]["cores"] == 1 and c["single_thread"]["value"] > 0
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+
+
+@pytest.mark.gpu
+def test_default_line_carries_all_five_configs():
+    """The driver's own command (default config C4) with fewer steps: one JSON line with the headline on C4 and a
+    `configs` record for C1 ... C5 (report for every config)."""
+    d = _run_bench("--steps", "3", "--warmup", "3", "--cpu-dirs", "16")
+    assert d["config"]["workload"].startswith("C4") and d["roofline"]["bound"] == "hbm" and "larger than L2" in d["config"]["l2"]
+    assert sorted(d["configs"]) == ["C1", "C2", "C3", "C4", "C5"]
+    for name, c in d["configs"].items():
+        assert c["value"] > 0 and c["ms_per_step"] > 0 and c["e2e"]["value"] > 0 and c["model_frac"] > 0
+        assert c["bound"] == ("hbm" if name in ("C4", "C5") else "l2")
+    assert d["configs"]["C4"]["ms_per_step"] == d["ms_per_step"]
+    t = d["roofline"]
+    assert t["traffic_table"] == "ok" or t["traffic"] is None        # never a stale ncu figure
+
+
+def test_traffic_table_names_the_kernel_sources():
+    """profiles/dram_traffic.json ties the ncu-measured DRAM bytes to the git blob hashes of the kernel sources;
+    bench.py drops `traffic` when a source has changed since the capture."""
+    sys.path.insert(0, ROOT)
+    import bench
+    t = json.load(open(bench.TRAFFIC_TABLE))
+    assert set(t["kernel_sources"]) == set(bench.KERNEL_SOURCES)
+    for name, e in t["entries"].items():
+        assert name in ("C1", "C2", "C3", "C4", "C5") and e["bytes_per_cell_dir_bin"] > 0 and os.path.exists(os.path.join(ROOT, e["source"]))
+    entries, state = bench.traffic_table()
+    assert state == "ok" or (state.startswith("stale") and entries == {})
 
 
 @pytest.mark.gpu

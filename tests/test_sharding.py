@@ -82,3 +82,50 @@ def test_two_gloo_ranks_reproduce_the_full_sweep(orc, tmp_path):
     j1 = np.load(tmp_path / "jin_1.npy")
     assert np.array_equal(j0, j1)                                  # identical on every rank
     assert np.abs(j0 / ref - 1).max() < 1e-12
+
+
+def _nccl_rank_main(rank, world, port, tmpdir):
+    import torch
+    import torch.distributed as dist
+    import paper_1410_0763_b200 as rt
+    from rt_inputs import make_fields
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    torch.cuda.set_device(rank)
+    dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", rank))
+    try:
+        dims = (64, 32, 48)
+        kap, S = make_fields("C3", dims=dims)
+        dirs = rt.healpix_dirs(4)
+        tr = rt.RayTracer(dims, 1, dirs[rt.shard_directions(dirs, world, rank)])
+        try:
+            tr.set_fields(torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda())
+            Jin = rt.sweep_sharded(tr, len(dirs), what=rt.RT_J_IN).cpu().numpy()
+        finally:
+            tr.close()
+        np.save(os.path.join(tmpdir, "nccl_jin_%d.npy" % rank), Jin)
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+def test_two_nccl_ranks_sweep_sharded(orc, tmp_path):
+    """sweep_sharded under NCCL on two devices of one node (one process per GPU): every rank sweeps its share with
+    RT_SUM_IN, one all-reduce, rt_combine -> J_in of the whole set on both ranks.  Skipped with fewer than two GPUs."""
+    import torch
+    import torch.multiprocessing as mp
+    if not torch.cuda.is_available() or torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    from rt_inputs import make_fields
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    mp.spawn(_nccl_rank_main, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    kap, S = make_fields("C3", dims=(64, 32, 48))
+    ref = orc.sweep(kap, S, orc.healpix_dirs(4), want_counts=False)["Jin"]
+    j0 = np.load(tmp_path / "nccl_jin_0.npy")
+    j1 = np.load(tmp_path / "nccl_jin_1.npy")
+    assert np.array_equal(j0, j1)
+    floor = 1e-30 * np.abs(ref).max()
+    assert (np.abs(j0 - ref) / np.maximum(np.abs(ref), floor)).max() <= 1e-5
