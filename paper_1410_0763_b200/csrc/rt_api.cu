@@ -99,7 +99,8 @@ struct rt_ctx {
     // overlapped schedule (small meshes): every class of directions (layout, dominant axis, pairs / singles, march
     // sense along b) has its own slot range and runs on its own internal stream ("lane"), so that the classes of a
     // sweep that does not fill the machine run side by side instead of one short launch after the other
-    struct ClassPlan { int l, pair, off, count, rev, Nc, tiles, slot_base, nslots; };
+    struct ClassPlan { int l, pair, off, count, rev, Nc, tiles, slot_base, nslots, cap; };
+    int wave_div = 0;                // overlapped schedule: work items per launch = one wave of resident CTAs / wave_div (0 = default)
     std::vector<ClassPlan> plan;
     int overlap = -1;                // rt_tune "overlap": -1 = automatic, 0 = off, 1 = on
     bool overlap_on = false;
@@ -354,6 +355,7 @@ extern "C" int rt_tune(rt_ctx *c, const char *key, int value)
     if (!strcmp(key, "handoff")) { if ((value != 0 && value != 1) || (value && c->stages != 2 && c->stages != 0)) return RT_EINVAL; c->handoff = value; if (value) c->stages = 2; return RT_OK; }
     if (!strcmp(key, "pair")) { if (value != 0 && value != 1) return RT_EINVAL; c->pair_enable = value != 0; return RT_OK; }
     if (!strcmp(key, "overlap")) { if (value < -1 || value > 1) return RT_EINVAL; c->overlap = value; return RT_OK; }
+    if (!strcmp(key, "wave_div")) { if (value < 1 || value > 16) return RT_EINVAL; c->wave_div = value; return RT_OK; }
     if (!strcmp(key, "graph")) { if (value < -1 || value > 1) return RT_EINVAL; c->graph = value; return RT_OK; }
     if (!strcmp(key, "rows")) { if (!(value == 1 || value == 2 || value == 4)) return RT_EINVAL; c->rows = value; return RT_OK; }
     return RT_EINVAL;
@@ -421,7 +423,13 @@ static bool build_overlap_plan(const rt_ctx *c, std::vector<rt_ctx::ClassPlan> &
                 p.l = l; p.pair = passes[ps].pair; p.off = passes[ps].off + i; p.count = n; p.rev = rev; p.Nc = Nc;
                 p.tiles = (Nc + kOwnedWarpsPerCta * rows - 1) / (kOwnedWarpsPerCta * rows);
                 p.slot_base = need[l];
-                p.nslots = std::max(1, std::min(n, passes[ps].S));
+                // launches of one wave / wave_div work items; a launch that starts anywhere touches at most
+                // (cap - 1) / tiles + 2 entries, each of which needs a slot of its own
+                const int wave = passes[ps].pair ? c->cap_pair[l] : c->cap_single[l];
+                const int div = c->wave_div > 0 ? c->wave_div : kOverlapWaveDiv;
+                p.cap = std::max(p.tiles, (wave > 0 ? wave : n * p.tiles) / div);
+                p.nslots = std::max(1, std::min(n, (p.cap - 1) / p.tiles + 2));
+                if (p.nslots >= n) p.cap = n * p.tiles;          // every entry has its own slot: one launch
                 need[l] += p.nslots;
                 *items += (long long)n * p.tiles * c->nbins;
                 plan.push_back(p);
@@ -722,45 +730,57 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
 // Overlapped J sweep (ensure_buffers decided c->overlap_on): the classes run on the context's lanes, forked from
 // and joined back into `st` with events.  Every class owns its slot range and its first nslots entries start from
 // zero ("fresh"), so no slot accumulator is cleared; the sparsely written seam accumulators are.
-static int run_overlapped(rt_ctx *c, cudaStream_t st, int *launches, int used[2], bool record_events)
+static int run_overlapped(rt_ctx *c, cudaStream_t st, int *launches, int used[2], bool record_events,
+                          OwnerStats *own = nullptr)
 {
     const int nbins = c->nbins;
+    const int mode = own ? MODE_OWNERS : MODE_J;           // writer-count check: same launches, one after the other on st
     for (int l = 0; l < 2; ++l) {
         used[l] = 0;
         for (const auto &p : c->plan) if (p.l == l) used[l] = std::max(used[l], p.slot_base + p.nslots);
         if (used[l] > 0) CK(cudaMemsetAsync(c->d_accC[l], 0, sizeof(float) * (size_t)c->ncell_l[l] * nbins * used[l], st));
     }
     if (record_events) CK(cudaEventRecord(c->ev0, st));
-    CK(cudaEventRecord(c->ev_fork, st));
+    if (!own) CK(cudaEventRecord(c->ev_fork, st));
     bool lane_used[rt_ctx::kLanes] = {};
     int idx = 0;
     for (const auto &p : c->plan) {
         const int ln = idx++ % rt_ctx::kLanes;
-        cudaStream_t ls = c->lane[ln];
-        if (!lane_used[ln]) { CK(cudaStreamWaitEvent(ls, c->ev_fork, 0)); lane_used[ln] = true; }
+        cudaStream_t ls = own ? st : c->lane[ln];
+        if (!own && !lane_used[ln]) { CK(cudaStreamWaitEvent(ls, c->ev_fork, 0)); lane_used[ln] = true; }
         const int l = p.l;
         SweepLaunch L;
         memset(&L, 0, sizeof(L));
         const size_t slot_stride = (size_t)c->ncell_l[l] * nbins;
         L.P = c->d_P[l]; L.acc = c->d_acc[l] + slot_stride * p.slot_base; L.accC = c->d_accC[l] + slot_stride * p.slot_base;
         L.dirs = c->d_dirs; L.prog = c->d_prog; L.nbins = nbins; L.ncell = c->ncell_l[l]; L.Ibc = c->d_Ibc;
-        L.rows = rows_for(c, l); L.mode = MODE_J; L.stages = stages_for(c, l); L.handoff = 0;
+        L.rows = rows_for(c, l); L.mode = mode; L.stages = stages_for(c, l); L.handoff = 0;
         L.Nb = c->pitch[l]; L.pp = c->pp[l]; L.pair = p.pair; L.rev = p.rev; L.Nc = p.Nc; L.tiles = p.tiles;
         L.batch = c->d_batch + p.off;
         L.nslots = p.nslots;
         L.fresh_below = p.nslots;
-        int cap = p.pair ? c->cap_pair[l] : c->cap_single[l];
-        if (cap < 1) cap = p.nslots * p.tiles;
-        else if (cap % p.tiles == 0) cap = std::max(p.tiles, std::min(cap, p.nslots * p.tiles));
-        else cap = std::max(p.tiles, std::min(cap, (p.nslots - 1) * p.tiles));
-        if (p.nslots == 1) cap = p.tiles;
-        if (p.nslots >= p.count) cap = p.count * p.tiles;           // every entry has its own slot: one launch
+        const int cap = p.cap;
         const long long total = (long long)p.count * p.tiles;
+        const size_t nacc = slot_stride * p.nslots;
         for (long long item0 = 0; item0 < total; item0 += cap) {
             L.item0 = (int)item0;
             L.nitems = (int)std::min<long long>(cap, total - item0);
+            if (own) {                                       // writer counts of this launch alone
+                CK(cudaMemsetAsync(L.acc, 0, sizeof(float) * nacc, ls));
+                CK(cudaMemsetAsync(L.accC, 0, sizeof(float) * nacc, ls));
+            }
             CK(launch_sweep_owned(L, ls));
             ++*launches;
+            if (own) {
+                CK(launch_owner_reduce(c->d_own, L.acc, (long long)nacc, ls));
+                CK(launch_owner_reduce(c->d_own + 2, L.accC, (long long)nacc, ls));
+                own->launches += 1;
+                if (L.item0 % p.tiles != 0 || (L.item0 + L.nitems) % p.tiles != 0) own->partial += 1;
+            }
+        }
+        if (own) {
+            own->entries += (unsigned long long)p.count;
+            own->expected += (unsigned long long)p.count * (unsigned long long)slot_stride;
         }
     }
     for (int ln = 0; ln < rt_ctx::kLanes; ++ln)
@@ -967,7 +987,8 @@ extern "C" int rt_debug_writer_counts(rt_ctx *c, unsigned long long *out_host, v
     CK(cudaMemsetAsync(c->d_own, 0, sizeof(unsigned long long) * 4, st));
     OwnerStats own;
     int launches = 0, used[2];
-    rc = run_traversal(c, MODE_OWNERS, -1, c->nbins, st, &launches, used, &own);
+    rc = c->overlap_on ? run_overlapped(c, st, &launches, used, false, &own)
+                       : run_traversal(c, MODE_OWNERS, -1, c->nbins, st, &launches, used, &own);
     if (rc != RT_OK) return rc;
     unsigned long long dev[4];
     CK(cudaMemcpyAsync(dev, c->d_own, sizeof(dev), cudaMemcpyDeviceToHost, st));

@@ -8,6 +8,7 @@ namespace rt {
 
 constexpr int kF = 20;                         // slope quantisation: 2^-20 (reading A4)
 constexpr long long kOne = 1ll << kF;
+constexpr float kEx2Bias = 4.0e-8f;           // relative correction of ex2.approx (rt_sweep.cuh one_minus_exp)
 constexpr float kKappaMin = 8.673617379884035e-19f;   // 2^-60: kappa floor in the packed copy (reading A7)
 
 // Slab program: the traversal of ONE slab for ALL rays of a direction (identical because lattice
@@ -89,6 +90,7 @@ cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat,
 bool owned_supported(int Nb, int Nc, int rows);
 int owned_ctas_per_sm(int Nb, int rows, int stages, bool pair);
 constexpr int kOwnedWarpsPerCta = 4;
+constexpr int kOverlapWaveDiv = 2;             // overlapped schedule: launches of 1 / kOverlapWaveDiv of a wave (rt_api.cu)
 constexpr int kShortRowStages = 2;             // TMA ring depth for rows of <= 64 cells (rt_api.cu stages_for)
 cudaError_t launch_sweep_owned(const SweepLaunch &L, cudaStream_t st);
 cudaError_t launch_sweep_generic(const SweepLaunch &L, int max_lattice_b, int max_lattice_c, cudaStream_t st);

@@ -188,11 +188,14 @@ __device__ __forceinline__ float ex2_approx(float x)
 __device__ __forceinline__ float one_minus_exp(float kap, float len, float ct, float &e)
 {
     const float x = kap * len;
-    e = ex2_approx(kap * ct);                                  // ct = -len*log2(e)
+    const float em = ex2_approx(kap * ct);                     // ct = -len*log2(e)
     float p = fmaf(x, -0.0377338513f, 0.1660640817f);          // x * poly(x) on [0, 1/4], rel. error 3.4e-7
     p = fmaf(x, p, -0.4999701648f);
     p = fmaf(x, p, 0.9999997683f);
-    return x < 0.25f ? x * p : 1.0f - e;
+    const float ec = fmaf(em, kEx2Bias, em);                   // ex2.approx is biased low (rt_sweep.cuh)
+    const float A = x < 0.25f ? x * p : 1.0f - ec;
+    e = x < 0.25f ? 1.0f - A : ec;                             // thin pieces: e consistent with A
+    return A;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -310,8 +313,25 @@ template <bool COUNTS> __device__ __forceinline__ typename std::conditional<COUN
 template <> __device__ __forceinline__ unsigned long long widen<true>(float v) { return (unsigned long long)__float2uint_rn(v); }
 template <> __device__ __forceinline__ double widen<false>(float v) { return (double)v; }
 
+// sum over the slots of (slot accumulator + seam accumulator) of one cell, four independent partial sums so that the
+// loads of several slots are in flight together (a 32^3 mesh is all latency here)
 template <bool COUNTS>
-__global__ void k_finalise(float *__restrict__ J, unsigned *__restrict__ counts, const float2 *__restrict__ Pnat, int ppN,
+__device__ __forceinline__ typename std::conditional<COUNTS, unsigned long long, double>::type
+sum_slots(const float *__restrict__ acc, const float *__restrict__ accC, int slots, size_t stride, size_t i)
+{
+    typename std::conditional<COUNTS, unsigned long long, double>::type s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+    int sl = 0;
+    for (; sl + 1 < slots; sl += 2) {
+        const float a0 = acc[sl * stride + i], c0 = accC[sl * stride + i];
+        const float a1 = acc[(sl + 1) * stride + i], c1 = accC[(sl + 1) * stride + i];
+        s0 += widen<COUNTS>(a0); s1 += widen<COUNTS>(c0); s2 += widen<COUNTS>(a1); s3 += widen<COUNTS>(c1);
+    }
+    if (sl < slots) { s0 += widen<COUNTS>(acc[sl * stride + i]); s1 += widen<COUNTS>(accC[sl * stride + i]); }
+    return (s0 + s1) + (s2 + s3);
+}
+
+template <bool COUNTS>
+__global__ void __launch_bounds__(1024) k_finalise(float *__restrict__ J, unsigned *__restrict__ counts, const float2 *__restrict__ Pnat, int ppN,
                            const float *__restrict__ accN, const float *__restrict__ accNC, int slotsN,
                            const float *__restrict__ accT, const float *__restrict__ accTC, int slotsT,
                            int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, int add_S, int zb0)
@@ -333,7 +353,7 @@ __global__ void k_finalise(float *__restrict__ J, unsigned *__restrict__ counts,
         SumT s = 0;
         if (x < nx && y < ny) {
             const size_t i = (size_t)bin * ncellT + ((size_t)x * nz + z) * nyp + y;
-            for (int sl = 0; sl < slotsT; ++sl) s += widen<COUNTS>(accT[sl * strideT + i]) + widen<COUNTS>(accTC[sl * strideT + i]);
+            s = sum_slots<COUNTS>(accT, accTC, slotsT, strideT, i);
         }
         tile[dx][threadIdx.x] = s;
     }
@@ -343,8 +363,7 @@ __global__ void k_finalise(float *__restrict__ J, unsigned *__restrict__ counts,
         if (x < nx && y < ny) {
             const size_t i = (size_t)bin * ncell + ((size_t)z * ny + y) * nx + x;
             const size_t ip = (size_t)bin * ncellN + ((size_t)z * ny + y) * nxp + x;
-            SumT s = tile[threadIdx.x][dy];
-            for (int sl = 0; sl < slotsN; ++sl) s += widen<COUNTS>(accN[sl * strideN + ip]) + widen<COUNTS>(accNC[sl * strideN + ip]);
+            const SumT s = tile[threadIdx.x][dy] + sum_slots<COUNTS>(accN, accNC, slotsN, strideN, ip);
             if (COUNTS) {
                 counts[i] = (unsigned)s;
             } else {
@@ -364,7 +383,7 @@ cudaError_t launch_normalise(float *J, const float2 *Pnat, int ppN, const float 
 {
     const long long planes = (long long)nz * nbins;
     for (long long zb0 = 0; zb0 < planes; zb0 += kMaxGridZ) {
-        dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, planes - zb0)), block(32, 8);
+        dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, planes - zb0)), block(32, 32);
         k_finalise<false><<<grid, block, 0, st>>>(J, nullptr, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT,
                                                   nx, ny, nz, nxp, nyp, nbins, inv_nd, add_S, (int)zb0);
         const cudaError_t e = cudaGetLastError();
@@ -399,7 +418,7 @@ __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, con
             double s = 0.0;
             if (x < nx && y < ny) {
                 const size_t i = (size_t)bin * ncellT + ((size_t)x * nz + z) * nyp + y;
-                for (int sl = 0; sl < slotsT; ++sl) s += (double)accT[sl * strideT + i] + (double)accTC[sl * strideT + i];
+                s = sum_slots<false>(accT, accTC, slotsT, strideT, i);
             }
             tile[dx][threadIdx.x] = s;
         }
@@ -409,8 +428,7 @@ __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, con
             const int x = x0 + threadIdx.x, y = y0 + dy;
             if (x < nx && y < ny) {
                 const size_t i = (size_t)bin * ncellN + ((size_t)z * ny + y) * nxp + x;
-                double s = tile[threadIdx.x][dy];
-                for (int sl = 0; sl < slotsN; ++sl) s += (double)accN[sl * strideN + i] + (double)accNC[sl * strideN + i];
+                const double s = tile[threadIdx.x][dy] + sum_slots<false>(accN, accNC, slotsN, strideN, i);
                 const size_t o = field_index(i, ppN);
                 const float kap = fN[o], src = fN[o + field_s_offset(ppN)];
                 const float jin = (float)(s * (double)inv_nd) / kap;
@@ -623,7 +641,7 @@ cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const fl
                                    int nx, int ny, int nz, int nxp, int nyp, cudaStream_t st)
 {
     for (long long zb0 = 0; zb0 < nz; zb0 += kMaxGridZ) {
-        dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, nz - zb0)), block(32, 8);
+        dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, nz - zb0)), block(32, 32);
         k_finalise<true><<<grid, block, 0, st>>>(nullptr, counts, nullptr, 0, accN, accNC, slotsN, accT, accTC, slotsT,
                                                  nx, ny, nz, nxp, nyp, 1, 1.0f, 0, (int)zb0);
         const cudaError_t e = cudaGetLastError();

@@ -84,53 +84,33 @@ __device__ __forceinline__ void unpack(const float4 &v, float2 &kap, float2 &src
 // Segment update (eq. 7, eq. 8), fp32
 //   A = 1 - exp(-kappa*len); contribution to the cell += I_in * A  (numerator of eq. 11 times kappa*L,
 //   see DESIGN.md "Arithmetic"); I_out = I_in * e + S * A with e = exp(-kappa*len).
-// e and A each keep a small RELATIVE error: e straight from ex2 (never as 1 - A: behind an opaque
-// cell the transmitted part I*e is all that is left), A from a polynomial where 1 - e would cancel.
+// e and A each keep a small RELATIVE error: behind an opaque cell the transmitted part I*e is all that is left, so
+// there e comes straight from ex2 (bias-corrected) and A = 1 - e; on thin pieces 1 - e would cancel, so A comes from
+// a polynomial and e = 1 - A.
 // With t = kappa * ct, ct = -len*log2(e):  e = 2^t,  x = kappa*len = -t*ln2, and for x < 1/4
 //   A = x (c0 + c1 x + c2 x^2 + c3 x^3)  (fitted on [0, 1/4], rel. error 3.4e-7)
 //     = t (d0 + d1 t + d2 t^2 + d3 t^3),  d_k = c_k (-ln 2)^(k+1).
 // ------------------------------------------------------------------------------------------------
-#ifndef RT_EXPVAR
-#define RT_EXPVAR 0
-#endif
-__device__ __forceinline__ float  vexact_e(float t) { return exp2f(t); }
-__device__ __forceinline__ float2 vexact_e(float2 t) { return make_float2(exp2f(t.x), exp2f(t.y)); }
-__device__ __forceinline__ float  vexact_A(float t) { return -expm1f(t * 0.6931471805599453f); }
-__device__ __forceinline__ float2 vexact_A(float2 t) { return make_float2(-expm1f(t.x * 0.6931471805599453f), -expm1f(t.y * 0.6931471805599453f)); }
 template <class T>
 __device__ __forceinline__ T one_minus_exp(T kap, T ctv, T &e)
 {
+    constexpr float thr = -0.36067376022224085f;                   // x < 1/4
     const T t = vmul(kap, ctv);
-#if RT_EXPVAR & 8
-    e = vexact_e(t);
-    return vexact_A(t);
-#else
-    e = vex2(t);
-#if RT_EXPVAR & 4
-    constexpr float thr = -0.7213475204444817f;
-    T p = vfma(t, vsplat<T>(-0.0010833843844011426f), vsplat<T>(-0.009464533999562263f));
-    p = vfma(t, p, vsplat<T>(-0.05546464025974274f));
-    p = vfma(t, p, vsplat<T>(-0.24022290110588074f));
-    p = vfma(t, p, vsplat<T>(-0.6931471228599548f));
-#elif RT_EXPVAR & 2
-    constexpr float thr = -0.36067376022224085f;
-    T p = vfma(t, vsplat<T>(-0.0012016557157039642f), vsplat<T>(-0.009577106684446335f));
-    p = vfma(t, p, vsplat<T>(-0.05549883097410202f));
-    p = vfma(t, p, vsplat<T>(-0.24022626876831055f));
-    p = vfma(t, p, vsplat<T>(-0.6931471824645996f));
-#else
-    constexpr float thr = -0.36067376022224085f;
+    const T em = vex2(t);
     T p = vfma(t, vsplat<T>(-0.00871029682457447f), vsplat<T>(-0.055303432047367096f));
     p = vfma(t, p, vsplat<T>(-0.24021217226982117f));
     p = vfma(t, p, vsplat<T>(-0.6931470036506653f));
-#endif
     const T As = vmul(t, p);
-    const T Ab = vfma(e, vsplat<T>(-1.0f), vsplat<T>(1.0f));       // 1 - e, one rounding
-#if RT_EXPVAR & 1
-    e = vsel_gt(t, thr, vfma(As, vsplat<T>(-1.0f), vsplat<T>(1.0f)), e);
-#endif
-    return vsel_gt(t, thr, As, Ab);
-#endif
+    // MUFU.EX2 is biased low (measured on B200: mean -0.3 ... -0.6 ulp, -2e-8 ... -5e-8 relative); over the ~200
+    // pieces of a ray through 60 optical depths that is the -5e-6 the deep-shadow cells of C3 were off by
+    const T ec = vfma(em, vsplat<T>(kEx2Bias), em);
+    const T Ab = vfma(ec, vsplat<T>(-1.0f), vsplat<T>(1.0f));      // 1 - e, one rounding
+    const T A = vsel_gt(t, thr, As, Ab);
+    // e consistent with A, without a second select: on thick pieces Ab - A = 0 exactly and e = ec; on thin pieces
+    // ec >= 1/2, so Ab = 1 - ec exactly and ec + (Ab - As) = RN(1 - As).  A thin medium is then in exact equilibrium
+    // at I = S (e + A = 1 to one rounding) instead of drifting by (e + A - 1) / A per piece.
+    e = vadd(ec, vadd(Ab, vmul(A, vsplat<T>(-1.0f))));
+    return A;
 }
 
 // Store of a finished accumulator chunk: the one writer of these cells in this launch and array.  In MODE_OWNERS
@@ -435,7 +415,9 @@ k_sweep_tma(const SweepLaunch L)
     constexpr bool REV = (V == 1);
     extern __shared__ __align__(128) unsigned char smem_raw[];
 
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    // warp index through a shuffle from lane 0: provably warp-uniform for the compiler, so that the address arithmetic of
+    // the bulk copies (issued by one lane) runs on the uniform datapath instead of being moved there value by value
+    const int lane = threadIdx.x & 31, wid = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     // A launch is a range of work items (entry, row tile) of a list of entries (directions or mirror pairs)
     // that need not end on an entry boundary, so that every launch fills all resident CTA slots.  An entry's
     // accumulators are those of slot = entry mod nslots; nslots exceeds the entries a launch can touch.
@@ -492,6 +474,8 @@ k_sweep_tma(const SweepLaunch L)
     }
     RowState ps;
     ps.init(q0, sub_offset(Dp->sub, 1));
+    // (Tried: lane r issuing the copies of ray row r, so that the R + 1 addresses are computed side by side. It removes
+    // a third of the instructions of this block and changes nothing measurable: the block is not what the slab waits for.)
     auto produce = [&](int s) {
         if (lane == 0) {
             const unsigned st = wbase_s + s * SG::kStage, bar = bars + 8 * s;
