@@ -100,6 +100,8 @@ struct rt_ctx {
     // sense along b) has its own slot range and runs on its own internal stream ("lane"), so that the classes of a
     // sweep that does not fill the machine run side by side instead of one short launch after the other
     struct ClassPlan { int l, pair, off, count, rev, Nc, tiles, slot_base, nslots, cap; };
+    int binpack = -1;                // rt_tune "binpack": -1 = automatic, 0 = bins are planes (one CTA per bin), 1 = three bins per row
+    int nbp = 1;                     // bins packed per row of the packed fields and accumulators (1 or 3), fixed by ensure_buffers
     int wave_div = 0;                // overlapped schedule: work items per launch = one wave of resident CTAs / wave_div (0 = default)
     std::vector<ClassPlan> plan;
     int overlap = -1;                // rt_tune "overlap": -1 = automatic, 0 = off, 1 = on
@@ -355,6 +357,7 @@ extern "C" int rt_tune(rt_ctx *c, const char *key, int value)
     if (!strcmp(key, "handoff")) { if ((value != 0 && value != 1) || (value && c->stages != 2 && c->stages != 0)) return RT_EINVAL; c->handoff = value; if (value) c->stages = 2; return RT_OK; }
     if (!strcmp(key, "pair")) { if (value != 0 && value != 1) return RT_EINVAL; c->pair_enable = value != 0; return RT_OK; }
     if (!strcmp(key, "overlap")) { if (value < -1 || value > 1) return RT_EINVAL; c->overlap = value; return RT_OK; }
+    if (!strcmp(key, "binpack")) { if (value < -1 || value > 1) return RT_EINVAL; c->binpack = value; return RT_OK; }
     if (!strcmp(key, "wave_div")) { if (value < 1 || value > 16) return RT_EINVAL; c->wave_div = value; return RT_OK; }
     if (!strcmp(key, "graph")) { if (value < -1 || value > 1) return RT_EINVAL; c->graph = value; return RT_OK; }
     if (!strcmp(key, "rows")) { if (!(value == 1 || value == 2 || value == 4)) return RT_EINVAL; c->rows = value; return RT_OK; }
@@ -369,6 +372,7 @@ static int rows_for(const rt_ctx *c, int layout)
     int r = c->rows > 0 ? c->rows : (c->pitch[layout] == 128 ? 4 : (c->pitch[layout] <= 64 ? 1 : 2));
     if (c->pitch[layout] == 512) r = 1;                       // 512-cell rows: one ray row per warp fills the registers
     if (r == 4 && c->pitch[layout] > 128) r = 2;            // four rows per warp only fit the registers for rows of <= 128 cells
+    if (c->nbp == 3) r = c->rows > 0 ? std::min(c->rows, 2) : (c->pitch[layout] == 128 ? kPackedRows128 : 1);   // three bins per row
     for (int i : c->order[layout])
         while (r > 1 && c->hd[i].Nc % r != 0) r >>= 1;
     return r;
@@ -416,7 +420,7 @@ static bool build_overlap_plan(const rt_ctx *c, std::vector<rt_ctx::ClassPlan> &
             int i = 0;
             while (i < nl) {
                 const int a = c->hd[list[i]].a, rev = eff_rev(list[i]), Nc = c->hd[list[i]].Nc;
-                if (!owned_supported(c->pitch[l], Nc, rows)) return false;
+                if (!owned_supported(c->pitch[l], Nc, rows, c->nbp)) return false;
                 int n = 0;
                 while (i + n < nl && c->hd[list[i + n]].a == a && eff_rev(list[i + n]) == rev) ++n;
                 rt_ctx::ClassPlan p;
@@ -431,7 +435,7 @@ static bool build_overlap_plan(const rt_ctx *c, std::vector<rt_ctx::ClassPlan> &
                 p.nslots = std::max(1, std::min(n, (p.cap - 1) / p.tiles + 2));
                 if (p.nslots >= n) p.cap = n * p.tiles;          // every entry has its own slot: one launch
                 need[l] += p.nslots;
-                *items += (long long)n * p.tiles * c->nbins;
+                *items += (long long)n * p.tiles * (c->nbins / c->nbp);
                 plan.push_back(p);
                 i += n;
             }
@@ -443,6 +447,15 @@ static bool build_overlap_plan(const rt_ctx *c, std::vector<rt_ctx::ClassPlan> &
 static int ensure_buffers(rt_ctx *c)
 {
     if (c->buffers_ready) return RT_OK;
+    // multi-bin packed rows: three bins of a cell row share the row (packed kernel), if every layout can run it
+    c->nbp = 1;
+    if (c->flags == RT_OWNED && c->nbins % 3 == 0 && !c->handoff && (c->stages == 0 || c->stages == 2) &&
+        (c->binpack == 1 || (c->binpack == -1 && kBinpackDefault))) {
+        bool ok = true;
+        for (int l = 0; l < 2; ++l)
+            if (!c->order[l].empty() && !(c->fast[l] && c->pitch[l] <= 128)) ok = false;
+        if (ok) c->nbp = 3;
+    }
     const size_t field_bytes_l[2] = {sizeof(float2) * (size_t)c->ncell_l[0] * c->nbins, sizeof(float2) * (size_t)c->ncell_l[1] * c->nbins};
     const size_t acc_bytes_l[2] = {sizeof(float) * (size_t)c->ncell_l[0] * c->nbins, sizeof(float) * (size_t)c->ncell_l[1] * c->nbins};
     size_t freeb = 0, totalb = 0;
@@ -459,14 +472,15 @@ static int ensure_buffers(rt_ctx *c)
                 int Nc = c->hd[c->order[l][0]].Nc;
                 for (int i : c->order[l]) Nc = std::min(Nc, c->hd[i].Nc);
                 const int rows = rows_for(c, l);
-                const int ctas_dir = ((Nc / rows + kOwnedWarpsPerCta - 1) / kOwnedWarpsPerCta) * c->nbins;
+                const int zgroups = c->nbins / c->nbp;               // grid.z of a J launch
+                const int ctas_dir = ((Nc / rows + kOwnedWarpsPerCta - 1) / kOwnedWarpsPerCta) * zgroups;
                 // A launch is one wave of resident CTAs, whole wave: `cap` work items (entry, row tile), not
                 // rounded to whole entries; the entries of a launch cycle through cap / tiles + 2 slots.
                 auto wave = [&](bool pair, int *cap) {
-                    int per_sm = c->fast[l] ? owned_ctas_per_sm(c->pitch[l], rows, stages_for(c, l), pair) : 0;
+                    int per_sm = c->fast[l] ? owned_ctas_per_sm(c->pitch[l], rows, stages_for(c, l), pair, c->nbp) : 0;
                     if (per_sm < 1) per_sm = 4;
                     const int resident = per_sm * c->sm_count;
-                    *cap = std::max(1, resident / std::max(1, c->nbins));
+                    *cap = std::max(1, resident / std::max(1, zgroups));
                     // (a wave that is a whole number of entries needs no spare slots: launches then end on entry boundaries)
                     return std::max(1, std::min(nd, resident / std::max(1, ctas_dir) + ((resident % std::max(1, ctas_dir)) ? 2 : 0)));
                 };
@@ -493,7 +507,7 @@ static int ensure_buffers(rt_ctx *c)
         long long items = 0;
         if (build_overlap_plan(c, plan, need, &items)) {
             long long capacity = 0;
-            for (int l = 0; l < 2; ++l) capacity = std::max<long long>(capacity, (long long)std::max(c->cap_pair[l], c->cap_single[l]) * c->nbins);
+            for (int l = 0; l < 2; ++l) capacity = std::max<long long>(capacity, (long long)std::max(c->cap_pair[l], c->cap_single[l]) * (c->nbins / c->nbp));
             const size_t budget = freeb / 3, need_fixed = field_bytes_l[0] + field_bytes_l[1];
             const size_t need_acc = 2 * (need[0] * acc_bytes_l[0] + need[1] * acc_bytes_l[1]);
             const bool fits = budget > need_fixed && need_acc <= budget - need_fixed;
@@ -553,7 +567,7 @@ extern "C" int rt_set_fields(rt_ctx *c, const float *kappa_dev, const float *S_d
     int rc = ensure_buffers(c);
     if (rc != RT_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    CK(launch_pack_fields(kappa_dev, S_dev, c->d_P[0], c->d_P[1], c->pp[0], c->pp[1], c->nx, c->ny, c->nz, c->pitch[0], c->pitch[1], c->nbins, st));
+    CK(launch_pack_fields(kappa_dev, S_dev, c->d_P[0], c->d_P[1], c->pp[0], c->pp[1], c->nx, c->ny, c->nz, c->pitch[0], c->pitch[1], c->nbins, c->nbp, st));
     c->fields_set = true;
     return RT_OK;
 }
@@ -617,6 +631,7 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
         L.dirs = c->d_dirs; L.prog = c->d_prog; L.nbins = nbins; L.ncell = c->ncell_l[l]; L.Ibc = c->d_Ibc;
         L.rows = rows_for(c, l); L.mode = mode; L.stages = stages_for(c, l); L.handoff = c->handoff;
         L.Nb = c->pitch[l]; L.pp = c->pp[l];
+        L.nbp = (nbins == c->nbins) ? c->nbp : 1;            // the counting modes run with one bin on plain rows
         const bool owned_l = c->fast[l];
         // the lists this traversal walks: (direction list, position in d_batch, slots per launch, paired)
         struct Pass { const std::vector<int> *list; int off; int S; int pair; };
@@ -643,7 +658,7 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
                 const int a = c->hd[list[i]].a;
                 const int rev = eff_rev(list[i]);
                 // owned kernel, full sweep: the batch is the whole class; it is cut into launches of work items below
-                const bool whole = owned_l && only_dir < 0 && owned_supported(L.Nb, c->hd[list[i]].Nc, L.rows);
+                const bool whole = owned_l && only_dir < 0 && owned_supported(L.Nb, c->hd[list[i]].Nc, L.rows, L.nbp);
                 int n = 0;
                 while (i + n < nl && (whole || n < S) && c->hd[list[i + n]].a == a && eff_rev(list[i + n]) == rev) ++n;
                 int first = i, count = n;
@@ -664,7 +679,7 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
                 L.nslots = count;
                 L.rev = rev;
                 L.Nc = c->hd[list[first]].Nc;
-                if (owned_l && owned_supported(L.Nb, L.Nc, L.rows)) {
+                if (owned_l && owned_supported(L.Nb, L.Nc, L.rows, L.nbp)) {
                     const int tiles = (L.Nc + kOwnedWarpsPerCta * L.rows - 1) / (kOwnedWarpsPerCta * L.rows);
                     L.tiles = tiles;
                     if (only_dir >= 0) {
@@ -755,7 +770,7 @@ static int run_overlapped(rt_ctx *c, cudaStream_t st, int *launches, int used[2]
         L.P = c->d_P[l]; L.acc = c->d_acc[l] + slot_stride * p.slot_base; L.accC = c->d_accC[l] + slot_stride * p.slot_base;
         L.dirs = c->d_dirs; L.prog = c->d_prog; L.nbins = nbins; L.ncell = c->ncell_l[l]; L.Ibc = c->d_Ibc;
         L.rows = rows_for(c, l); L.mode = mode; L.stages = stages_for(c, l); L.handoff = 0;
-        L.Nb = c->pitch[l]; L.pp = c->pp[l]; L.pair = p.pair; L.rev = p.rev; L.Nc = p.Nc; L.tiles = p.tiles;
+        L.Nb = c->pitch[l]; L.pp = c->pp[l]; L.nbp = c->nbp; L.pair = p.pair; L.rev = p.rev; L.Nc = p.Nc; L.tiles = p.tiles;
         L.batch = c->d_batch + p.off;
         L.nslots = p.nslots;
         L.fresh_below = p.nslots;
@@ -801,7 +816,7 @@ static int enqueue_sweep(rt_ctx *c, float *J_dev, unsigned what, cudaStream_t st
                            : run_traversal(c, MODE_J, -1, c->nbins, st, &launches, used, nullptr, record_events);
     if (rc != RT_OK) return rc;
     CK(launch_normalise(J_dev, c->d_P[0], c->pp[0], c->d_acc[0], c->d_accC[0], used[0], c->d_acc[1], c->d_accC[1], used[1],
-                        c->nx, c->ny, c->nz, c->pitch[0], c->pitch[1], c->nbins, what == RT_SUM_IN ? 1.0f : (float)(1.0 / (double)c->ndirs),
+                        c->nx, c->ny, c->nz, c->pitch[0], c->pitch[1], c->nbins, c->nbp, what == RT_SUM_IN ? 1.0f : (float)(1.0 / (double)c->ndirs),
                         what == RT_J_TOTAL ? 1 : 0, st));
     c->last_launches = launches + 1;
     return RT_OK;
@@ -859,7 +874,7 @@ extern "C" int rt_combine(rt_ctx *c, const float *sum_dev, long long ndirs_total
     if (!c || !sum_dev || !J_dev || ndirs_total < 1 || what > 1u) return RT_EINVAL;
     DevGuard dev_guard(c->device);
     if (!c->fields_set) return RT_ESTATE;
-    CK(launch_combine(J_dev, sum_dev, c->d_P[0], c->pp[0], (size_t)c->ncell * c->nbins, c->nx, c->pitch[0], (float)(1.0 / (double)ndirs_total),
+    CK(launch_combine(J_dev, sum_dev, c->d_P[0], c->pp[0], c->nx, c->ny, c->nz, c->pitch[0], c->nbins, c->nbp, (float)(1.0 / (double)ndirs_total),
                       what == RT_J_TOTAL ? 1 : 0, (cudaStream_t)stream));
     return RT_OK;
 }
@@ -880,10 +895,11 @@ extern "C" int rt_sweep_rates(rt_ctx *c, float *Gamma_dev, float *Heat_dev, cons
     cudaStream_t st = (cudaStream_t)stream;
     int launches = 0;
     int used[2];
-    int rc = run_traversal(c, MODE_J, -1, c->nbins, st, &launches, used);
+    int rc = c->overlap_on ? run_overlapped(c, st, &launches, used, true)
+                           : run_traversal(c, MODE_J, -1, c->nbins, st, &launches, used);
     if (rc != RT_OK) return rc;
     CK(launch_rates(Gamma_dev, Heat_dev, c->d_P[0], c->pp[0], c->d_acc[0], c->d_accC[0], used[0], c->d_acc[1], c->d_accC[1],
-                    used[1], c->nx, c->ny, c->nz, c->pitch[0], c->pitch[1], c->nbins, (float)(1.0 / (double)c->ndirs), w4.data(), st));
+                    used[1], c->nx, c->ny, c->nz, c->pitch[0], c->pitch[1], c->nbins, c->nbp, (float)(1.0 / (double)c->ndirs), w4.data(), st));
     c->last_launches = launches + 1;
     return RT_OK;
 }
@@ -945,7 +961,7 @@ extern "C" int rt_point_sources(rt_ctx *c, const int *src_fix_host, const double
     const float *d_lum = reinterpret_cast<const float *>(c->d_src + sizeof(int) * 3 * (size_t)nsrc);
     if (steps_host) CK(cudaMemsetAsync(c->d_u64, 0, sizeof(unsigned long long), st));
     CK(launch_point_sources(Q_dev, tau_dev, c->d_P[0], c->pp[0], c->nx, c->ny, c->nz, c->pitch[0], d_src, d_lum, nsrc,
-                            c->nbins, (float)c->cell_width, diag_src, diag_bin, steps_host ? c->d_u64 : nullptr, st));
+                            c->nbins, c->nbp, (float)c->cell_width, diag_src, diag_bin, steps_host ? c->d_u64 : nullptr, st));
     c->last_launches = 1;
     if (steps_host) {                                            // the one synchronising variant: the count comes back to the host
         CK(cudaMemcpyAsync(steps_host, c->d_u64, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
@@ -1067,7 +1083,7 @@ extern "C" int rt_direction_records(rt_ctx *c, long long *rec, double *L_host)
         rec[6 * i + 1] = h.refl[0] | (h.refl[1] << 1) | (h.refl[2] << 2);
         rec[6 * i + 2] = h.Mb;
         rec[6 * i + 3] = h.Mc;
-        rec[6 * i + 4] = (c->fast[h.layout] && owned_supported(c->pitch[h.layout], h.Nc, rows_for(c, h.layout))) ? 0 : 1;
+        rec[6 * i + 4] = (c->fast[h.layout] && owned_supported(c->pitch[h.layout], h.Nc, rows_for(c, h.layout), c->nbp)) ? 0 : 1;
         rec[6 * i + 5] = c->rays;
         if (L_host) L_host[i] = h.L;
     }

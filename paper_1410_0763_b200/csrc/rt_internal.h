@@ -72,6 +72,7 @@ struct SweepLaunch {
     int pair;                // owned TMA kernel, MODE_J: every slot carries a direction and its b-mirror (rt_kernels.cu "mirror pairs")
     int pp;                  // P is pair-packed (below)
     int handoff;             // owned kernel: seam partials are handed to the next warp of the CTA in shared memory (ablation)
+    int nbp;                 // bins packed per row of P / acc / accC (1: bins are planes; 3: packed_cell below, packed kernel)
 };
 
 // Packed-field layouts.  Interleaved: float2 (kappa, S) per cell.  Pair-packed (layouts swept by the
@@ -82,28 +83,38 @@ struct SweepLaunch {
 __host__ __device__ __forceinline__ size_t field_index(size_t o, int pp) { return pp ? 4 * (o >> 1) + (o & 1) : 2 * o; }
 __host__ __device__ __forceinline__ int field_s_offset(int pp) { return pp ? 2 : 1; }
 
+// Offset (in cells) of (bin, row, column) in a packed field or accumulator of one layout.  nbp = 1: bins are planes
+// [bin][row][column].  nbp > 1 (multi-bin packed loads): groups of nbp bins share a row, [group][row][bin in group][column],
+// so that one bulk copy of a row feeds nbp intensity recurrences.  rows = rows per bin of the layout, pitch = padded row width.
+__host__ __device__ __forceinline__ size_t packed_cell(int bin, size_t row, int col, int nbp, int pitch, size_t rows)
+{
+    return (((size_t)(bin / nbp) * rows + row) * nbp + (size_t)(bin % nbp)) * pitch + col;
+}
+
 // launchers (rt_kernels.cu); all return cudaError_t of the launch
 cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, int max_na, SlabProg *prog, double cell_width,
                                   const double *Lvals, cudaStream_t st);
 cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat, float2 *PT, int ppN, int ppT,
-                               int nx, int ny, int nz, int nxp, int nyp, int nbins, cudaStream_t st);
-bool owned_supported(int Nb, int Nc, int rows);
-int owned_ctas_per_sm(int Nb, int rows, int stages, bool pair);
+                               int nx, int ny, int nz, int nxp, int nyp, int nbins, int nbp, cudaStream_t st);
+bool owned_supported(int Nb, int Nc, int rows, int nbp = 1);
+int owned_ctas_per_sm(int Nb, int rows, int stages, bool pair, int nbp = 1);
 constexpr int kOwnedWarpsPerCta = 4;
+constexpr bool kBinpackDefault = false;        // three bins per row by default when eligible (rt_api.cu ensure_buffers)
+constexpr int kPackedRows128 = 1;              // ray rows per warp of the packed kernel on 128-cell rows
 constexpr int kOverlapWaveDiv = 2;             // overlapped schedule: launches of 1 / kOverlapWaveDiv of a wave (rt_api.cu)
 constexpr int kShortRowStages = 2;             // TMA ring depth for rows of <= 64 cells (rt_api.cu stages_for)
 cudaError_t launch_sweep_owned(const SweepLaunch &L, cudaStream_t st);
 cudaError_t launch_sweep_generic(const SweepLaunch &L, int max_lattice_b, int max_lattice_c, cudaStream_t st);
 cudaError_t launch_normalise(float *J, const float2 *Pnat, int ppN, const float *accN, const float *accNC, int slotsN,
                              const float *accT, const float *accTC, int slotsT,
-                             int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, int add_S, cudaStream_t st);
+                             int nx, int ny, int nz, int nxp, int nyp, int nbins, int nbp, float inv_nd, int add_S, cudaStream_t st);
 cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN, const float *accN, const float *accNC,
                          int slotsN, const float *accT, const float *accTC, int slotsT, int nx, int ny, int nz,
-                         int nxp, int nyp, int nbins, float inv_nd, const float *w4, cudaStream_t st);
-cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int ppN, size_t n, int nx, int nxp,
-                           float inv_nd, int add_S, cudaStream_t st);
+                         int nxp, int nyp, int nbins, int nbp, float inv_nd, const float *w4, cudaStream_t st);
+cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int ppN, int nx, int ny, int nz, int nxp,
+                           int nbins, int nbp, float inv_nd, int add_S, cudaStream_t st);
 cudaError_t launch_point_sources(float *Q, float *tau_out, const float2 *Pnat, int ppN, int nx, int ny, int nz, int nxp,
-                                 const int *src_dev, const float *lum_dev, int nsrc, int nbins, float cell_width,
+                                 const int *src_dev, const float *lum_dev, int nsrc, int nbins, int nbp, float cell_width,
                                  int diag_src, int diag_bin, unsigned long long *steps_dev, cudaStream_t st);
 cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const float *accNC, int slotsN,
                                    const float *accT, const float *accTC, int slotsT,

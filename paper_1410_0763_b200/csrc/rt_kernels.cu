@@ -84,7 +84,7 @@ cudaError_t launch_build_programs(const DirDev *dirs, int ndirs, int max_na, Sla
 // ------------------------------------------------------------------------------------------------
 __global__ void k_pack_fields(const float *__restrict__ kappa, const float *__restrict__ S,
                               float2 *__restrict__ Pnat, float2 *__restrict__ PT, int ppN, int ppT, int nx, int ny, int nz,
-                              int nxp, int nyp, int zb0)
+                              int nxp, int nyp, int nbp, int zb0)
 {
     float *__restrict__ fN = reinterpret_cast<float *>(Pnat);
     float *__restrict__ fT = reinterpret_cast<float *>(PT);
@@ -95,14 +95,14 @@ __global__ void k_pack_fields(const float *__restrict__ kappa, const float *__re
     const size_t ncell = (size_t)nx * ny * nz;
     const size_t boff = (size_t)bin * ncell;
     // rows of the packed copies have pitch nxp / nyp >= nx / ny (pad cells stay zero: kappa = 0 and S = 0
-    // leave a ray unchanged and add nothing to an accumulator)
-    const size_t boffN = (size_t)bin * nxp * ny * nz, boffT = (size_t)bin * nyp * nz * nx;
+    // leave a ray unchanged and add nothing to an accumulator); bins are planes or packed per row (packed_cell)
+    const size_t rowsN = (size_t)ny * nz, rowsT = (size_t)nz * nx;
     for (int dy = threadIdx.y; dy < 32; dy += blockDim.y) {
         int x = x0 + threadIdx.x, y = y0 + dy;
         if (x < nx && y < ny) {
             size_t i = boff + ((size_t)z * ny + y) * nx + x;
             float2 v = make_float2(fmaxf(kappa[i], kKappaMin), S[i]);
-            const size_t o = field_index(boffN + ((size_t)z * ny + y) * nxp + x, ppN);
+            const size_t o = field_index(packed_cell(bin, (size_t)z * ny + y, x, nbp, nxp, rowsN), ppN);
             fN[o] = v.x; fN[o + field_s_offset(ppN)] = v.y;
             tile[dy][threadIdx.x] = v;
         }
@@ -112,19 +112,19 @@ __global__ void k_pack_fields(const float *__restrict__ kappa, const float *__re
         int x = x0 + dx, y = y0 + threadIdx.x;
         if (x < nx && y < ny) {
             const float2 v = tile[threadIdx.x][dx];
-            const size_t o = field_index(boffT + ((size_t)x * nz + z) * nyp + y, ppT);
+            const size_t o = field_index(packed_cell(bin, (size_t)x * nz + z, y, nbp, nyp, rowsT), ppT);
             fT[o] = v.x; fT[o + field_s_offset(ppT)] = v.y;
         }
     }
 }
 
 cudaError_t launch_pack_fields(const float *kappa, const float *S, float2 *Pnat, float2 *PT, int ppN, int ppT,
-                               int nx, int ny, int nz, int nxp, int nyp, int nbins, cudaStream_t st)
+                               int nx, int ny, int nz, int nxp, int nyp, int nbins, int nbp, cudaStream_t st)
 {
     const long long planes = (long long)nz * nbins;
     for (long long zb0 = 0; zb0 < planes; zb0 += kMaxGridZ) {
         dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, planes - zb0)), block(32, 8);
-        k_pack_fields<<<grid, block, 0, st>>>(kappa, S, Pnat, PT, ppN, ppT, nx, ny, nz, nxp, nyp, (int)zb0);
+        k_pack_fields<<<grid, block, 0, st>>>(kappa, S, Pnat, PT, ppN, ppT, nx, ny, nz, nxp, nyp, nbp, (int)zb0);
         const cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
@@ -144,9 +144,18 @@ int ctas_per_sm_nb64(int rows, int stages, bool pair);
 int ctas_per_sm_nb128(int rows, int stages, bool pair);
 int ctas_per_sm_nb256(int rows, int stages, bool pair);
 int ctas_per_sm_nb512(int rows, int stages, bool pair);
+// three bins packed per row (rt_sweep_nb*x3.cu)
+cudaError_t launch_sweep_nb32x3(const SweepLaunch &L, cudaStream_t st);
+cudaError_t launch_sweep_nb64x3(const SweepLaunch &L, cudaStream_t st);
+cudaError_t launch_sweep_nb128x3(const SweepLaunch &L, cudaStream_t st);
+int ctas_per_sm_nb32x3(int rows, bool pair);
+int ctas_per_sm_nb64x3(int rows, bool pair);
+int ctas_per_sm_nb128x3(int rows, bool pair);
 
-bool owned_supported(int Nb, int Nc, int rows)
+bool owned_supported(int Nb, int Nc, int rows, int nbp)
 {
+    if (nbp == 3) return (Nb == 32 || Nb == 64 || Nb == 128) && (rows == 1 || rows == 2) && Nc % rows == 0;
+    if (nbp != 1) return false;
     if (!(Nb == 32 || Nb == 64 || Nb == 128 || Nb == 256 || Nb == 512)) return false;
     if (Nb == 512 && rows != 1) return false;
     if (!(rows == 1 || rows == 2 || (rows == 4 && Nb <= 128))) return false;
@@ -154,8 +163,16 @@ bool owned_supported(int Nb, int Nc, int rows)
 }
 
 // resident CTAs (of kOwnedWarpsPerCta warps) per SM of the J-mode owned kernel; 0 if it cannot launch
-int owned_ctas_per_sm(int Nb, int rows, int stages, bool pair)
+int owned_ctas_per_sm(int Nb, int rows, int stages, bool pair, int nbp)
 {
+    if (nbp == 3) {
+        switch (Nb) {
+        case 32:  return ctas_per_sm_nb32x3(rows, pair);
+        case 64:  return ctas_per_sm_nb64x3(rows, pair);
+        case 128: return ctas_per_sm_nb128x3(rows, pair);
+        }
+        return 0;
+    }
     switch (Nb) {
     case 32:  return ctas_per_sm_nb32(rows, stages, pair);
     case 64:  return ctas_per_sm_nb64(rows, stages, pair);
@@ -168,6 +185,14 @@ int owned_ctas_per_sm(int Nb, int rows, int stages, bool pair)
 
 cudaError_t launch_sweep_owned(const SweepLaunch &L, cudaStream_t st)
 {
+    if (L.nbp == 3 && L.nbins % 3 == 0) {                  // counting modes run with one bin on plain rows
+        switch (L.Nb) {
+        case 32:  return launch_sweep_nb32x3(L, st);
+        case 64:  return launch_sweep_nb64x3(L, st);
+        case 128: return launch_sweep_nb128x3(L, st);
+        }
+        return cudaErrorInvalidValue;
+    }
     switch (L.Nb) {
     case 32:  return launch_sweep_nb32(L, st);
     case 64:  return launch_sweep_nb64(L, st);
@@ -334,7 +359,7 @@ template <bool COUNTS>
 __global__ void __launch_bounds__(1024) k_finalise(float *__restrict__ J, unsigned *__restrict__ counts, const float2 *__restrict__ Pnat, int ppN,
                            const float *__restrict__ accN, const float *__restrict__ accNC, int slotsN,
                            const float *__restrict__ accT, const float *__restrict__ accTC, int slotsT,
-                           int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, int add_S, int zb0)
+                           int nx, int ny, int nz, int nxp, int nyp, int nbins, int nbp, float inv_nd, int add_S, int zb0)
 {
     using SumT = typename std::conditional<COUNTS, unsigned long long, double>::type;
     __shared__ SumT tile[32][33];
@@ -352,7 +377,7 @@ __global__ void __launch_bounds__(1024) k_finalise(float *__restrict__ J, unsign
         const int x = x0 + dx, y = y0 + threadIdx.x;
         SumT s = 0;
         if (x < nx && y < ny) {
-            const size_t i = (size_t)bin * ncellT + ((size_t)x * nz + z) * nyp + y;
+            const size_t i = packed_cell(bin, (size_t)x * nz + z, y, nbp, nyp, (size_t)nz * nx);
             s = sum_slots<COUNTS>(accT, accTC, slotsT, strideT, i);
         }
         tile[dx][threadIdx.x] = s;
@@ -362,7 +387,7 @@ __global__ void __launch_bounds__(1024) k_finalise(float *__restrict__ J, unsign
         const int x = x0 + threadIdx.x, y = y0 + dy;
         if (x < nx && y < ny) {
             const size_t i = (size_t)bin * ncell + ((size_t)z * ny + y) * nx + x;
-            const size_t ip = (size_t)bin * ncellN + ((size_t)z * ny + y) * nxp + x;
+            const size_t ip = packed_cell(bin, (size_t)z * ny + y, x, nbp, nxp, (size_t)ny * nz);
             const SumT s = tile[threadIdx.x][dy] + sum_slots<COUNTS>(accN, accNC, slotsN, strideN, ip);
             if (COUNTS) {
                 counts[i] = (unsigned)s;
@@ -379,13 +404,13 @@ __global__ void __launch_bounds__(1024) k_finalise(float *__restrict__ J, unsign
 
 cudaError_t launch_normalise(float *J, const float2 *Pnat, int ppN, const float *accN, const float *accNC, int slotsN,
                              const float *accT, const float *accTC, int slotsT,
-                             int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, int add_S, cudaStream_t st)
+                             int nx, int ny, int nz, int nxp, int nyp, int nbins, int nbp, float inv_nd, int add_S, cudaStream_t st)
 {
     const long long planes = (long long)nz * nbins;
     for (long long zb0 = 0; zb0 < planes; zb0 += kMaxGridZ) {
         dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, planes - zb0)), block(32, 32);
         k_finalise<false><<<grid, block, 0, st>>>(J, nullptr, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT,
-                                                  nx, ny, nz, nxp, nyp, nbins, inv_nd, add_S, (int)zb0);
+                                                  nx, ny, nz, nxp, nyp, nbins, nbp, inv_nd, add_S, (int)zb0);
         const cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
@@ -402,7 +427,7 @@ struct RateWeights { float wG[16], lG[16], wH[16], lH[16]; };
 __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, const float2 *__restrict__ Pnat, int ppN,
                         const float *__restrict__ accN, const float *__restrict__ accNC, int slotsN,
                         const float *__restrict__ accT, const float *__restrict__ accTC, int slotsT,
-                        int nx, int ny, int nz, int nxp, int nyp, int nbins, float inv_nd, const RateWeights W, int z0)
+                        int nx, int ny, int nz, int nxp, int nyp, int nbins, int nbp, float inv_nd, const RateWeights W, int z0)
 {
     __shared__ double tile[32][33];
     const int z = (int)blockIdx.z + z0;
@@ -417,7 +442,7 @@ __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, con
             const int x = x0 + dx, y = y0 + threadIdx.x;
             double s = 0.0;
             if (x < nx && y < ny) {
-                const size_t i = (size_t)bin * ncellT + ((size_t)x * nz + z) * nyp + y;
+                const size_t i = packed_cell(bin, (size_t)x * nz + z, y, nbp, nyp, (size_t)nz * nx);
                 s = sum_slots<false>(accT, accTC, slotsT, strideT, i);
             }
             tile[dx][threadIdx.x] = s;
@@ -427,7 +452,7 @@ __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, con
         for (int dy = threadIdx.y; dy < 32; dy += blockDim.y, ++j) {
             const int x = x0 + threadIdx.x, y = y0 + dy;
             if (x < nx && y < ny) {
-                const size_t i = (size_t)bin * ncellN + ((size_t)z * ny + y) * nxp + x;
+                const size_t i = packed_cell(bin, (size_t)z * ny + y, x, nbp, nxp, (size_t)ny * nz);
                 const double s = tile[threadIdx.x][dy] + sum_slots<false>(accN, accNC, slotsN, strideN, i);
                 const size_t o = field_index(i, ppN);
                 const float kap = fN[o], src = fN[o + field_s_offset(ppN)];
@@ -451,7 +476,7 @@ __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, con
 
 cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN, const float *accN, const float *accNC,
                          int slotsN, const float *accT, const float *accTC, int slotsT, int nx, int ny, int nz,
-                         int nxp, int nyp, int nbins,
+                         int nxp, int nyp, int nbins, int nbp,
                          float inv_nd, const float *w4 /* host: wG, lG, wH, lH, each [nbins] */, cudaStream_t st)
 {
     RateWeights W;
@@ -463,7 +488,7 @@ cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN,
     for (long long z0 = 0; z0 < nz; z0 += kMaxGridZ) {
         dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, nz - z0)), block(32, 8);
         k_rates<<<grid, block, 0, st>>>(Gamma, Heat, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT, nx, ny, nz, nxp, nyp,
-                                       nbins, inv_nd, W, (int)z0);
+                                       nbins, nbp, inv_nd, W, (int)z0);
         const cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
@@ -475,23 +500,28 @@ cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN,
 // shards have been added (all-reduce); J_in = sum / N_d (eq. 13), J = J_in + S (eq. 12).
 // ------------------------------------------------------------------------------------------------
 __global__ void k_combine(float *__restrict__ J, const float *__restrict__ sum, const float2 *__restrict__ Pnat, int ppN,
-                          size_t n, int nx, int nxp, float inv_nd, int add_S)
+                          size_t n, int nx, int ny, int nz, int nxp, int nbp, float inv_nd, int add_S)
 {
     const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
+    const size_t rows = (size_t)ny * nz;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         float v = sum[i] * inv_nd;
-        const size_t ip = (i / nx) * nxp + (i % nx);              // rows of the packed copy have pitch nxp
-        if (add_S) v += fN[field_index(ip, ppN) + field_s_offset(ppN)];
+        if (add_S) {
+            const size_t r = i / nx;                               // (bin, z, y) of the caller's [nbins][nz][ny][nx] array
+            const size_t ip = packed_cell((int)(r / rows), r % rows, (int)(i % nx), nbp, nxp, rows);
+            v += fN[field_index(ip, ppN) + field_s_offset(ppN)];
+        }
         J[i] = v;
     }
 }
 
-cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int ppN, size_t n, int nx, int nxp,
-                           float inv_nd, int add_S, cudaStream_t st)
+cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int ppN, int nx, int ny, int nz, int nxp,
+                           int nbins, int nbp, float inv_nd, int add_S, cudaStream_t st)
 {
+    const size_t n = (size_t)nx * ny * nz * nbins;
     size_t blocks = (n + 255) / 256;
     if (blocks > 148 * 16) blocks = 148 * 16;
-    k_combine<<<(unsigned)blocks, 256, 0, st>>>(J, sum, Pnat, ppN, n, nx, nxp, inv_nd, add_S);
+    k_combine<<<(unsigned)blocks, 256, 0, st>>>(J, sum, Pnat, ppN, n, nx, ny, nz, nxp, nbp, inv_nd, add_S);
     return cudaGetLastError();
 }
 
@@ -534,22 +564,25 @@ template <class TT>
 __global__ void __launch_bounds__(128)
 k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2 *__restrict__ Pnat, int ppN,
                 int nx, int ny, int nz, int nxp, const int *__restrict__ src, const float *__restrict__ lum, int nsrc,
-                int nbins, float cell_width, int diag_src, int diag_bin, unsigned long long *__restrict__ steps)
+                int nbins, int nbp, float cell_width, int diag_src, int diag_bin, unsigned long long *__restrict__ steps)
 {
     const int bin = blockIdx.z;
     const long long ncell = (long long)nx * ny * nz;
     const long long cidx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const bool live = cidx < ncell;
     const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
-    const size_t boffN = (size_t)bin * nxp * ny * nz;
+    // this bin's cells in the packed native copy: cell (row, x) at boffN + row * rowp + x (packed_cell: bins are planes,
+    // or nbp bins share a row)
+    const size_t boffN = packed_cell(bin, 0, 0, nbp, nxp, (size_t)ny * nz);
+    const int rowp = nxp * nbp;
     unsigned nstep = 0;
     if (live) {
         const int tgt[3] = {(int)(cidx % nx), (int)((cidx / nx) % ny), (int)(cidx / ((long long)nx * ny))};
-        const float kap_t = fN[field_index(boffN + ((size_t)tgt[2] * ny + tgt[1]) * nxp + tgt[0], ppN)];
-        const float *__restrict__ fbin = fN + 2 * boffN;          // this bin's plane of the packed copy (boffN is even: nxp is)
+        const float kap_t = fN[field_index(boffN + ((size_t)tgt[2] * ny + tgt[1]) * rowp + tgt[0], ppN)];
+        const float *__restrict__ fbin = fN + 2 * boffN;          // this bin's cells of the packed copy (boffN is even: nxp is)
         double q = 0.0;
         // linear index of a cell in the packed native copy (row pitch nxp) and its change per step along an axis
-        const int idx_t = (tgt[2] * ny + tgt[1]) * nxp + tgt[0];
+        const int idx_t = (tgt[2] * ny + tgt[1]) * rowp + tgt[0];
         const TT kInf = PsInf<TT>::v();
         for (int a = 0; a < nsrc; ++a) {
             long long s[3], d[3], ad[3];
@@ -567,8 +600,8 @@ k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2
                 if (s[i] % kPsFix == 0 && stp[i] < 0) c -= 1;     // a source on a boundary belongs to the cell the ray moves into
                 cur[i] = c;
             }
-            int idx = (cur[2] * ny + cur[1]) * nxp + cur[0];
-            const int didx[3] = {stp[0], stp[1] * nxp, stp[2] * nxp * ny};
+            int idx = (cur[2] * ny + cur[1]) * rowp + cur[0];
+            const int didx[3] = {stp[0], stp[1] * rowp, stp[2] * rowp * ny};
             // common denominator over the moving axes; T_i = n_i * prod_{j != i} |d_j|
             const long long f0 = ad[0] ? ad[0] : 1, f1 = ad[1] ? ad[1] : 1, f2 = ad[2] ? ad[2] : 1;
             const long long W[3] = {f1 * f2, f0 * f2, f0 * f1};
@@ -622,16 +655,16 @@ k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2
 }
 
 cudaError_t launch_point_sources(float *Q, float *tau_out, const float2 *Pnat, int ppN, int nx, int ny, int nz, int nxp,
-                                 const int *src_dev, const float *lum_dev, int nsrc, int nbins, float cell_width,
+                                 const int *src_dev, const float *lum_dev, int nsrc, int nbins, int nbp, float cell_width,
                                  int diag_src, int diag_bin, unsigned long long *steps_dev, cudaStream_t st)
 {
     const long long ncell = (long long)nx * ny * nz;
     dim3 grid((unsigned)((ncell + 127) / 128), 1, nbins);
     if (nx <= 512 && ny <= 512 && nz <= 512)
-        k_point_sources<double><<<grid, 128, 0, st>>>(Q, tau_out, Pnat, ppN, nx, ny, nz, nxp, src_dev, lum_dev, nsrc, nbins, cell_width,
+        k_point_sources<double><<<grid, 128, 0, st>>>(Q, tau_out, Pnat, ppN, nx, ny, nz, nxp, src_dev, lum_dev, nsrc, nbins, nbp, cell_width,
                                                       diag_src, diag_bin, steps_dev);
     else
-        k_point_sources<long long><<<grid, 128, 0, st>>>(Q, tau_out, Pnat, ppN, nx, ny, nz, nxp, src_dev, lum_dev, nsrc, nbins, cell_width,
+        k_point_sources<long long><<<grid, 128, 0, st>>>(Q, tau_out, Pnat, ppN, nx, ny, nz, nxp, src_dev, lum_dev, nsrc, nbins, nbp, cell_width,
                                                          diag_src, diag_bin, steps_dev);
     return cudaGetLastError();
 }
@@ -643,7 +676,7 @@ cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const fl
     for (long long zb0 = 0; zb0 < nz; zb0 += kMaxGridZ) {
         dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, nz - zb0)), block(32, 32);
         k_finalise<true><<<grid, block, 0, st>>>(nullptr, counts, nullptr, 0, accN, accNC, slotsN, accT, accTC, slotsT,
-                                                 nx, ny, nz, nxp, nyp, 1, 1.0f, 0, (int)zb0);
+                                                 nx, ny, nz, nxp, nyp, 1, 1, 1.0f, 0, (int)zb0);
         const cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }

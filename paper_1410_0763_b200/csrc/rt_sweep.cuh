@@ -195,11 +195,17 @@ struct Seam {
 //   I[r][g][d] : intensities of the rays currently in the CW columns of chunk g of ray row r,
 //             direction d; elements in MEMORY order.
 // ------------------------------------------------------------------------------------------------
-template <int CW, int G, int R, int MODE, int FLC, int V>
+//
+// Multi-bin packed rows (NB > 1; eqs. 22-23: independent bins sharing one geometry): a row holds
+// the NB bins of its cells one after the other, [bin][column], so the G chunks of a lane are GB = G / NB chunks per
+// bin; one bulk copy per row feeds all bins, and the slab program, the addresses, the barrier wait and the pattern
+// dispatch are shared.  Only the ray handoff along b knows about bins: its chunk-to-chunk carry starts anew, with
+// that bin's inflow, at every bin.
+template <int CW, int G, int R, int MODE, int FLC, int V, int NB>
 __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>::T (&I)[R][G][(V == 2) ? 2 : 1],
                                           const unsigned char *__restrict__ sp, unsigned char *__restrict__ sa,
                                           const float len0, const float len1, const float len2,
-                                          const float Ib0, const float Ib1, const float Ic, const float invL,
+                                          const float (&Ib0)[NB], const float (&Ib1)[NB], const float (&Ic)[NB], const float invL,
                                           const int lane, const int lwrap, const unsigned padmask,
                                           float *const (&rowp)[R + 1], const Seam &seam)
 {
@@ -207,6 +213,7 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
     using DV = typename VT<CW>::D;
     constexpr int ND = (V == 2) ? 2 : 1;
     constexpr bool REV = (V == 1);
+    constexpr int GB = G / NB;                  // chunks per bin
     constexpr int kRowP = 32 * CW * G * (int)sizeof(float2), kRowA = 32 * CW * G * (int)sizeof(float);
     constexpr unsigned FULL = 0xffffffffu;
     constexpr float LOG2E = 1.4426950408889634f;
@@ -215,7 +222,7 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
     const T invLv = vsplat<T>(invL);
     const bool anySC = (fl & (F_SC1 | F_SC2)) != 0;
     // memory chunk of canonical chunk g, as element offsets within a row
-#define RT_MG(g) ((REV ? (G - 1 - (g)) : (g)) * 32 * CW)
+#define RT_MG(g) ((((g) / GB) * GB + (REV ? (GB - 1 - (g) % GB) : (g) % GB)) * 32 * CW)
 #define RT_OLD(r, g) (*reinterpret_cast<T *>(sa + (r) * kRowA + RT_MG(g) * (int)sizeof(float)))
 
     T part_hi[G];                 // partial of memory row r + 1
@@ -252,9 +259,10 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
                         // direction 0: hand every ray to the owner of the next column in canonical order
                         // (canonical lane + 1 is always the physical lane + 1); a new ray enters at
                         // canonical column 0.  Within a chunk, memory element 0 is upstream unless REV.
-                        float carry = Ib0;               // inflow of the side face direction 0 enters through
+                        float carry = 0.0f;
 #pragma unroll
                         for (int g = 0; g < G; ++g) {
+                            if (g % GB == 0) carry = Ib0[g / GB];    // inflow of the side face direction 0 enters through
                             const float out = REV ? vfirst(Ir[g][0]) : vlast(Ir[g][0]);
                             const float t = __shfl_sync(FULL, out, (lane + 31) & 31);
                             const float in = (lane == 0) ? carry : t;
@@ -264,9 +272,9 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
                         }
                         if (ND == 2) {
                             // mirrored direction: towards lower columns; a new ray enters the last column
-                            carry = Ib1;                 // the mirror image enters through the opposite face
 #pragma unroll
                             for (int g = G - 1; g >= 0; --g) {
+                                if (g % GB == GB - 1) carry = Ib1[g / GB];   // the mirror image enters through the opposite face
                                 const float t = __shfl_sync(FULL, vfirst(Ir[g][ND - 1]), (lane + 1) & 31);
                                 const float in = (lane == 31) ? carry : t;
                                 carry = t;
@@ -279,7 +287,7 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
                         for (int g = 0; g < G; ++g)
 #pragma unroll
                             for (int d = 0; d < ND; ++d)           // pad columns hold rays that have yet to cross the b face
-                                Ir[g][d] = vpad(vsplat<T>(Ic), d == 0 ? Ib0 : Ib1, (padmask >> (g * CW)) & 3u);
+                                Ir[g][d] = vpad(vsplat<T>(Ic[g / GB]), d == 0 ? Ib0[g / GB] : Ib1[g / GB], (padmask >> ((g % GB) * CW)) & 3u);
                     }
                 }
                 if (fl & fsc) sel = true;
@@ -340,13 +348,13 @@ __device__ __forceinline__ void slab_rows(const unsigned fl_rt, typename VT<CW>:
 
 #define RT_DISPATCH_SLAB(fl, ...)                                                         \
     switch (fl) {                                                                         \
-    case kPatNone: slab_rows<CW, G, R, MODE, kPatNone, V>(__VA_ARGS__); break;            \
-    case kPatB:    slab_rows<CW, G, R, MODE, kPatB, V>(__VA_ARGS__); break;               \
-    case kPatC:    slab_rows<CW, G, R, MODE, kPatC, V>(__VA_ARGS__); break;               \
-    case kPatBC:   slab_rows<CW, G, R, MODE, kPatBC, V>(__VA_ARGS__); break;              \
-    case kPatCB:   slab_rows<CW, G, R, MODE, kPatCB, V>(__VA_ARGS__); break;              \
-    case kPatD:    slab_rows<CW, G, R, MODE, kPatD, V>(__VA_ARGS__); break;               \
-    default:       slab_rows<CW, G, R, MODE, -1, V>(__VA_ARGS__); break;                  \
+    case kPatNone: slab_rows<CW, G, R, MODE, kPatNone, V, NB>(__VA_ARGS__); break;        \
+    case kPatB:    slab_rows<CW, G, R, MODE, kPatB, V, NB>(__VA_ARGS__); break;           \
+    case kPatC:    slab_rows<CW, G, R, MODE, kPatC, V, NB>(__VA_ARGS__); break;           \
+    case kPatBC:   slab_rows<CW, G, R, MODE, kPatBC, V, NB>(__VA_ARGS__); break;          \
+    case kPatCB:   slab_rows<CW, G, R, MODE, kPatCB, V, NB>(__VA_ARGS__); break;          \
+    case kPatD:    slab_rows<CW, G, R, MODE, kPatD, V, NB>(__VA_ARGS__); break;           \
+    default:       slab_rows<CW, G, R, MODE, -1, V, NB>(__VA_ARGS__); break;              \
     }
 
 // ------------------------------------------------------------------------------------------------
@@ -405,10 +413,12 @@ struct StageGeom {
 // memory (its own unused seam-accumulator rows) instead of the seam accumulator in global memory:
 // only the CTA's last warp still reads and writes accC.  The producer may run two stepping slabs
 // ahead of its consumer; the consumer never waits unless it has caught up.
-template <int CW, int G, int R, int MODE, int D, int V, int W, bool HO>
+template <int CW, int G, int R, int MODE, int D, int V, int W, bool HO, int NB = 1>
 __global__ void __launch_bounds__(32 * W)
 k_sweep_tma(const SweepLaunch L)
 {
+    static_assert(G % NB == 0 && (NB == 1 || !HO), "NB bins per row; the seam handoff exists for single-bin rows only");
+    constexpr int GB = G / NB;
     using SG = StageGeom<CW, G, R, D>;
     using T = typename VT<CW>::T;
     constexpr int ND = (V == 2) ? 2 : 1;
@@ -423,21 +433,25 @@ k_sweep_tma(const SweepLaunch L)
     // accumulators are those of slot = entry mod nslots; nslots exceeds the entries a launch can touch.
     const int item = (int)blockIdx.x + L.item0;
     const int ent = item / L.tiles, tile = item - ent * L.tiles;
-    const int slot = ent % L.nslots, bin = blockIdx.z;
+    const int slot = ent % L.nslots, bin = blockIdx.z * NB;      // first bin of this CTA's group of NB packed bins
     const DirDev *__restrict__ Dp = L.dirs + L.batch[ent];
     const int Nc = Dp->Nc, Na = Dp->Na, Mc = Dp->Mc;
     const int q0c = tile * (W * R);                              // first ray row of the CTA (L.tiles of them cover Nc)
     const int nact = min(W, (Nc - q0c) / R);                     // warps of this CTA that own rows (Nc % R == 0)
     const int q0 = q0c + wid * R;
-    const int sk = (int)Dp->sk, sl = (int)Dp->sl;                // |offsets| < 2^31: checked by rt_create
+    const int sk = (int)Dp->sk * NB, sl = (int)Dp->sl * NB;      // |offsets| < 2^31: checked by rt_create (rows hold NB bins)
     const float invL = (MODE == MODE_J) ? Dp->invL : 1.0f;
     // inflow of the faces this slot's rays enter through (DirDev::layout carries the face indices)
-    const float *__restrict__ Ibin = L.Ibc + 6 * bin;
     const int fcs = Dp->layout;
-    const float Ia = Ibin[(fcs >> 8) & 7], Ib0 = Ibin[(fcs >> 12) & 7], Ib1 = Ibin[((fcs >> 12) & 7) ^ 1], Ic = Ibin[(fcs >> 16) & 7];
+    float Ia[NB], Ib0[NB], Ib1[NB], Ic[NB];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+        const float *__restrict__ Ibin = L.Ibc + 6 * (bin + b);
+        Ia[b] = Ibin[(fcs >> 8) & 7]; Ib0[b] = Ibin[(fcs >> 12) & 7]; Ib1[b] = Ibin[((fcs >> 12) & 7) ^ 1]; Ic[b] = Ibin[(fcs >> 16) & 7];
+    }
     const SlabProg *__restrict__ prog = L.prog + Dp->prog_off;
 
-    const long long foff = (long long)bin * L.ncell + Dp->base;
+    const long long foff = (long long)bin * L.ncell + Dp->base * NB;
     const float2 *__restrict__ P = L.P + foff;
     float *__restrict__ acc = L.acc + ((long long)slot * L.nbins) * L.ncell + foff;
     float *__restrict__ accC = L.accC + ((long long)slot * L.nbins) * L.ncell + foff;
@@ -503,17 +517,17 @@ k_sweep_tma(const SweepLaunch L)
     // it always holds that face's inflow: at the start and after a row wrap.
     unsigned padmask = 0;
 #pragma unroll
-    for (int g = 0; g < G; ++g)
+    for (int g = 0; g < GB; ++g)                                  // the same for every bin
 #pragma unroll
         for (int i = 0; i < CW; ++i)
-            if (CW * (REV ? 31 - lane : lane) + i + (REV ? (G - 1 - g) : g) * 32 * CW >= Dp->Nb) padmask |= 1u << (g * CW + i);
+            if (CW * (REV ? 31 - lane : lane) + i + (REV ? (GB - 1 - g) : g) * 32 * CW >= Dp->Nb) padmask |= 1u << (g * CW + i);
     T I[R][G][ND];
 #pragma unroll
     for (int r = 0; r < R; ++r)
 #pragma unroll
         for (int g = 0; g < G; ++g)
 #pragma unroll
-            for (int d = 0; d < ND; ++d) I[r][g][d] = vpad(vsplat<T>(Ia), d == 0 ? Ib0 : Ib1, (padmask >> (g * CW)) & 3u);
+            for (int d = 0; d < ND; ++d) I[r][g][d] = vpad(vsplat<T>(Ia[g / GB]), d == 0 ? Ib0[g / GB] : Ib1[g / GB], (padmask >> ((g % GB) * CW)) & 3u);
 
     // this lane's first memory column (canonical chunk 0 is memory chunk G-1 when REV)
     const int lcol = CW * (REV ? 31 - lane : lane);
@@ -574,12 +588,12 @@ k_sweep_tma(const SweepLaunch L)
 // ------------------------------------------------------------------------------------------------
 constexpr int kW = kOwnedWarpsPerCta;
 
-template <int CW, int G, int R, int MODE, int D, int V, bool HO>
+template <int CW, int G, int R, int MODE, int D, int V, bool HO, int NB = 1>
 static cudaError_t launch_tma_ho(const SweepLaunch &L, dim3 grid, cudaStream_t st)
 {
     constexpr int smem = kW * StageGeom<CW, G, R, D>::kWarpBytes;
     if (smem > 227 * 1024) return cudaErrorInvalidValue;
-    auto kern = k_sweep_tma<CW, G, R, MODE, D, V, kW, HO>;
+    auto kern = k_sweep_tma<CW, G, R, MODE, D, V, kW, HO, NB>;
     // the shared-memory opt-in is per kernel and device: set once, not on every launch
     static bool opted_in[64] = {};
     int dev = 0;
@@ -614,6 +628,51 @@ static cudaError_t launch_variant(const SweepLaunch &L, dim3 grid, cudaStream_t 
         if (L.pair) return cudaErrorInvalidValue;
     }
     return L.rev ? launch_tma<CW, G, R, MODE, D, 1>(L, grid, st) : launch_tma<CW, G, R, MODE, D, 0>(L, grid, st);
+}
+
+// NB bins packed per row (rt_sweep_nb*x3.cu): J mode and the writer-count mode, ring depth 2, no seam handoff
+template <int CW, int G, int R, int NB>
+static cudaError_t launch_rows_packed(const SweepLaunch &L, cudaStream_t st)
+{
+    if (L.tiles != (L.Nc + kW * R - 1) / (kW * R) || L.nitems < 1 || L.nbins % NB != 0 || L.handoff) return cudaErrorInvalidValue;
+    const dim3 grid(L.nitems, 1, L.nbins / NB);
+    if (L.mode == MODE_J) {
+        if (L.pair) return launch_tma_ho<CW, G, R, MODE_J, 2, 2, false, NB>(L, grid, st);
+        return L.rev ? launch_tma_ho<CW, G, R, MODE_J, 2, 1, false, NB>(L, grid, st) : launch_tma_ho<CW, G, R, MODE_J, 2, 0, false, NB>(L, grid, st);
+    }
+    if (L.mode == MODE_OWNERS) {
+        if (L.pair) return launch_tma_ho<CW, G, R, MODE_OWNERS, 2, 2, false, NB>(L, grid, st);
+        return L.rev ? launch_tma_ho<CW, G, R, MODE_OWNERS, 2, 1, false, NB>(L, grid, st) : launch_tma_ho<CW, G, R, MODE_OWNERS, 2, 0, false, NB>(L, grid, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+// G = NB * (chunks per bin); rows per warp 1 or 2
+template <int CW, int G, int NB>
+cudaError_t launch_sweep_packed(const SweepLaunch &L, cudaStream_t st)
+{
+    switch (L.rows) {
+    case 1: return launch_rows_packed<CW, G, 1, NB>(L, st);
+    case 2: return launch_rows_packed<CW, G, 2, NB>(L, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+template <int CW, int G, int NB>
+int ctas_per_sm_packed(int rows, bool pair)
+{
+    int n = 0;
+    auto q = [&](auto kern, int smem) {
+        if (smem > 227 * 1024) return cudaErrorInvalidValue;
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, 32 * kW, smem);
+    };
+    cudaError_t e = cudaErrorInvalidValue;
+    if (rows == 1) e = pair ? q(k_sweep_tma<CW, G, 1, MODE_J, 2, 2, kW, false, NB>, kW * StageGeom<CW, G, 1, 2>::kWarpBytes)
+                            : q(k_sweep_tma<CW, G, 1, MODE_J, 2, 0, kW, false, NB>, kW * StageGeom<CW, G, 1, 2>::kWarpBytes);
+    if (rows == 2) e = pair ? q(k_sweep_tma<CW, G, 2, MODE_J, 2, 2, kW, false, NB>, kW * StageGeom<CW, G, 2, 2>::kWarpBytes)
+                            : q(k_sweep_tma<CW, G, 2, MODE_J, 2, 0, kW, false, NB>, kW * StageGeom<CW, G, 2, 2>::kWarpBytes);
+    return e == cudaSuccess ? n : 0;
 }
 
 template <int CW, int G, int R>

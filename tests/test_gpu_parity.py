@@ -524,6 +524,58 @@ def test_schedules_agree(orc, tune):
     assert rel_err(again, ref2["Jin"]).max() <= J_TOL
 
 
+@pytest.mark.parametrize("dims,nb,rows,rays,nside", [
+    ((32, 64, 16), 3, None, 1, 2),          # 32- and 64-cell rows, three bins in one group
+    ((128, 64, 40), 3, 1, 1, 2),            # 128-cell rows (C5's width), one ray row per warp
+    ((128, 128, 24), 3, 2, 1, 2),           # two ray rows per warp
+    ((64, 32, 24), 6, None, 1, 2),          # two groups of three bins (grid.z = 2)
+    ((100, 60, 24), 3, None, 1, 2),         # padded rows
+    ((32, 64, 24), 3, None, 2, 1),          # r = 2 sub-lattices
+])
+def test_packed_bins(orc, dims, nb, rows, rays, nside):
+    """rt_tune("binpack", 1): the multi-bin packed kernel (three bins of a cell row share the row: one bulk copy, one
+    slab program, one set of addresses for three intensity recurrences) against the oracle, with
+    per-face inflow that differs per bin (the b-handoff's carry restarts at every bin), plus everything that reads the
+    packed layout: J total, the rates epilogue, rt_combine, point sources, counts, writer counts."""
+    import paper_1410_0763_b200 as rt
+    torch = _torch()
+    kap, S = _rand(dims, 41, nb=nb)
+    kap *= (0.3 + 0.5 * np.arange(nb, dtype=np.float32))[:, None, None, None]
+    dirs = np.concatenate([orc.healpix_dirs(nside), np.array([[1, 1, 1], [-1, 0.5, 0.25], [0, 0, -1], [0.3, -1, 0]], dtype=np.float64)])
+    rng = np.random.default_rng(5)
+    faces = rng.uniform(0.0, 1.0, (nb, 6))
+    w = rng.uniform(0.2, 3.0, (4, nb))
+    ref = orc.sweep(kap, S, dirs, Ibc_faces=faces, rays_per_cell=rays)
+    Gr, Hr = orc.rates(ref["Jin"], S.astype(np.float64), w[0], w[1], w[2], w[3])
+    src = np.array([[0, 0, 0], [dims[0] * 128, dims[1] * 128 + 77, dims[2] * 256]], dtype=np.int32)
+    lum = rng.uniform(0.5, 2.0, (2, nb))
+    refQ = orc.point_sources(kap, src, lum, want_diag=False)
+    tr = rt.RayTracer(dims, nb, dirs, rows=rows, rays_per_cell=rays, tune={"binpack": 1})
+    try:
+        tr.set_inflow_faces(faces)
+        tr.set_fields(torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda())
+        Jin = tr.sweep(what=rt.RT_J_IN).cpu().numpy()
+        Jin2 = tr.sweep(what=rt.RT_J_IN).cpu().numpy()
+        J = tr.sweep(what=rt.RT_J_TOTAL).cpu().numpy()
+        G, H = tr.sweep_rates(w[0], w[1], w[2], w[3])
+        G, H = G.cpu().numpy(), H.cpu().numpy()
+        tot = tr.sweep(what=rt.RT_SUM_IN)
+        Jc = tr.combine(tot, len(dirs), what=rt.RT_J_TOTAL).cpu().numpy()
+        Q, _, steps = tr.point_sources(src, lum, want_steps=True)
+        Q = Q.cpu().numpy()
+        cnt = tr.segment_counts(-1).cpu().numpy().astype(np.uint32)
+        wr = tr.debug_writer_counts()
+    finally:
+        tr.close()
+    assert np.array_equal(Jin, Jin2)
+    assert np.array_equal(cnt, ref["cnt_sum"])
+    assert rel_err(Jin, ref["Jin"]).max() <= J_TOL and rel_err(J, ref["J"]).max() <= J_TOL
+    assert rel_err(Jc, ref["J"]).max() <= J_TOL
+    assert rel_err(G, Gr).max() <= J_TOL and rel_err(H, Hr).max() <= J_TOL
+    assert steps == refQ["steps"] and rel_err(Q, refQ["Q"]).max() <= J_TOL
+    assert wr["max_writers"] == 1 and wr["max_seam_writers"] <= 1 and wr["stores"] == wr["expected_stores"]
+
+
 def test_sweep_is_deterministic_and_repeatable(orc):
     from rt_inputs import make_fields
     import paper_1410_0763_b200 as rt
