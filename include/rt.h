@@ -174,6 +174,29 @@ int rt_point_sources(rt_ctx *ctx, const int *src_fix_host, const double *lum_hos
                      int diag_src, int diag_bin, float *tau_dev, unsigned long long *steps_host, void *cuda_stream);
 
 /*
+ * Per-species photo-ionisation and photo-heating rates from the point-source absorption rate (Appendix 1,
+ * PAPER.md:378-388, eqs. A4-A6), as an elementwise epilogue of rt_point_sources.  With Q_b the absorbed
+ * energy per unit time and shell volume in bin b (rt_point_sources), kappa_b the total opacity of the cell
+ * (the kappa of the last rt_set_fields), kappa_i,b the part of it contributed by species i, n_i the number
+ * density of species i and h nu_b the photon energy of bin b:
+ *     Gamma_i = (1/n_i) sum_{b: h nu_b >= h nu_i}  (kappa_i,b / kappa_b)  Q_b / (h nu_b)                    (A4, A5)
+ *     Heat_i  = (1/n_i) sum_{b: h nu_b >= h nu_i}  (kappa_i,b / kappa_b)  Q_b (h nu_b - h nu_i) / (h nu_b)  (A6)
+ * (dtau_i / dtau = kappa_i / kappa inside one cell; N_i = n_i x shell volume, and Q is already per unit shell
+ * volume; the frequency integrals are sums over the rectangular bins of eqs. 22-23.  Eq. A6 is read with the
+ * species' own absorption rate, like eq. 6: DESIGN.md reading PS-f.)  A cell with n_i <= 0 gets 0.
+ *   Q_dev        : DEVICE, fp32 [nbins][nz][ny][nx] (output of rt_point_sources)
+ *   kappa_sp_dev : DEVICE, fp32 [nspecies][nbins][nz][ny][nx], opacity contributed by each species (>= 0)
+ *   n_sp_dev     : DEVICE, fp32 [nspecies][nz][ny][nx], number densities
+ *   hnu_host     : HOST, fp64 [nbins], photon energy of each bin (> 0)
+ *   hnu_thr_host : HOST, fp64 [nspecies], threshold energy h nu_i of each species (>= 0)
+ *   Gamma_dev, Heat_dev : DEVICE, fp32 [nspecies][nz][ny][nx], fully overwritten
+ * 1 <= nspecies <= 8 (RT_EINVAL otherwise).  Asynchronous on `cuda_stream`; RT_ESTATE before rt_set_fields.
+ */
+int rt_point_source_rates(rt_ctx *ctx, const float *Q_dev, const float *kappa_sp_dev, const float *n_sp_dev, int nspecies,
+                          const double *hnu_host, const double *hnu_thr_host, float *Gamma_dev, float *Heat_dev,
+                          void *cuda_stream);
+
+/*
  * Diagnostics required by the parity gates (integer traversal data, summed ds).  They run the same
  * traversal kernel as rt_sweep with the transfer arithmetic replaced by counting.
  *

@@ -215,5 +215,35 @@ def point_sources(kappa, src_fix, lum, cell_width: float = 1.0, diag=(0, 0), wan
     return {"Q": Q, "tau": d[0], "dtau": d[1], "r_in": d[2], "r_out": d[3], "steps": int(steps.value)}
 
 
+def point_source_rates(Q, kappa, kappa_sp, n_sp, hnu, hnu_thr):
+    """Per-species photo-ionisation and photo-heating rates of the point-source absorption, fp64 (Appendix 1,
+    PAPER.md:378-388, eqs. A4-A6), written out per cell:
+      absorbed photons per unit time and shell volume in bin b      Ndot_b   = Q_b / (h nu_b)              (A3)
+      share of species i (dtau_i / dtau = kappa_i / kappa in a cell) Ndot_i,b = (kappa_i,b / kappa_b) Ndot_b (A4)
+      Gamma_i = (1 / n_i) sum_{b: h nu_b >= h nu_i} Ndot_i,b                                               (A5)
+      Heat_i  = (1 / n_i) sum_{b: h nu_b >= h nu_i} Ndot_i,b (h nu_b - h nu_i)                             (A6, reading PS-f)
+    (N_i = n_i x shell volume; Q is per unit shell volume; the integrals are sums over rectangular bins, eqs. 22-23.)
+    Q [nb][cells...], kappa [nb][...] total opacity, kappa_sp [ns][nb][...], n_sp [ns][...]; cells with n_i <= 0 get 0.
+    Pinned by tests/test_point_sources.py::test_ps5_*."""
+    Q = np.asarray(Q, dtype=np.float64)
+    kappa = np.asarray(kappa, dtype=np.float64)
+    kappa_sp = np.asarray(kappa_sp, dtype=np.float64)
+    n_sp = np.asarray(n_sp, dtype=np.float64)
+    ns, nb = kappa_sp.shape[0], kappa_sp.shape[1]
+    G = np.zeros(n_sp.shape, dtype=np.float64)
+    H = np.zeros(n_sp.shape, dtype=np.float64)
+    for i in range(ns):
+        for b in range(nb):
+            if float(hnu[b]) < float(hnu_thr[i]):
+                continue
+            ndot_ib = kappa_sp[i, b] / kappa[b] * (Q[b] / float(hnu[b]))
+            G[i] += ndot_ib
+            H[i] += ndot_ib * (float(hnu[b]) - float(hnu_thr[i]))
+        ok = n_sp[i] > 0
+        G[i] = np.where(ok, G[i] / np.where(ok, n_sp[i], 1.0), 0.0)
+        H[i] = np.where(ok, H[i] / np.where(ok, n_sp[i], 1.0), 0.0)
+    return G, H
+
+
 def num_threads() -> int:
     return int(lib().orc_num_threads())

@@ -12,7 +12,7 @@ RT_OWNED, RT_ATOMIC_ABLATION, RT_PAPER_GROUPS = 0, 1, 2
 RT_J_IN, RT_J_TOTAL, RT_SUM_IN = 0, 1, 2
 
 EXPORTED_SYMBOLS = [
-    "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_set_inflow_faces", "rt_sweep", "rt_combine", "rt_sweep_rates", "rt_point_sources", "rt_segment_counts",
+    "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_set_inflow_faces", "rt_sweep", "rt_combine", "rt_sweep_rates", "rt_point_sources", "rt_point_source_rates", "rt_segment_counts",
     "rt_sum_ds", "rt_total_segments", "rt_debug_writer_counts", "rt_working_set_bytes", "rt_probe_bandwidth", "rt_direction_records", "rt_tune", "rt_last_launch_count",
     "rt_last_sweep_kernel_ms", "rt_destroy", "rt_strerror", "rt_last_cuda_error",
 ]
@@ -57,6 +57,8 @@ def load_library():
     L.rt_sweep_rates.restype = C.c_int
     L.rt_point_sources.argtypes = [vp, C.POINTER(C.c_int), dp, C.c_int, vp, C.c_int, C.c_int, vp, C.POINTER(C.c_ulonglong), vp]
     L.rt_point_sources.restype = C.c_int
+    L.rt_point_source_rates.argtypes = [vp, vp, vp, vp, C.c_int, dp, dp, vp, vp, vp]
+    L.rt_point_source_rates.restype = C.c_int
     L.rt_segment_counts.argtypes = [vp, C.c_int, vp, vp]
     L.rt_segment_counts.restype = C.c_int
     L.rt_sum_ds.argtypes = [vp, dp, dp, dp, vp]
@@ -184,6 +186,22 @@ def rt_point_sources(h, src_fix, lum, Q, numel, nbins, tau=None, diag=(0, 0), wa
     return int(steps.value)
 
 
+def rt_point_source_rates(h, Q, kappa_sp, n_sp, hnu, hnu_thr, Gamma, Heat, ncell, nbins, stream=None):
+    import torch
+    hnu = np.ascontiguousarray(hnu, dtype=np.float64).reshape(-1)
+    thr = np.ascontiguousarray(hnu_thr, dtype=np.float64).reshape(-1)
+    ns = thr.shape[0]
+    if hnu.shape[0] != nbins:
+        raise ValueError("hnu must have one entry per bin")
+    p = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+    _check(load_library().rt_point_source_rates(h, _dev_ptr(Q, torch.float32, ncell * nbins, "Q"),
+                                                _dev_ptr(kappa_sp, torch.float32, ns * nbins * ncell, "kappa_sp"),
+                                                _dev_ptr(n_sp, torch.float32, ns * ncell, "n_sp"), ns, p(hnu), p(thr),
+                                                _dev_ptr(Gamma, torch.float32, ns * ncell, "Gamma"),
+                                                _dev_ptr(Heat, torch.float32, ns * ncell, "Heat"), _stream(stream)),
+           "rt_point_source_rates")
+
+
 def rt_segment_counts(h, dir_index, counts, numel, stream=None):
     import torch
     _check(load_library().rt_segment_counts(h, int(dir_index), _dev_ptr(counts, torch.int32, numel, "counts"),
@@ -299,6 +317,15 @@ class RayTracer:
         tau = torch.empty((self.nz, self.ny, self.nx), dtype=torch.float32, device="cuda") if diag is not None else None
         n = rt_point_sources(self.h, src_fix, lum, Q, self.numel, self.nbins, tau, diag or (0, 0), want_steps, stream)
         return Q, tau, n
+
+    def point_source_rates(self, Q, kappa_sp, n_sp, hnu, hnu_thr, stream=None):
+        """rt_point_source_rates: per-species (Gamma, Heat), each [nspecies][nz][ny][nx] (eqs. A4-A6)."""
+        import torch
+        ns = int(n_sp.shape[0])
+        G = torch.empty((ns, self.nz, self.ny, self.nx), dtype=torch.float32, device="cuda")
+        H = torch.empty_like(G)
+        rt_point_source_rates(self.h, Q, kappa_sp, n_sp, hnu, hnu_thr, G, H, self.nx * self.ny * self.nz, self.nbins, stream)
+        return G, H
 
     def segment_counts(self, dir_index=-1, stream=None):
         import torch

@@ -970,6 +970,31 @@ extern "C" int rt_point_sources(rt_ctx *c, const int *src_fix_host, const double
     return RT_OK;
 }
 
+extern "C" int rt_point_source_rates(rt_ctx *c, const float *Q_dev, const float *kappa_sp_dev, const float *n_sp_dev, int nspecies,
+                                     const double *hnu_host, const double *hnu_thr_host, float *Gamma_dev, float *Heat_dev, void *stream)
+{
+    if (!c || !Q_dev || !kappa_sp_dev || !n_sp_dev || !hnu_host || !hnu_thr_host || !Gamma_dev || !Heat_dev) return RT_EINVAL;
+    if (nspecies < 1 || nspecies > kMaxSpecies) return RT_EINVAL;
+    DevGuard dev_guard(c->device);
+    if (!c->fields_set) return RT_ESTATE;
+    SpeciesWeights W;
+    memset(&W, 0, sizeof(W));
+    for (int b = 0; b < c->nbins; ++b)
+        if (!(hnu_host[b] > 0.0) || !std::isfinite(hnu_host[b])) return RT_EINVAL;
+    for (int s = 0; s < nspecies; ++s) {
+        if (!(hnu_thr_host[s] >= 0.0) || !std::isfinite(hnu_thr_host[s])) return RT_EINVAL;
+        for (int b = 0; b < c->nbins; ++b)
+            if (hnu_host[b] >= hnu_thr_host[s]) {              // the integrals of eqs. A5-A6 start at the threshold
+                W.wG[s][b] = (float)(1.0 / hnu_host[b]);
+                W.wH[s][b] = (float)((hnu_host[b] - hnu_thr_host[s]) / hnu_host[b]);
+            }
+    }
+    CK(launch_point_source_rates(Gamma_dev, Heat_dev, Q_dev, kappa_sp_dev, n_sp_dev, c->d_P[0], c->pp[0], c->nx, c->ny, c->nz,
+                                 c->pitch[0], c->nbins, c->nbp, nspecies, W, c->sm_count, (cudaStream_t)stream));
+    c->last_launches = 1;
+    return RT_OK;
+}
+
 extern "C" int rt_segment_counts(rt_ctx *c, int dir_index, unsigned int *counts_dev, void *stream)
 {
     if (!c || !counts_dev || dir_index < -1 || dir_index >= c->ndirs) return RT_EINVAL;

@@ -116,6 +116,13 @@ cudaError_t launch_combine(float *J, const float *sum, const float2 *Pnat, int p
 cudaError_t launch_point_sources(float *Q, float *tau_out, const float2 *Pnat, int ppN, int nx, int ny, int nz, int nxp,
                                  const int *src_dev, const float *lum_dev, int nsrc, int nbins, int nbp, float cell_width,
                                  int diag_src, int diag_bin, unsigned long long *steps_dev, cudaStream_t st);
+// weights of the per-species point-source rates (rt_point_source_rates, eqs. A5-A6): wG = 1 / h nu_b, wH = (h nu_b - h nu_i) / h nu_b
+// for bins at or above the species' threshold, 0 below it
+constexpr int kMaxSpecies = 8;
+struct SpeciesWeights { float wG[kMaxSpecies][16], wH[kMaxSpecies][16]; };
+cudaError_t launch_point_source_rates(float *Gamma, float *Heat, const float *Q, const float *ksp, const float *nsp,
+                                      const float2 *Pnat, int ppN, int nx, int ny, int nz, int nxp, int nbins, int nbp,
+                                      int nspecies, const SpeciesWeights &W, int sm_count, cudaStream_t st);
 cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const float *accNC, int slotsN,
                                    const float *accT, const float *accTC, int slotsT,
                                    int nx, int ny, int nz, int nxp, int nyp, cudaStream_t st);

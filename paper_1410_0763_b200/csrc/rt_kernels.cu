@@ -669,6 +669,57 @@ cudaError_t launch_point_sources(float *Q, float *tau_out, const float2 *Pnat, i
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------
+// Per-species rates of the point-source absorption (Appendix 1, eqs. A4-A6): one thread
+// per cell, species and bins looped inside (elementwise; every array is read once, coalesced).
+//   Gamma_i = (1/n_i) sum_b (kappa_ib / kappa_b) Q_b wG[i][b],  wG = 1 / h nu_b            for h nu_b >= h nu_i, else 0
+//   Heat_i  = (1/n_i) sum_b (kappa_ib / kappa_b) Q_b wH[i][b],  wH = (h nu_b - h nu_i) / h nu_b
+// ------------------------------------------------------------------------------------------------
+__global__ void k_point_source_rates(float *__restrict__ Gamma, float *__restrict__ Heat, const float *__restrict__ Q,
+                                     const float *__restrict__ ksp, const float *__restrict__ nsp,
+                                     const float2 *__restrict__ Pnat, int ppN, int nx, int nxp, size_t rows, size_t ncell,
+                                     int nbins, int nbp, int nspecies, const SpeciesWeights W)
+{
+    const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncell; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t row = i / nx;
+        const int x = (int)(i - row * nx);
+        float g[kMaxSpecies], h[kMaxSpecies];
+#pragma unroll
+        for (int s = 0; s < kMaxSpecies; ++s) g[s] = h[s] = 0.0f;
+        for (int b = 0; b < nbins; ++b) {
+            const float kap = fN[field_index(packed_cell(b, row, x, nbp, nxp, rows), ppN)];
+            const float qk = Q[(size_t)b * ncell + i] / kap;          // kappa > 0: floored in the packed copy
+#pragma unroll
+            for (int s = 0; s < kMaxSpecies; ++s)
+                if (s < nspecies) {
+                    const float part = ksp[((size_t)s * nbins + b) * ncell + i] * qk;      // (dtau_i / dtau) Q_b   (A4)
+                    g[s] = fmaf(part, W.wG[s][b], g[s]);
+                    h[s] = fmaf(part, W.wH[s][b], h[s]);
+                }
+        }
+#pragma unroll
+        for (int s = 0; s < kMaxSpecies; ++s)
+            if (s < nspecies) {
+                const float n = nsp[(size_t)s * ncell + i];
+                Gamma[(size_t)s * ncell + i] = n > 0.0f ? g[s] / n : 0.0f;
+                Heat[(size_t)s * ncell + i] = n > 0.0f ? h[s] / n : 0.0f;
+            }
+    }
+}
+
+cudaError_t launch_point_source_rates(float *Gamma, float *Heat, const float *Q, const float *ksp, const float *nsp,
+                                      const float2 *Pnat, int ppN, int nx, int ny, int nz, int nxp, int nbins, int nbp,
+                                      int nspecies, const SpeciesWeights &W, int sm_count, cudaStream_t st)
+{
+    const size_t ncell = (size_t)nx * ny * nz;
+    size_t blocks = (ncell + 255) / 256;
+    if (blocks > (size_t)sm_count * 8) blocks = (size_t)sm_count * 8;
+    k_point_source_rates<<<(unsigned)blocks, 256, 0, st>>>(Gamma, Heat, Q, ksp, nsp, Pnat, ppN, nx, nxp, (size_t)ny * nz, ncell,
+                                                           nbins, nbp, nspecies, W);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_counts_finalise(unsigned *counts, const float *accN, const float *accNC, int slotsN,
                                    const float *accT, const float *accTC, int slotsT,
                                    int nx, int ny, int nz, int nxp, int nyp, cudaStream_t st)

@@ -120,6 +120,72 @@ def test_ps4_mirror_symmetry(orc):
         assert np.allclose(np.flip(qm, axis=3 - ax), q, rtol=1e-12)
 
 
+def _species_case(rng, shape, nb, ns):
+    """Seeded per-species cross sections and densities: kappa_i,b = n_i sigma_i,b, kappa_b = sum_i kappa_i,b."""
+    n_sp = rng.uniform(0.1, 2.0, (ns,) + shape)
+    sigma = rng.uniform(0.05, 0.6, (ns, nb))
+    kappa_sp = n_sp[:, None] * sigma.reshape(ns, nb, *([1] * len(shape)))
+    return n_sp, sigma, kappa_sp, kappa_sp.sum(axis=0)
+
+
+def test_ps5_species_split_conserves_photons(orc):
+    """A4 summed over the species is A3: with every threshold below every bin, sum_i n_i Gamma_i = sum_b Q_b / (h nu_b)
+    (each absorbed photon ionises exactly one particle), and sum_i n_i Heat_i = sum_b sum_i share_i Q_b (1 - h nu_i / h nu_b)."""
+    rng = np.random.default_rng(71)
+    nb, ns, shape = 3, 3, (4, 5, 6)
+    n_sp, sigma, kappa_sp, kappa = _species_case(rng, shape, nb, ns)
+    Q = rng.uniform(0.0, 3.0, (nb,) + shape)
+    hnu = np.array([1.0, 1.7, 3.2])
+    thr = np.array([0.5, 0.8, 1.0])
+    G, H = orc.point_source_rates(Q, kappa, kappa_sp, n_sp, hnu, thr)
+    photons = sum(Q[b] / hnu[b] for b in range(nb))
+    assert np.allclose((n_sp * G).sum(axis=0), photons, rtol=1e-13)
+    heat = sum(kappa_sp[i, b] / kappa[b] * Q[b] * (1.0 - thr[i] / hnu[b]) for i in range(ns) for b in range(nb))
+    assert np.allclose((n_sp * H).sum(axis=0), heat, rtol=1e-13)
+
+
+def test_ps5_single_species_and_thresholds(orc):
+    """One species carrying all the opacity: Gamma = sum_b Q_b / (n h nu_b) (A5 from A3).  A bin below a species'
+    threshold contributes nothing to that species (the integrals of A5-A6 start at nu_i); n_i = 0 gives 0."""
+    rng = np.random.default_rng(72)
+    shape = (3, 4, 5)
+    n = rng.uniform(0.5, 2.0, (1,) + shape)
+    kap = rng.uniform(0.1, 1.0, (2,) + shape)
+    Q = rng.uniform(0.0, 2.0, (2,) + shape)
+    hnu = np.array([1.2, 2.5])
+    G, H = orc.point_source_rates(Q, kap, kap[None], n, hnu, [1.0])
+    assert np.allclose(G[0], (Q[0] / 1.2 + Q[1] / 2.5) / n[0], rtol=1e-14)
+    assert np.allclose(H[0], (Q[0] * (0.2 / 1.2) + Q[1] * (1.5 / 2.5)) / n[0], rtol=1e-13)
+    G2, H2 = orc.point_source_rates(Q, kap, kap[None], n, hnu, [2.0])          # bin 0 lies below the threshold
+    assert np.allclose(G2[0], Q[1] / 2.5 / n[0], rtol=1e-14) and np.allclose(H2[0], Q[1] * (0.5 / 2.5) / n[0], rtol=1e-13)
+    n0 = n.copy()
+    n0[0, 0, 0, 0] = 0.0
+    G3, H3 = orc.point_source_rates(Q, kap, kap[None], n0, hnu, [1.0])
+    assert G3[0, 0, 0, 0] == 0.0 and H3[0, 0, 0, 0] == 0.0 and np.array_equal(G3[0].ravel()[1:], G[0].ravel()[1:])
+
+
+def test_ps5_thin_limit_is_eqs_5_and_6(orc):
+    """kappa -> 0: the photon-conserving rates reduce to eqs. 5-6 with the flux of eq. 4, bin by bin:
+    Gamma_i -> sum_b L_b sigma_i,b / (4 pi r^2 h nu_b), Heat_i -> sum_b L_b sigma_i,b (h nu_b - h nu_i) / (4 pi r^2 h nu_b),
+    with 1 / r^2 -> 3 / (r_out^2 + r_out r_in + r_in^2) for a shell of finite width (pin PS3)."""
+    rng = np.random.default_rng(73)
+    nb, ns, shape = 2, 2, (8, 8, 8)
+    n_sp = rng.uniform(0.5, 2.0, (ns,) + shape) * 1e-9
+    sigma = np.array([[0.3, 0.1], [0.0, 0.5]])                  # species 1 does not absorb in bin 0
+    kappa_sp = n_sp[:, None] * sigma.reshape(ns, nb, 1, 1, 1)
+    kappa = kappa_sp.sum(axis=0).astype(np.float32)             # the oracle's traversal takes fp32 kappa
+    kappa_sp = kappa_sp * (kappa.astype(np.float64) / kappa_sp.sum(axis=0))[None]   # shares consistent with the rounded total
+    lum = np.array([[4.0, 1.5]])
+    hnu, thr = np.array([1.0, 2.0]), np.array([0.9, 1.6])
+    r = orc.point_sources(kappa, [[0, 0, 0]], lum)
+    G, H = orc.point_source_rates(r["Q"], kappa, kappa_sp, n_sp, hnu, thr)
+    geom = 1.0 / (4 * math.pi / 3 * (r["r_out"] ** 2 + r["r_out"] * r["r_in"] + r["r_in"] ** 2))
+    for i in range(ns):
+        g = sum(lum[0, b] * sigma[i, b] / hnu[b] for b in range(nb) if hnu[b] >= thr[i]) * geom
+        h = sum(lum[0, b] * sigma[i, b] * (hnu[b] - thr[i]) / hnu[b] for b in range(nb) if hnu[b] >= thr[i]) * geom
+        assert np.allclose(G[i], g, rtol=1e-6) and np.allclose(H[i], h, rtol=1e-6)
+
+
 # ---------------------------------------------------------------------------------------------
 # CUDA path against the oracle
 PS_TOL = 1e-5          # relative, with the A14 floor: fp32 output of fp64 path sums over fp32 kappa
@@ -181,3 +247,37 @@ def test_point_sources_c3_sampled(orc):
     assert steps == ref["steps"]
     assert _ps_rel(tau.cpu().numpy(), ref["tau"]).max() <= PS_TOL
     assert _ps_rel(Q.cpu().numpy(), ref["Q"]).max() <= PS_TOL
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dims,nb,ns,binpack", [((33, 20, 17), 2, 3, 0), ((64, 40, 12), 3, 2, 0), ((64, 40, 12), 3, 8, 1), ((5, 4, 3), 1, 1, 0)])
+def test_point_source_rates_parity(orc, dims, nb, ns, binpack):
+    """rt_point_source_rates (eqs. A4-A6) against the oracle's per-species split of the oracle's own Q, on every cell;
+    thresholds that cut bins off, a species with zero density somewhere, bins as planes and packed rows."""
+    import torch
+    import paper_1410_0763_b200 as rt
+    nx, ny, nz = dims
+    rng = np.random.default_rng(81)
+    n_sp, sigma, kappa_sp, kappa = _species_case(rng, (nz, ny, nx), nb, ns)
+    n_sp[0, 0, 0, : nx // 2] = 0.0
+    kappa_sp = n_sp[:, None] * sigma.reshape(ns, nb, 1, 1, 1)
+    kap32 = kappa_sp.sum(axis=0).astype(np.float32)
+    ksp32, n32 = kappa_sp.astype(np.float32), n_sp.astype(np.float32)
+    hnu = np.linspace(1.0, 3.0, nb) if nb > 1 else np.array([1.3])
+    thr = np.linspace(0.8, 2.2, ns)
+    src = np.array([[0, 0, 0], [(nx // 2) * FIX + 128, (ny // 2) * FIX + 128, (nz // 2) * FIX + 128]], dtype=np.int32)
+    lum = rng.uniform(0.5, 2.0, (2, nb))
+    tr = rt.RayTracer(dims, nb, rt.healpix_dirs(1), tune={"binpack": binpack})
+    try:
+        tr.set_fields(torch.from_numpy(kap32).cuda(), torch.zeros(kap32.shape, device="cuda"))
+        Q, _, _ = tr.point_sources(src, lum)
+        G, H = tr.point_source_rates(Q, torch.from_numpy(ksp32).cuda(), torch.from_numpy(n32).cuda(), hnu, thr)
+        with pytest.raises(rt.RtError):
+            tr.point_source_rates(Q, torch.from_numpy(ksp32).cuda(), torch.from_numpy(n32).cuda(), -hnu, thr)
+    finally:
+        tr.close()
+    ref = orc.point_sources(kap32, src, lum, want_diag=False)
+    Gr, Hr = orc.point_source_rates(ref["Q"], kap32, ksp32, n32, hnu, thr)
+    assert _ps_rel(G.cpu().numpy(), Gr).max() <= PS_TOL
+    assert _ps_rel(H.cpu().numpy(), Hr).max() <= PS_TOL
+    assert np.all(G.cpu().numpy()[0, 0, 0, : nx // 2] == 0.0)
