@@ -99,7 +99,7 @@ struct rt_ctx {
     // overlapped schedule (small meshes): every class of directions (layout, dominant axis, pairs / singles, march
     // sense along b) has its own slot range and runs on its own internal stream ("lane"), so that the classes of a
     // sweep that does not fill the machine run side by side instead of one short launch after the other
-    struct ClassPlan { int l, pair, off, count, rev, Nc, tiles, slot_base, nslots, cap; };
+    struct ClassPlan { int l, pair, off, count, rev, Nc, tiles, slot_base, nslots, cap, lane, first; };
     int binpack = -1;                // rt_tune "binpack": -1 = automatic, 0 = bins are planes (one CTA per bin), 1 = three bins per row
     int nbp = 1;                     // bins packed per row of the packed fields and accumulators (1 or 3), fixed by ensure_buffers
     int wave_div = 0;                // overlapped schedule: work items per launch = one wave of resident CTAs / wave_div (0 = default)
@@ -386,14 +386,19 @@ static int stages_for(const rt_ctx *c, int layout)
     return c->pitch[layout] <= 64 ? kShortRowStages : 2;
 }
 
-// Classes of a full J sweep in launch order, each with a slot range of its own (overlapped schedule).  The
-// enumeration is the one run_traversal walks: per layout the mirror pairs, then the singles, cut where the dominant
-// axis or the march sense along b changes.  false if some class cannot run on the owned kernel.
-static bool build_overlap_plan(const rt_ctx *c, std::vector<rt_ctx::ClassPlan> &plan, int need[2], long long *items)
+// Classes of a full J sweep in launch order (overlapped schedule).  The enumeration is the one run_traversal walks:
+// per layout the mirror pairs, then the singles, cut where the dominant axis or the march sense along b changes.
+// The classes of one (layout, dominant axis) share a lane (an internal stream) and a slot range: they run one after
+// the other on that lane, so the slots of the first (largest) class serve the later ones too and the normalisation
+// reads, and the seam clear writes, one range per lane instead of one per class.  false if some class cannot run on
+// the owned kernel.
+static bool build_overlap_plan(const rt_ctx *c, std::vector<rt_ctx::ClassPlan> &plan, int need[2], long long *items, bool share_lanes)
 {
     plan.clear();
     need[0] = need[1] = 0;
     *items = 0;
+    int lane_of[2][3], lane_base[2][3], lane_slots[2][3], nlanes = 0;
+    for (int l = 0; l < 2; ++l) for (int a = 0; a < 3; ++a) lane_of[l][a] = -1;
     int off_all = 0, off_j = c->nv;
     for (int l = 0; l < 2; ++l) {
         const int nd = (int)c->order[l].size();
@@ -426,15 +431,29 @@ static bool build_overlap_plan(const rt_ctx *c, std::vector<rt_ctx::ClassPlan> &
                 rt_ctx::ClassPlan p;
                 p.l = l; p.pair = passes[ps].pair; p.off = passes[ps].off + i; p.count = n; p.rev = rev; p.Nc = Nc;
                 p.tiles = (Nc + kOwnedWarpsPerCta * rows - 1) / (kOwnedWarpsPerCta * rows);
-                p.slot_base = need[l];
                 // launches of one wave / wave_div work items; a launch that starts anywhere touches at most
                 // (cap - 1) / tiles + 2 entries, each of which needs a slot of its own
                 const int wave = passes[ps].pair ? c->cap_pair[l] : c->cap_single[l];
                 const int div = c->wave_div > 0 ? c->wave_div : kOverlapWaveDiv;
                 p.cap = std::max(p.tiles, (wave > 0 ? wave : n * p.tiles) / div);
-                p.nslots = std::max(1, std::min(n, (p.cap - 1) / p.tiles + 2));
-                if (p.nslots >= n) p.cap = n * p.tiles;          // every entry has its own slot: one launch
-                need[l] += p.nslots;
+                int want = std::max(1, std::min(n, (p.cap - 1) / p.tiles + 2));
+                if (want >= n) p.cap = n * p.tiles;              // every entry has its own slot: one launch
+                // (a sweep of a wave or two is all launch latency: there every class gets a lane and slots of its own)
+                p.first = !share_lanes || lane_of[l][a] < 0;
+                if (p.first) {                                   // the lane's first class fixes its slot range
+                    if (share_lanes && nlanes >= rt_ctx::kLanes) return false;
+                    lane_of[l][a] = nlanes++ % rt_ctx::kLanes;
+                    lane_base[l][a] = need[l];
+                    lane_slots[l][a] = want;
+                    need[l] += want;
+                } else if (want > lane_slots[l][a]) {
+                    // a later class lives in the slots the first one left: whole entries per launch, one slot to spare
+                    want = lane_slots[l][a];
+                    p.cap = std::max(1, want - 1) * p.tiles;
+                }
+                p.lane = lane_of[l][a];
+                p.slot_base = lane_base[l][a];
+                p.nslots = p.first ? want : lane_slots[l][a];
                 *items += (long long)n * p.tiles * (c->nbins / c->nbp);
                 plan.push_back(p);
                 i += n;
@@ -505,7 +524,7 @@ static int ensure_buffers(rt_ctx *c)
         std::vector<rt_ctx::ClassPlan> plan;
         int need[2];
         long long items = 0;
-        if (build_overlap_plan(c, plan, need, &items)) {
+        if (build_overlap_plan(c, plan, need, &items, false)) {
             long long capacity = 0;
             for (int l = 0; l < 2; ++l) capacity = std::max<long long>(capacity, (long long)std::max(c->cap_pair[l], c->cap_single[l]) * (c->nbins / c->nbp));
             const size_t budget = freeb / 3, need_fixed = field_bytes_l[0] + field_bytes_l[1];
@@ -518,7 +537,8 @@ static int ensure_buffers(rt_ctx *c)
             cudaDeviceGetAttribute(&l2_bytes, cudaDevAttrL2CacheSize, c->device);
             const bool resident = need_fixed <= (size_t)l2_bytes / 2;
             c->tiny = items <= 2 * capacity;
-            if ((c->overlap == 1 || (c->overlap == -1 && resident)) && fits) {
+            if (!c->tiny && !build_overlap_plan(c, plan, need, &items, true)) plan.clear();
+            if ((c->overlap == 1 || (c->overlap == -1 && resident)) && fits && !plan.empty()) {
                 c->plan.swap(plan);
                 c->overlap_on = true;
                 for (int l = 0; l < 2; ++l) c->slots[l] = std::max(c->slots[l], need[l]);
@@ -742,9 +762,10 @@ static int run_traversal(rt_ctx *c, int mode, int only_dir, int nbins, cudaStrea
     return RT_OK;
 }
 
-// Overlapped J sweep (ensure_buffers decided c->overlap_on): the classes run on the context's lanes, forked from
-// and joined back into `st` with events.  Every class owns its slot range and its first nslots entries start from
-// zero ("fresh"), so no slot accumulator is cleared; the sparsely written seam accumulators are.
+// Overlapped J sweep (ensure_buffers decided c->overlap_on): the lanes of the plan (one per layout and dominant axis)
+// run side by side on the context's internal streams, forked from and joined back into `st` with events; the classes
+// of a lane run one after the other in its slot range.  The first class of a lane starts the slots from zero
+// ("fresh" entries), so no slot accumulator is cleared; the sparsely written seam accumulators are.
 static int run_overlapped(rt_ctx *c, cudaStream_t st, int *launches, int used[2], bool record_events,
                           OwnerStats *own = nullptr)
 {
@@ -758,9 +779,8 @@ static int run_overlapped(rt_ctx *c, cudaStream_t st, int *launches, int used[2]
     if (record_events) CK(cudaEventRecord(c->ev0, st));
     if (!own) CK(cudaEventRecord(c->ev_fork, st));
     bool lane_used[rt_ctx::kLanes] = {};
-    int idx = 0;
     for (const auto &p : c->plan) {
-        const int ln = idx++ % rt_ctx::kLanes;
+        const int ln = p.lane;
         cudaStream_t ls = own ? st : c->lane[ln];
         if (!own && !lane_used[ln]) { CK(cudaStreamWaitEvent(ls, c->ev_fork, 0)); lane_used[ln] = true; }
         const int l = p.l;
@@ -773,7 +793,9 @@ static int run_overlapped(rt_ctx *c, cudaStream_t st, int *launches, int used[2]
         L.Nb = c->pitch[l]; L.pp = c->pp[l]; L.nbp = c->nbp; L.pair = p.pair; L.rev = p.rev; L.Nc = p.Nc; L.tiles = p.tiles;
         L.batch = c->d_batch + p.off;
         L.nslots = p.nslots;
-        L.fresh_below = p.nslots;
+        // the first class of a lane starts its slots from zero ("fresh" entries: it has at least nslots entries, and an
+        // entry writes every cell of its slot); the later classes of the lane add to what it left
+        L.fresh_below = p.first ? p.nslots : 0;
         const int cap = p.cap;
         const long long total = (long long)p.count * p.tiles;
         const size_t nacc = slot_stride * p.nslots;

@@ -20,6 +20,10 @@ struct SlabProg {
     unsigned flags;
 };
 enum : unsigned { F_SB1 = 1u, F_SC1 = 2u, F_SB2 = 4u, F_SC2 = 8u, F_P1 = 16u, F_P2 = 32u };
+// Above the traversal flags the flags word carries the row shift of the slab, floor(v0 + k m_c) mod Nc (v0 = the
+// sub-lattice's offset along c): the memory row of ray row q at slab k is (q + shift) mod Nc.  Extents are <= 2^20.
+constexpr unsigned kFlagMask = 63u;
+constexpr int kShiftBit = 8;
 
 // Per-direction device record.
 struct DirDev {

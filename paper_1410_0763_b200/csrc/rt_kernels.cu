@@ -61,7 +61,9 @@ __global__ void k_build_programs(const DirDev *__restrict__ dirs, int ndirs, Sla
         else                { l0 = tb; l1 = 1.0 - tb; f |= F_SB1 | F_SC1 | F_P1; }   // diagonal step
     }
     SlabProg s;
-    s.len0 = (float)(l0 * Lw); s.len1 = (float)(l1 * Lw); s.len2 = (float)(l2 * Lw); s.flags = f;
+    // row shift of the slab (rt_internal.h kShiftBit): whole cells the rays have moved along c before slab k, mod Nc
+    const long long shift = (((long long)sub_offset(D.sub, 1) + (long long)k * Mc) >> kF) % D.Nc;
+    s.len0 = (float)(l0 * Lw); s.len1 = (float)(l1 * Lw); s.len2 = (float)(l2 * Lw); s.flags = f | ((unsigned)shift << kShiftBit);
     prog[D.prog_off + k] = s;
 }
 
@@ -338,20 +340,23 @@ template <bool COUNTS> __device__ __forceinline__ typename std::conditional<COUN
 template <> __device__ __forceinline__ unsigned long long widen<true>(float v) { return (unsigned long long)__float2uint_rn(v); }
 template <> __device__ __forceinline__ double widen<false>(float v) { return (double)v; }
 
-// sum over the slots of (slot accumulator + seam accumulator) of one cell, four independent partial sums so that the
-// loads of several slots are in flight together (a 32^3 mesh is all latency here)
+// sum over the slots of (slot accumulator + seam accumulator) of one cell: eight independent loads per step (four
+// slots) so that enough bytes are in flight per SM to keep HBM busy (the kernel reads every slot of both layouts once:
+// 4 GB at C4), with streaming loads (nothing is read twice); a 32^3 mesh is all latency here
 template <bool COUNTS>
 __device__ __forceinline__ typename std::conditional<COUNTS, unsigned long long, double>::type
 sum_slots(const float *__restrict__ acc, const float *__restrict__ accC, int slots, size_t stride, size_t i)
 {
     typename std::conditional<COUNTS, unsigned long long, double>::type s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+    const float *__restrict__ pa = acc + i, *__restrict__ pc = accC + i;
     int sl = 0;
-    for (; sl + 1 < slots; sl += 2) {
-        const float a0 = acc[sl * stride + i], c0 = accC[sl * stride + i];
-        const float a1 = acc[(sl + 1) * stride + i], c1 = accC[(sl + 1) * stride + i];
+    for (; sl + 3 < slots; sl += 4, pa += 4 * stride, pc += 4 * stride) {
+        const float a0 = __ldcs(pa), c0 = __ldcs(pc), a1 = __ldcs(pa + stride), c1 = __ldcs(pc + stride);
+        const float a2 = __ldcs(pa + 2 * stride), c2 = __ldcs(pc + 2 * stride), a3 = __ldcs(pa + 3 * stride), c3 = __ldcs(pc + 3 * stride);
         s0 += widen<COUNTS>(a0); s1 += widen<COUNTS>(c0); s2 += widen<COUNTS>(a1); s3 += widen<COUNTS>(c1);
+        s0 += widen<COUNTS>(a2); s1 += widen<COUNTS>(c2); s2 += widen<COUNTS>(a3); s3 += widen<COUNTS>(c3);
     }
-    if (sl < slots) { s0 += widen<COUNTS>(acc[sl * stride + i]); s1 += widen<COUNTS>(accC[sl * stride + i]); }
+    for (; sl < slots; ++sl, pa += stride, pc += stride) { s0 += widen<COUNTS>(__ldcs(pa)); s1 += widen<COUNTS>(__ldcs(pc)); }
     return (s0 + s1) + (s2 + s3);
 }
 

@@ -372,23 +372,24 @@ __device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned
                  :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 
-// Row bookkeeping of one march, advanced slab by slab with adds only:
-//   frac = fractional part of v0 + k*m_c in units of 2^-20, v0 = 1/2 for one ray per cell (m_c = Mc / 2^20 <= 1)
-//   lb   = (q0 + floor(1/2 + k*m_c)) mod Nc : memory row of the first ray row at slab k
-//   offk = k * sk                            : element offset of slab k
-struct RowState {
-    int lb, offk;
-    unsigned frac;
-    __device__ __forceinline__ void init(int q0, int v0) { lb = q0; offk = 0; frac = (unsigned)v0; }
-    // true iff the rays step along c inside the current slab (cross or exact touch)
-    __device__ __forceinline__ bool steps(int Mc) const { return frac + (unsigned)Mc >= (unsigned)kOne; }
-    __device__ __forceinline__ void advance(int Mc, int Nc, int sk)
-    {
-        frac += (unsigned)Mc;
-        if (frac >= (unsigned)kOne) { frac -= (unsigned)kOne; lb = (lb + 1 == Nc) ? 0 : lb + 1; }
-        offk += sk;
-    }
-};
+// One lane of a converged warp, chosen by the hardware: inside `if (elect_one())` the compiler knows that a single
+// thread is active, so a bulk copy is one ELECT-predicated UBLKCP instead of a loop over the active lanes (which is
+// what `if (lane == 0)` around the asm statement compiles to: 15 instructions per copy).
+__device__ __forceinline__ bool elect_one()
+{
+    unsigned pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
+
+// flags word of a slab program (rt_internal.h SlabProg): traversal flags | row shift << kShiftBit.  A volatile asm
+// load keeps its place at the top of the slab, a whole slab body ahead of its use by the producer.
+__device__ __forceinline__ unsigned ld_flags(const SlabProg *p)
+{
+    unsigned v;
+    asm volatile("ld.global.nc.u32 %0, [%1];" : "=r"(v) : "l"(&p->flags));
+    return v;
+}
 
 // Shared memory of a warp: D stages, each the packed-field rows and the old accumulator rows of one
 // slab for the warp's R ray rows plus the seam row above them; then the warp's mbarriers.
@@ -401,7 +402,8 @@ struct StageGeom {
     static constexpr int kBarFull = D * kStage;               // D mbarriers: stage filled (transaction bytes)
     static constexpr int kBarHand = kBarFull + 32;            // 2 mbarriers: handoff ring slot h holds this warp's seam partial
     static constexpr int kBarEmpty = kBarHand + 32;           // 2 mbarriers: the next warp has taken slot h's partial
-    static constexpr int kWarpBytes = D * kStage + 128;
+    static constexpr int kProg = D * kStage + 128;            // D slab programs (16 B each): slab k's travels with its stage
+    static constexpr int kWarpBytes = D * kStage + 128 + 64;
     static_assert(D <= 4, "barrier block holds 4 stages");
 };
 
@@ -486,31 +488,37 @@ k_sweep_tma(const SweepLaunch L)
                 *reinterpret_cast<float4 *>(wbase + s * SG::kStage + (R + 1) * SG::kRowP + 16 * i) = make_float4(0.f, 0.f, 0.f, 0.f);
         __syncwarp();
     }
-    RowState ps;
-    ps.init(q0, sub_offset(Dp->sub, 1));
-    // (Tried: lane r issuing the copies of ray row r, so that the R + 1 addresses are computed side by side. It removes
-    // a third of the instructions of this block and changes nothing measurable: the block is not what the slab waits for.)
-    auto produce = [&](int s) {
-        if (lane == 0) {
+    // Row bookkeeping of one march comes from the slab programs: the flags word of slab k carries, above the traversal
+    // flags, the row shift floor(v0 + k m_c) mod Nc (rt_kernels.cu k_build_programs), so the memory row of the first
+    // ray row at slab k is (q0 + shift) mod Nc, and the rays step along c inside the slab iff an SC flag is set.
+    int poffk = 0;                                               // element offset of the slab being produced (k * sk)
+    auto produce = [&](int s, int kp, unsigned fw) {
+        if (elect_one()) {
             const unsigned st = wbase_s + s * SG::kStage, bar = bars + 8 * s;
-            const bool stp = ps.steps(Mc);
+            const bool stp = (fw & (F_SC1 | F_SC2)) != 0;
+            int lb = q0 + (int)(fw >> kShiftBit); if (lb >= Nc) lb -= Nc;
             const int nP = (MODE == MODE_J) ? R + (stp ? 1 : 0) : 0;
             const bool seamA = stp && seam.last;
-            mbar_expect_tx(bar, (unsigned)(nP * SG::kRowP + ((fresh ? 0 : R) + (seamA ? 1 : 0)) * SG::kRowA));
+            mbar_expect_tx(bar, (unsigned)(sizeof(SlabProg) + nP * SG::kRowP + ((fresh ? 0 : R) + (seamA ? 1 : 0)) * SG::kRowA));
+            bulk_g2s(wbase_s + SG::kProg + (unsigned)sizeof(SlabProg) * s, prog + kp, (unsigned)sizeof(SlabProg), bar);
 #pragma unroll
             for (int r = 0; r <= R; ++r) {
-                int l = ps.lb + r; if (l >= Nc) l -= Nc;
-                const int o = ps.offk + l * sl;
+                int l = lb + r; if (l >= Nc) l -= Nc;
+                const int o = poffk + l * sl;
                 // packed rows: 2 floats per cell in either packed layout, rows start at even cells
                 if (r < nP) bulk_g2s(st + r * SG::kRowP, P + o, SG::kRowP, bar);
                 if (r < R ? !fresh : seamA)
                     bulk_g2s(st + (R + 1) * SG::kRowP + r * SG::kRowA, (r < R ? acc : accC) + o, SG::kRowA, bar);
             }
         }
-        ps.advance(Mc, Nc, sk);
+        poffk += sk;
     };
-#pragma unroll 1
-    for (int kk = 0; kk < D && kk < Na; ++kk) produce(kk);
+    unsigned fwq[D];                                             // flags words of the slabs in flight, oldest first
+#pragma unroll
+    for (int kk = 0; kk < D; ++kk) {
+        fwq[kk] = 0;
+        if (kk < Na) { fwq[kk] = ld_flags(prog + kk); produce(kk, kk, fwq[kk]); }
+    }
 
     // Rows narrower than the template width are padded (rt_api.cu): a pad column carries a ray that has not yet
     // crossed the b side face (it matters for rays moving towards lower columns, which cross the pad first), so
@@ -537,24 +545,25 @@ k_sweep_tma(const SweepLaunch L)
     float *const accC_l = accC + lcol;
     unsigned hcnt = 0;                   // slabs with a step along c so far: handoff ring slot = hcnt & 1, use = hcnt >> 1
 
-    RowState cs;
-    cs.init(q0, sub_offset(Dp->sub, 1));
-    SlabProg pr = prog[0];
+    int coffk = 0;                                               // element offset of the current slab
     int s = 0;
     unsigned phase = 0;
 
 #pragma unroll 1
     for (int k = 0; k < Na; ++k) {
-        const unsigned fl = pr.flags;
-        const float len0 = pr.len0, len1 = pr.len1, len2 = pr.len2;
-        if (k + 1 < Na) pr = prog[k + 1];
+        // flags word of the slab this iteration's copies are for: loaded now, used after the slab body
+        unsigned fwn = 0;
+        if (k + D < Na) fwn = ld_flags(prog + k + D);
+        const unsigned fw = fwq[0];
+        const unsigned fl = fw & kFlagMask;
         float *rowp[R + 1];
+        int lb = q0 + (int)(fw >> kShiftBit); if (lb >= Nc) lb -= Nc;
 #pragma unroll
         for (int r = 0; r <= R; ++r) {
-            int l = cs.lb + r; if (l >= Nc) l -= Nc;
-            rowp[r] = (r < R ? acc_l : accC_l) + (cs.offk + l * sl);
+            int l = lb + r; if (l >= Nc) l -= Nc;
+            rowp[r] = (r < R ? acc_l : accC_l) + (coffk + l * sl);
         }
-        const int lwrap = Nc - 1 - cs.lb;
+        const int lwrap = Nc - 1 - lb;
         const unsigned char *sp = lane_p + s * SG::kStage;
         unsigned char *sa = lane_a + s * SG::kStage;
         const bool anySC = (fl & (F_SC1 | F_SC2)) != 0;
@@ -572,13 +581,19 @@ k_sweep_tma(const SweepLaunch L)
             ++hcnt;
         }
         mbar_wait(bars + 8 * s, phase);
+        // piece lengths of this slab: they came with the stage (one 16-byte bulk copy), every lane reads the same address
+        const float4 prv = *reinterpret_cast<const float4 *>(wbase + SG::kProg + sizeof(SlabProg) * s);
+        const float len0 = prv.x, len1 = prv.y, len2 = prv.z;
         RT_DISPATCH_SLAB(fl, fl, I, sp, sa, len0, len1, len2, Ib0, Ib1, Ic, invL, lane, lwrap, padmask, rowp, seam)
         __syncwarp();                     // every lane is done with stage s
         if (k + D < Na) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            produce(s);
+            produce(s, k + D, fwn);
         }
-        cs.advance(Mc, Nc, sk);
+#pragma unroll
+        for (int i = 0; i + 1 < D; ++i) fwq[i] = fwq[i + 1];
+        fwq[D - 1] = fwn;
+        coffk += sk;
         if (++s == D) { s = 0; phase ^= 1u; }
     }
 }
