@@ -245,6 +245,22 @@ def workload_name(spec):
         spec.name, spec.dims[0], spec.dims[1], spec.dims[2], spec.nside, spec.ndirs, spec.nbins, spec.seed)
 
 
+def sweep_entries(rec):
+    """Work entries of one owned sweep: a direction and its mirror image along the memory-contiguous transverse axis
+    (same dominant axis, march sense, |slopes|) are carried by one warp and share every accumulator read-modify-write;
+    directions without a partner (zero slope along that axis) run alone.  From rt_direction_records (host data)."""
+    from collections import Counter
+    pos, neg, n = Counter(), Counter(), len(rec)
+    for a, refl, Mb, Mc, _, _ in rec:
+        if Mb == 0:
+            continue
+        b, c = (1 if a == 0 else 0), (1 if a == 2 else 2)
+        key = (int(a), (int(refl) >> int(a)) & 1, (int(refl) >> c) & 1, int(Mb), int(Mc))
+        (neg if (int(refl) >> b) & 1 else pos)[key] += 1
+    pairs = sum(min(v, neg.get(k, 0)) for k, v in pos.items())
+    return pairs + (n - 2 * pairs)
+
+
 class Runner:
     """One config on this rank's GPU: device-resident timing, end-to-end timing, roofline figures."""
 
@@ -271,6 +287,7 @@ class Runner:
         self.tr.set_fields(self.kd, self.sd)
         self.updates = self.tr.total_segments() * spec.nbins          # exact integer traversal count x bins
         self.cell_dir_bins = spec.ncell * dirs.shape[0] * spec.nbins
+        self.entries = sweep_entries(self.tr.direction_records()[0]) if (args.flags == 0 and args.pair in (None, 1)) else dirs.shape[0]
         if self.sharded:                                               # whole-job updates: sum over the shares
             t = torch.tensor([self.updates], device="cuda", dtype=torch.int64)
             dist.all_reduce(t)
@@ -369,6 +386,7 @@ class Runner:
         bytes_per_launch = ALGO_BYTES_PER_CELL_DIR_BIN * self.cell_dir_bins / n_sweep_launches
         achieved = bytes_per_launch / (avg_launch_ms * 1e-3) / 1e9
         return {"ms": ms, "steps": steps, "value": value, "e2e": e2e, "clocks": clocks, "launches": launches,
+                "floor_bytes": 8.0 * self.spec.ncell * self.spec.nbins * self.entries, "entries": self.entries,
                 "kernel_ms": kernel_ms, "n_sweep_launches": n_sweep_launches, "avg_launch_ms": avg_launch_ms,
                 "bytes_per_launch": bytes_per_launch, "achieved": achieved}
 
@@ -395,6 +413,11 @@ def roofline_of(r, name, run, peaks, default_tuning):
            "note": "a mirror pair of directions shares every field load and accumulator read-modify-write, and the entries "
                    "of a launch find the fields in L2, so the 16-byte model is no upper bound on this schedule and frac "
                    "may exceed 1 (SURVEY.md 8(d)); dram_frac_from_traffic is the fraction of the HBM peak the kernel really draws"}
+    # what THIS schedule must move through HBM at the least: one 4-byte read + one 4-byte write of a private slot
+    # accumulator per cell, bin and work entry (a mirror pair of directions is one entry); <= 1 by construction
+    floor_gbs = run["floor_bytes"] / (run["kernel_ms"] * 1e-3) / 1e9
+    out["schedule_floor"] = {"what": "accumulator read-modify-write, 8 B per cell, bin and work entry", "entries": run["entries"],
+                             "bytes_per_step": run["floor_bytes"], "gbs": floor_gbs, "frac_of_hbm_peak": floor_gbs / hbm_peak}
     table, state = traffic_table()
     out["traffic_table"] = state
     if default_tuning and name in table:
@@ -404,6 +427,10 @@ def roofline_of(r, name, run, peaks, default_tuning):
         out["traffic_source"] = table[name].get("source")
         out["dram_gbs_from_traffic"] = traffic / (run["avg_launch_ms"] * 1e-3) / 1e9
         out["dram_frac_from_traffic"] = out["dram_gbs_from_traffic"] / hbm_peak
+        if "l2_bytes_per_cell_dir_bin" in table[name]:          # lts__t_bytes of the same launches, against the L2 read probe
+            l2t = float(table[name]["l2_bytes_per_cell_dir_bin"]) * r.cell_dir_bins / run["n_sweep_launches"]
+            out["l2_gbs_from_traffic"] = l2t / (run["avg_launch_ms"] * 1e-3) / 1e9
+            out["l2_frac_from_traffic"] = out["l2_gbs_from_traffic"] / peaks["l2_read"]
     return out
 
 
@@ -479,7 +506,7 @@ def main():
                 ws, fl, cdb, upd, sp = working_set, flushed, cell_dir_bins, r.updates, spec
             else:
                 rr = Runner(name, args, rt, torch, dist, world, rank)
-                run = rr.run(3, 3, sample_clocks=False)
+                run = rr.run({"C1": 20, "C2": 10, "C3": 5}.get(name, 3), 3, sample_clocks=False)   # short sweeps: more of them
                 ws, fl, cdb, upd, sp = rr.working_set, rr.flush, rr.cell_dir_bins, rr.updates, rr.spec
             rf = roofline_of(rr or r, name, run, peaks, True)
             configs[name] = {
@@ -487,7 +514,9 @@ def main():
                 "unit": UNIT, "updates_per_step": upd, "gpu_launches_per_step": run["launches"],
                 "e2e": {k: run["e2e"][k] for k in ("value", "ms_per_step", "h2d_ms", "pack_ms", "sweep_ms", "d2h_ms")},
                 "bound": rf["bound"], "peak": rf["peak"], "model_frac": rf["frac"], "model_frac_of_hbm_peak": rf["frac_of_hbm_peak"],
-                "dram_frac_from_traffic": rf.get("dram_frac_from_traffic"), "kernel_share_of_step": rf["kernel_share_of_step"],
+                "dram_frac_from_traffic": rf.get("dram_frac_from_traffic"), "l2_frac_from_traffic": rf.get("l2_frac_from_traffic"),
+                "schedule_floor_frac": rf["schedule_floor"]["frac_of_hbm_peak"],
+                "kernel_share_of_step": rf["kernel_share_of_step"],
                 "working_set_bytes": ws, "l2": "L2 flushed between timed steps" if fl else "working set larger than L2",
             }
             if rr is not None:

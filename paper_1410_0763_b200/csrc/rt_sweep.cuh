@@ -437,7 +437,7 @@ k_sweep_tma(const SweepLaunch L)
     const int ent = item / L.tiles, tile = item - ent * L.tiles;
     const int slot = ent % L.nslots, bin = blockIdx.z * NB;      // first bin of this CTA's group of NB packed bins
     const DirDev *__restrict__ Dp = L.dirs + L.batch[ent];
-    const int Nc = Dp->Nc, Na = Dp->Na, Mc = Dp->Mc;
+    const int Nc = Dp->Nc, Na = Dp->Na;
     const int q0c = tile * (W * R);                              // first ray row of the CTA (L.tiles of them cover Nc)
     const int nact = min(W, (Nc - q0c) / R);                     // warps of this CTA that own rows (Nc % R == 0)
     const int q0 = q0c + wid * R;
@@ -587,6 +587,7 @@ k_sweep_tma(const SweepLaunch L)
         RT_DISPATCH_SLAB(fl, fl, I, sp, sa, len0, len1, len2, Ib0, Ib1, Ic, invL, lane, lwrap, padmask, rowp, seam)
         __syncwarp();                     // every lane is done with stage s
         if (k + D < Na) {
+            // (measured without this fence: C3 / C4 / C5 unchanged to 0.5 %, so the ordering is kept explicit)
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             produce(s, k + D, fwn);
         }
