@@ -407,12 +407,88 @@ __global__ void __launch_bounds__(1024) k_finalise(float *__restrict__ J, unsign
     }
 }
 
+// Two adjacent cells per thread (float2 streaming loads, 64 x 64 tiles): every warp access is a 256-byte run of one
+// accumulator row instead of 128 bytes, which is what the DRAM pages want when 2 x (slotsN + slotsT) arrays are read
+// side by side (the 32 x 32 form reads the 4 GB of C4 at 3.1 TB/s).  Same arithmetic per cell, in the same order,
+// as k_finalise<false>.  Needs even nx and ny (the row pitches always are).
+__device__ __forceinline__ void sum_slots2(const float *__restrict__ acc, const float *__restrict__ accC, int slots, size_t stride,
+                                           size_t i, double &r0, double &r1)
+{
+    double a0 = 0, a1 = 0, a2 = 0, a3 = 0, b0 = 0, b1 = 0, b2 = 0, b3 = 0;       // the four partial sums of sum_slots, per cell
+    const float2 *__restrict__ pa = reinterpret_cast<const float2 *>(acc + i), *__restrict__ pc = reinterpret_cast<const float2 *>(accC + i);
+    const size_t st2 = stride / 2;                                               // stride (cells per slot) is even
+    int sl = 0;
+    for (; sl + 3 < slots; sl += 4, pa += 4 * st2, pc += 4 * st2) {
+        const float2 u0 = __ldcs(pa), v0 = __ldcs(pc), u1 = __ldcs(pa + st2), v1 = __ldcs(pc + st2);
+        const float2 u2 = __ldcs(pa + 2 * st2), v2 = __ldcs(pc + 2 * st2), u3 = __ldcs(pa + 3 * st2), v3 = __ldcs(pc + 3 * st2);
+        a0 += (double)u0.x; a1 += (double)v0.x; a2 += (double)u1.x; a3 += (double)v1.x;
+        a0 += (double)u2.x; a1 += (double)v2.x; a2 += (double)u3.x; a3 += (double)v3.x;
+        b0 += (double)u0.y; b1 += (double)v0.y; b2 += (double)u1.y; b3 += (double)v1.y;
+        b0 += (double)u2.y; b1 += (double)v2.y; b2 += (double)u3.y; b3 += (double)v3.y;
+    }
+    for (; sl < slots; ++sl, pa += st2, pc += st2) {
+        const float2 u = __ldcs(pa), v = __ldcs(pc);
+        a0 += (double)u.x; a1 += (double)v.x; b0 += (double)u.y; b1 += (double)v.y;
+    }
+    r0 = (a0 + a1) + (a2 + a3);
+    r1 = (b0 + b1) + (b2 + b3);
+}
+
+__global__ void __launch_bounds__(1024) k_finalise_wide(float *__restrict__ J, const float2 *__restrict__ Pnat, int ppN,
+                           const float *__restrict__ accN, const float *__restrict__ accNC, int slotsN,
+                           const float *__restrict__ accT, const float *__restrict__ accTC, int slotsT,
+                           int nx, int ny, int nz, int nxp, int nyp, int nbins, int nbp, float inv_nd, int add_S, int zb0)
+{
+    __shared__ double tile[64][65];
+    const int zb = (int)blockIdx.z + zb0;
+    const int bin = zb / nz, z = zb % nz;
+    const int x0 = blockIdx.x * 64, y0 = blockIdx.y * 64;
+    const size_t ncell = (size_t)nx * ny * nz;
+    const size_t ncellN = (size_t)nxp * ny * nz, ncellT = (size_t)nyp * nz * nx;
+    const size_t strideN = ncellN * nbins, strideT = ncellT * nbins;
+    // transposed layout [x][z][y]: two adjacent y per thread
+    for (int dx = threadIdx.y; dx < 64; dx += 32) {
+        const int x = x0 + dx, y = y0 + 2 * (int)threadIdx.x;
+        double s0 = 0.0, s1 = 0.0;
+        if (x < nx && y < ny)
+            sum_slots2(accT, accTC, slotsT, strideT, packed_cell(bin, (size_t)x * nz + z, y, nbp, nyp, (size_t)nz * nx), s0, s1);
+        tile[dx][2 * threadIdx.x] = s0;
+        tile[dx][2 * threadIdx.x + 1] = s1;
+    }
+    __syncthreads();
+    const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
+    for (int dy = threadIdx.y; dy < 64; dy += 32) {
+        const int x = x0 + 2 * (int)threadIdx.x, y = y0 + dy;
+        if (x < nx && y < ny) {
+            const size_t ip = packed_cell(bin, (size_t)z * ny + y, x, nbp, nxp, (size_t)ny * nz);
+            double n0, n1;
+            sum_slots2(accN, accNC, slotsN, strideN, ip, n0, n1);
+            const double s0 = tile[2 * threadIdx.x][dy] + n0, s1 = tile[2 * threadIdx.x + 1][dy] + n1;
+            // (kappa, S) of the two cells: one 16-byte load in either packed form (rt_internal.h field_index; ip is even)
+            const float4 f = *reinterpret_cast<const float4 *>(fN + 2 * ip);
+            const float k0 = f.x, k1 = ppN ? f.y : f.z, S0 = ppN ? f.z : f.y, S1 = f.w;
+            const float j0 = (float)(s0 * (double)inv_nd) / k0, j1 = (float)(s1 * (double)inv_nd) / k1;
+            const size_t i = (size_t)bin * ncell + ((size_t)z * ny + y) * nx + x;
+            *reinterpret_cast<float2 *>(J + i) = make_float2(add_S ? j0 + S0 : j0, add_S ? j1 + S1 : j1);
+        }
+    }
+}
+
 cudaError_t launch_normalise(float *J, const float2 *Pnat, int ppN, const float *accN, const float *accNC, int slotsN,
                              const float *accT, const float *accTC, int slotsT,
                              int nx, int ny, int nz, int nxp, int nyp, int nbins, int nbp, float inv_nd, int add_S, cudaStream_t st)
 {
     const long long planes = (long long)nz * nbins;
+    const bool wide = nx % 2 == 0 && ny % 2 == 0 && nx >= 128 && ny >= 128 && (reinterpret_cast<uintptr_t>(J) & 7u) == 0;
     for (long long zb0 = 0; zb0 < planes; zb0 += kMaxGridZ) {
+        if (wide) {
+            dim3 grid((nx + 63) / 64, (ny + 63) / 64, (unsigned)std::min<long long>(kMaxGridZ, planes - zb0)), block(32, 32);
+            k_finalise_wide<<<grid, block, 0, st>>>(J, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT,
+                                                    nx, ny, nz, nxp, nyp, nbins, nbp, inv_nd, add_S, (int)zb0);
+            const cudaError_t e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+            continue;
+        }
         dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, planes - zb0)), block(32, 32);
         k_finalise<false><<<grid, block, 0, st>>>(J, nullptr, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT,
                                                   nx, ny, nz, nxp, nyp, nbins, nbp, inv_nd, add_S, (int)zb0);
@@ -631,25 +707,32 @@ k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2
             // cell a step moves into is requested as soon as that cell is known and used one step later, so that its
             // latency (L1 hit rate 78 %, the rest from L2) is covered by the step's own arithmetic instead of waited for
             // (long-scoreboard stalls were 5.3 warps per issue slot).
-            float kap = fbin[2 * idx - (idx & ppN)];
-            for (;;) {
-                const TT Tn = ps_min(T[0], ps_min(T[1], T[2]));
-                if (idx == idx_t) {                                 // (padded linear indices of distinct cells differ)
-                    if (Tn == kInf) { r_in = 0.0; dr = r_out = 0.5 * (double)cell_width; }   // source at this cell's centre
-                    else { r_in = (double)T0 * scale; dr = (double)(Tn - T0) * scale; r_out = r_in + dr; }
-                    nstep += 1;
-                    break;
-                }
-                const double dT = (double)(Tn - T0);
-                nstep += 1;
-                ps_advance(T[0], idx, Tn, inc[0], didx[0]);
-                ps_advance(T[1], idx, Tn, inc[1], didx[1]);
-                ps_advance(T[2], idx, Tn, inc[2], didx[2]);
-                const float kap_next = fbin[2 * idx - (idx & ppN)];   // the cell just entered (at the latest the target cell)
-                tauT = fma((double)kap, dT, tauT);
-                kap = kap_next;
-                T0 = Tn;
+            // Two steps per loop turn with the two kappa registers swapping roles: a register move at the end of a
+            // step would wait for the load it copies (it did: 29 % of all stall samples on that one move).
+#define RT_PS_STEP(KUSE, KLOAD)                                                                                         \
+            {                                                                                                           \
+                const TT Tn = ps_min(T[0], ps_min(T[1], T[2]));                                                         \
+                if (idx == idx_t) {                                 /* (padded linear indices of distinct cells differ) */ \
+                    if (Tn == kInf) { r_in = 0.0; dr = r_out = 0.5 * (double)cell_width; }   /* source at this cell's centre */ \
+                    else { r_in = (double)T0 * scale; dr = (double)(Tn - T0) * scale; r_out = r_in + dr; }              \
+                    nstep += 1;                                                                                         \
+                    break;                                                                                              \
+                }                                                                                                       \
+                const double dT = (double)(Tn - T0);                                                                    \
+                nstep += 1;                                                                                             \
+                ps_advance(T[0], idx, Tn, inc[0], didx[0]);                                                             \
+                ps_advance(T[1], idx, Tn, inc[1], didx[1]);                                                             \
+                ps_advance(T[2], idx, Tn, inc[2], didx[2]);                                                             \
+                KLOAD = fbin[2 * idx - (idx & ppN)];                /* the cell just entered (at the latest the target cell) */ \
+                tauT = fma((double)KUSE, dT, tauT);                                                                     \
+                T0 = Tn;                                                                                                \
             }
+            float kap0 = fbin[2 * idx - (idx & ppN)], kap1 = 0.0f;
+            for (;;) {
+                RT_PS_STEP(kap0, kap1)
+                RT_PS_STEP(kap1, kap0)
+            }
+#undef RT_PS_STEP
             const double tau = tauT * scale;
             const double dtau = (double)kap_t * dr;
             const double vol = 4.0 * 3.14159265358979323846 / 3.0 * dr * (r_out * r_out + r_out * r_in + r_in * r_in);
