@@ -217,6 +217,24 @@ def run_point(args):
         dt = time.perf_counter() - t0
         cpu = {"value": r["steps"] * spec.nbins / dt, "unit": "ray steps/s", "cores": oracle.num_threads(), "kind": "oracle",
                "sample": "%d of %d sources, full mesh, %.1f s" % (ns, args.sources, dt)}
+    # issue-slot ceiling: the kernel is bound by instruction issue, not by memory.  Executed
+    # thread-instructions per ray step come from the committed ncu capture, valid for the kernel source it names.
+    roof, note = None, "no committed instruction count for this kernel source"
+    try:
+        t = json.load(open(os.path.join(ROOT, "profiles", "point_sources.json")))
+        if git_blob_sha(os.path.join(ROOT, t["kernel_source"])) == t["kernel_source_sha"]:
+            props = torch.cuda.get_device_properties(0)
+            clk = 1e6 * float(clocks.get("sm_max_mhz") or 1965.0)
+            peak = props.multi_processor_count * 4 * 32 * clk          # 4 schedulers x 1 warp-instruction per clock x 32 lanes
+            ach = float(t["thread_instructions_per_ray_step"]) * steps * spec.nbins / (ms * 1e-3)
+            roof = {"bound": "alu", "achieved": ach, "peak": peak, "unit": "thread-instructions/s", "frac": ach / peak,
+                    "traffic": None, "thread_instructions_per_ray_step": t["thread_instructions_per_ray_step"],
+                    "peak_kind": "SMs x 4 schedulers x 32 lanes x max SM clock (issue slots)", "source": t["source"]}
+            note = "issue-bound gather along long characteristics; DRAM traffic is negligible (kappa is L2-resident)"
+        else:
+            note = "stale: %s changed since the ncu capture" % t["kernel_source"]
+    except Exception:
+        pass
     print(json.dumps({
         "metric": "point_source_ray_steps_per_sec", "value": steps * spec.nbins / (ms * 1e-3), "unit": "ray steps/s",
         "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
@@ -224,7 +242,7 @@ def run_point(args):
         "config": {"workload": "point sources on " + workload_name(spec), "sources": args.sources,
                    "ray_steps_per_step": steps * spec.nbins, "rays_per_step": args.sources * spec.ncell * spec.nbins},
         "clocks": clocks, "gpu_launches": args.steps,
-        "roofline": None, "note": "gather along long characteristics: latency / integer-ALU bound, no roofline claimed",
+        "roofline": roof, "note": note,
         "cpu_baseline": cpu}))
 
 

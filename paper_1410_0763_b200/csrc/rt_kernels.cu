@@ -641,12 +641,16 @@ __device__ __forceinline__ void ps_advance(long long &T, int &idx, long long Tn,
     if (T == Tn) { idx += didx; T += inc; }
 }
 
-template <class TT>
+// PP: the packed native copy is pair-packed (a compile-time constant keeps its index arithmetic out of the ray step);
+// COUNT: the step count is wanted (the parity gate), else the counter is not kept
+template <class TT, int PP, bool COUNT>
 __global__ void __launch_bounds__(128)
-k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2 *__restrict__ Pnat, int ppN,
+k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2 *__restrict__ Pnat, int ppN_,
                 int nx, int ny, int nz, int nxp, const int *__restrict__ src, const float *__restrict__ lum, int nsrc,
                 int nbins, int nbp, float cell_width, int diag_src, int diag_bin, unsigned long long *__restrict__ steps)
 {
+    constexpr int ppN = PP;
+    (void)ppN_;
     const int bin = blockIdx.z;
     const long long ncell = (long long)nx * ny * nz;
     const long long cidx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -715,11 +719,11 @@ k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2
                 if (idx == idx_t) {                                 /* (padded linear indices of distinct cells differ) */ \
                     if (Tn == kInf) { r_in = 0.0; dr = r_out = 0.5 * (double)cell_width; }   /* source at this cell's centre */ \
                     else { r_in = (double)T0 * scale; dr = (double)(Tn - T0) * scale; r_out = r_in + dr; }              \
-                    nstep += 1;                                                                                         \
+                    if (COUNT) nstep += 1;                                                                              \
                     break;                                                                                              \
                 }                                                                                                       \
                 const double dT = (double)(Tn - T0);                                                                    \
-                nstep += 1;                                                                                             \
+                if (COUNT) nstep += 1;                                                                                           \
                 ps_advance(T[0], idx, Tn, inc[0], didx[0]);                                                             \
                 ps_advance(T[1], idx, Tn, inc[1], didx[1]);                                                             \
                 ps_advance(T[2], idx, Tn, inc[2], didx[2]);                                                             \
@@ -741,7 +745,7 @@ k_point_sources(float *__restrict__ Q, float *__restrict__ tau_out, const float2
         }
         Q[(size_t)bin * ncell + cidx] = (float)q;
     }
-    if (steps && bin == 0) {
+    if (COUNT && steps && bin == 0) {
         unsigned n = nstep;
         for (int o = 16; o > 0; o >>= 1) n += __shfl_xor_sync(0xffffffffu, n, o);
         if ((threadIdx.x & 31) == 0 && n) atomicAdd(steps, (unsigned long long)n);
@@ -754,12 +758,18 @@ cudaError_t launch_point_sources(float *Q, float *tau_out, const float2 *Pnat, i
 {
     const long long ncell = (long long)nx * ny * nz;
     dim3 grid((unsigned)((ncell + 127) / 128), 1, nbins);
-    if (nx <= 512 && ny <= 512 && nz <= 512)
-        k_point_sources<double><<<grid, 128, 0, st>>>(Q, tau_out, Pnat, ppN, nx, ny, nz, nxp, src_dev, lum_dev, nsrc, nbins, nbp, cell_width,
-                                                      diag_src, diag_bin, steps_dev);
-    else
-        k_point_sources<long long><<<grid, 128, 0, st>>>(Q, tau_out, Pnat, ppN, nx, ny, nz, nxp, src_dev, lum_dev, nsrc, nbins, nbp, cell_width,
-                                                         diag_src, diag_bin, steps_dev);
+    const bool small = nx <= 512 && ny <= 512 && nz <= 512, count = steps_dev != nullptr;
+#define RT_PS_LAUNCH(TT, PP, COUNT)                                                                                      \
+    k_point_sources<TT, PP, COUNT><<<grid, 128, 0, st>>>(Q, tau_out, Pnat, ppN, nx, ny, nz, nxp, src_dev, lum_dev, nsrc, nbins, nbp, \
+                                                         cell_width, diag_src, diag_bin, steps_dev)
+    if (small) {
+        if (ppN) { if (count) RT_PS_LAUNCH(double, 1, true); else RT_PS_LAUNCH(double, 1, false); }
+        else     { if (count) RT_PS_LAUNCH(double, 0, true); else RT_PS_LAUNCH(double, 0, false); }
+    } else {
+        if (ppN) { if (count) RT_PS_LAUNCH(long long, 1, true); else RT_PS_LAUNCH(long long, 1, false); }
+        else     { if (count) RT_PS_LAUNCH(long long, 0, true); else RT_PS_LAUNCH(long long, 0, false); }
+    }
+#undef RT_PS_LAUNCH
     return cudaGetLastError();
 }
 

@@ -95,3 +95,11 @@ def test_traffic_table_names_the_kernel_sources():
 def test_point_workload_line():
     d = _run_bench("--workload", "point", "--config", "C2", "--steps", "2", "--sources", "3")
     assert d["metric"] == "point_source_ray_steps_per_sec" and d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle"
+
+
+def test_point_source_instruction_count_names_its_kernel_source():
+    """profiles/point_sources.json ties the ncu-measured thread-instructions per ray step to the git blob hash of the
+    kernel source; bench.py --workload point drops its issue-slot roofline when the source has changed."""
+    t = json.load(open(os.path.join(ROOT, "profiles", "point_sources.json")))
+    assert os.path.exists(os.path.join(ROOT, t["kernel_source"])) and os.path.exists(os.path.join(ROOT, t["source"]))
+    assert len(t["kernel_source_sha"]) == 40 and 10 < t["thread_instructions_per_ray_step"] < 200
