@@ -233,8 +233,9 @@ def _rand(dims, seed, nb=1):
 
 @pytest.mark.parametrize("dims", [(20, 12, 10), (33, 7, 5), (1, 1, 1), (64, 20, 12), (20, 64, 12)])
 def test_generic_fallback_dims(orc, dims):
-    """Mesh sizes the owned kernel does not cover run on the generic (four-group) kernel; mixed cases
-    (one layout fast, the other generic) too.  Same gates."""
+    """Small and odd mesh sizes: since rows are padded to 32/64/128/256/512 cells these all run on the owned kernel
+    (R falls back to 1 for odd N_c; the 1 x 1 x 1 mesh too); only rows wider than 512 cells use the generic four-group
+    kernel (test_padded_rows_take_the_owned_path covers (600, 8, 4)).  Same gates."""
     kap, S = _rand(dims, 5)
     dirs = orc.healpix_dirs(2)
     out = gpu_run(kap, S, dirs, count_dirs=range(0, 48, 5))
