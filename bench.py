@@ -445,10 +445,18 @@ def roofline_of(r, name, run, peaks, default_tuning):
         out["traffic_source"] = table[name].get("source")
         out["dram_gbs_from_traffic"] = traffic / (run["avg_launch_ms"] * 1e-3) / 1e9
         out["dram_frac_from_traffic"] = out["dram_gbs_from_traffic"] / hbm_peak
-        if "l2_bytes_per_cell_dir_bin" in table[name]:          # lts__t_bytes of the same launches, against the L2 read probe
-            l2t = float(table[name]["l2_bytes_per_cell_dir_bin"]) * r.cell_dir_bins / run["n_sweep_launches"]
+        if "l2_sm_bytes_per_cell_dir_bin" in table[name]:
+            # bytes the SMs request from L2 in the same launches, against what the streaming probe reaches for this
+            # read / write mix: 1 / ((1 - w) / read + w / write), with write from the read-modify-write probe
+            # (2 / rmw = 1 / read + 1 / write)
+            w = float(table[name].get("l2_sm_write_share", 0.25))
+            l2t = float(table[name]["l2_sm_bytes_per_cell_dir_bin"]) * r.cell_dir_bins / run["n_sweep_launches"]
+            rd, rmw = peaks["l2_read"], peaks["l2_rmw"]
+            wr = 1.0 / max(2.0 / rmw - 1.0 / rd, 1e-9)
+            ceiling = 1.0 / ((1.0 - w) / rd + w / wr)
             out["l2_gbs_from_traffic"] = l2t / (run["avg_launch_ms"] * 1e-3) / 1e9
-            out["l2_frac_from_traffic"] = out["l2_gbs_from_traffic"] / peaks["l2_read"]
+            out["l2_mix_ceiling_gbs"] = ceiling
+            out["l2_frac_from_traffic"] = out["l2_gbs_from_traffic"] / ceiling
     return out
 
 
