@@ -118,6 +118,16 @@ class ClockSampler:
         return out
 
 
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def host_cores():
     try:
         return max(1, min(len(os.sched_getaffinity(0)), 32))
@@ -169,7 +179,7 @@ def run_reference(args):
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(spec), "sample": sample},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu_model": cpu_model(), "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
@@ -504,6 +514,9 @@ def main():
     torch.cuda.set_device(local)
     dist = None
     if world > 1:
+        # leave NCCL's communicator lines in the log (ranks, transports) so that a scaling run can be checked
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
@@ -543,6 +556,8 @@ def main():
                 "dram_frac_from_traffic": rf.get("dram_frac_from_traffic"), "l2_frac_from_traffic": rf.get("l2_frac_from_traffic"),
                 "schedule_floor_frac": rf["schedule_floor"]["frac_of_hbm_peak"],
                 "kernel_share_of_step": rf["kernel_share_of_step"],
+                # what a step spends outside the traversal launches: seam-accumulator clears + the normalisation kernel
+                "clear_and_normalise_ms": max(0.0, run["ms"] / run["steps"] - run["kernel_ms"]),
                 "working_set_bytes": ws, "l2": "L2 flushed between timed steps" if fl else "working set larger than L2",
             }
             if rr is not None:
@@ -560,7 +575,7 @@ def main():
         cores = host_cores()
         dirs_all = oracle.healpix_dirs(spec.nside)
         val, dt, nd, stride = oracle_rate(oracle, kap, S, dirs_all, max(1, min(spec.ndirs, args.cpu_dirs)), cores, spec.nbins)
-        cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+        cpu = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu_model": cpu_model(),
                "sample": "%d of %d directions (every %dth), full mesh, %.1f s" % (nd, spec.ndirs, stride, dt)}
         n1 = max(1, min(spec.ndirs, args.cpu_dirs // 12))
         v1, dt1, nd1, st1 = oracle_rate(oracle, kap, S, dirs_all, n1, 1, spec.nbins)
