@@ -1,6 +1,8 @@
 """bench.py's reference arm runs on the host (the oracle on a bounded sample) and prints one JSON line with
 the contract's keys; the GPU arm refuses to run without a CUDA device (no CPU fallback)."""
 import json
+
+import numpy as np
 import os
 import subprocess
 import sys
@@ -103,3 +105,30 @@ def test_point_source_instruction_count_names_its_kernel_source():
     t = json.load(open(os.path.join(ROOT, "profiles", "point_sources.json")))
     assert os.path.exists(os.path.join(ROOT, t["kernel_source"])) and os.path.exists(os.path.join(ROOT, t["source"]))
     assert len(t["kernel_source_sha"]) == 40 and 10 < t["thread_instructions_per_ray_step"] < 200
+
+
+def test_sweep_entries_counts_mirror_pairs():
+    """bench.sweep_entries (host logic of the schedule floor): a direction and its mirror image along the
+    memory-contiguous transverse axis are one work entry; directions with a zero slope along that axis run alone."""
+    sys.path.insert(0, ROOT)
+    import bench
+    # records: (dominant axis a, reflection bits x|y<<1|z<<2, Mb, Mc, generic flag, rays); b = y for a = 0, else x
+    rec = np.array([
+        [2, 0b000, 100, 50, 0, 1], [2, 0b001, 100, 50, 0, 1],      # z-dominant, mirrored in x: one pair
+        [2, 0b100, 100, 50, 0, 1],                                  # other march sense: no partner
+        [2, 0b000, 0, 70, 0, 1], [2, 0b001, 0, 70, 0, 1],           # zero slope along b: two singles
+        [0, 0b000, 30, 20, 0, 1], [0, 0b010, 30, 20, 0, 1],         # x-dominant, mirrored in y: one pair
+        [1, 0b000, 30, 20, 0, 1], [1, 0b100, 30, 20, 0, 1],         # y-dominant, c = z reflected: different rows, no pair
+    ], dtype=np.int64)
+    assert bench.sweep_entries(rec) == 1 + 1 + 2 + 1 + 2
+    from oracle import oracle
+    oracle.build()
+    dirs = oracle.healpix_dirs(16)
+    # HEALPix: every direction with a non-zero b-slope has its mirror image in the set (128 of 3072 have none)
+    recs = np.array([[int(np.argmax(np.abs(d))), (d[0] < 0) | ((d[1] < 0) << 1) | ((d[2] < 0) << 2), 0, 0, 0, 1] for d in dirs], dtype=np.int64)
+    for i, d in enumerate(dirs):
+        a = recs[i, 0]
+        b, c = (1 if a == 0 else 0), (1 if a == 2 else 2)
+        recs[i, 2] = round(abs(d[b] / d[a]) * 2 ** 20)
+        recs[i, 3] = round(abs(d[c] / d[a]) * 2 ** 20)
+    assert bench.sweep_entries(recs) == 1594
