@@ -555,6 +555,59 @@ __global__ void k_rates(float *__restrict__ Gamma, float *__restrict__ Heat, con
     }
 }
 
+// k_rates with two adjacent cells per thread and 64 x 64 tiles (see k_finalise_wide): same arithmetic per cell
+__global__ void __launch_bounds__(1024) k_rates_wide(float *__restrict__ Gamma, float *__restrict__ Heat, const float2 *__restrict__ Pnat, int ppN,
+                        const float *__restrict__ accN, const float *__restrict__ accNC, int slotsN,
+                        const float *__restrict__ accT, const float *__restrict__ accTC, int slotsT,
+                        int nx, int ny, int nz, int nxp, int nyp, int nbins, int nbp, float inv_nd, const RateWeights W, int z0)
+{
+    __shared__ double tile[64][65];
+    const int z = (int)blockIdx.z + z0;
+    const int x0 = blockIdx.x * 64, y0 = blockIdx.y * 64;
+    const size_t ncellN = (size_t)nxp * ny * nz, ncellT = (size_t)nyp * nz * nx;
+    const size_t strideN = ncellN * nbins, strideT = ncellT * nbins;
+    const float *__restrict__ fN = reinterpret_cast<const float *>(Pnat);
+    float g[2][2] = {{0.0f, 0.0f}, {0.0f, 0.0f}}, h[2][2] = {{0.0f, 0.0f}, {0.0f, 0.0f}};      // [row ty + 32 j][cell]
+    for (int bin = 0; bin < nbins; ++bin) {
+        for (int dx = threadIdx.y; dx < 64; dx += 32) {
+            const int x = x0 + dx, y = y0 + 2 * (int)threadIdx.x;
+            double s0 = 0.0, s1 = 0.0;
+            if (x < nx && y < ny)
+                sum_slots2(accT, accTC, slotsT, strideT, packed_cell(bin, (size_t)x * nz + z, y, nbp, nyp, (size_t)nz * nx), s0, s1);
+            tile[dx][2 * threadIdx.x] = s0;
+            tile[dx][2 * threadIdx.x + 1] = s1;
+        }
+        __syncthreads();
+        int j = 0;
+        for (int dy = threadIdx.y; dy < 64; dy += 32, ++j) {
+            const int x = x0 + 2 * (int)threadIdx.x, y = y0 + dy;
+            if (x < nx && y < ny) {
+                const size_t ip = packed_cell(bin, (size_t)z * ny + y, x, nbp, nxp, (size_t)ny * nz);
+                double n0, n1;
+                sum_slots2(accN, accNC, slotsN, strideN, ip, n0, n1);
+                const double s0 = tile[2 * threadIdx.x][dy] + n0, s1 = tile[2 * threadIdx.x + 1][dy] + n1;
+                const float4 f = *reinterpret_cast<const float4 *>(fN + 2 * ip);
+                const float k0 = f.x, k1 = ppN ? f.y : f.z, S0 = ppN ? f.z : f.y, S1 = f.w;
+                const float j0 = (float)(s0 * (double)inv_nd) / k0, j1 = (float)(s1 * (double)inv_nd) / k1;
+                g[j][0] = fmaf(W.wG[bin], j0, fmaf(W.lG[bin], S0, g[j][0]));
+                g[j][1] = fmaf(W.wG[bin], j1, fmaf(W.lG[bin], S1, g[j][1]));
+                h[j][0] = fmaf(W.wH[bin], j0, fmaf(W.lH[bin], S0, h[j][0]));
+                h[j][1] = fmaf(W.wH[bin], j1, fmaf(W.lH[bin], S1, h[j][1]));
+            }
+        }
+        __syncthreads();
+    }
+    int j = 0;
+    for (int dy = threadIdx.y; dy < 64; dy += 32, ++j) {
+        const int x = x0 + 2 * (int)threadIdx.x, y = y0 + dy;
+        if (x < nx && y < ny) {
+            const size_t i = ((size_t)z * ny + y) * nx + x;
+            *reinterpret_cast<float2 *>(Gamma + i) = make_float2(g[j][0], g[j][1]);
+            *reinterpret_cast<float2 *>(Heat + i) = make_float2(h[j][0], h[j][1]);
+        }
+    }
+}
+
 cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN, const float *accN, const float *accNC,
                          int slotsN, const float *accT, const float *accTC, int slotsT, int nx, int ny, int nz,
                          int nxp, int nyp, int nbins, int nbp,
@@ -566,7 +619,17 @@ cudaError_t launch_rates(float *Gamma, float *Heat, const float2 *Pnat, int ppN,
         W.wG[b] = in ? w4[b] : 0.0f;             W.lG[b] = in ? w4[nbins + b] : 0.0f;
         W.wH[b] = in ? w4[2 * nbins + b] : 0.0f; W.lH[b] = in ? w4[3 * nbins + b] : 0.0f;
     }
+    const bool wide = nx % 2 == 0 && ny % 2 == 0 && nx >= 128 && ny >= 128 &&
+                      ((reinterpret_cast<uintptr_t>(Gamma) | reinterpret_cast<uintptr_t>(Heat)) & 7u) == 0;
     for (long long z0 = 0; z0 < nz; z0 += kMaxGridZ) {
+        if (wide) {
+            dim3 grid((nx + 63) / 64, (ny + 63) / 64, (unsigned)std::min<long long>(kMaxGridZ, nz - z0)), block(32, 32);
+            k_rates_wide<<<grid, block, 0, st>>>(Gamma, Heat, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT, nx, ny, nz, nxp, nyp,
+                                                nbins, nbp, inv_nd, W, (int)z0);
+            const cudaError_t e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+            continue;
+        }
         dim3 grid((nx + 31) / 32, (ny + 31) / 32, (unsigned)std::min<long long>(kMaxGridZ, nz - z0)), block(32, 8);
         k_rates<<<grid, block, 0, st>>>(Gamma, Heat, Pnat, ppN, accN, accNC, slotsN, accT, accTC, slotsT, nx, ny, nz, nxp, nyp,
                                        nbins, nbp, inv_nd, W, (int)z0);

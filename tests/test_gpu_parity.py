@@ -316,7 +316,8 @@ def test_inflow_cellwidth_multibin(orc):
     check_full(orc, kap, S, dirs, out, ref, cell_width=0.7)
 
 
-@pytest.mark.parametrize("name,dims,nside", [("C5", (64, 32, 48), 2), ("C2", (32, 32, 32), 2), ("C5", (20, 12, 10), 1)])
+@pytest.mark.parametrize("name,dims,nside", [("C5", (64, 32, 48), 2), ("C2", (32, 32, 32), 2), ("C5", (20, 12, 10), 1),
+                                             ("C5", (128, 130, 12), 1), ("C3", (192, 128, 8), 1)])   # the 64 x 64-tile epilogue
 def test_rates_epilogue(orc, name, dims, nside):
     """rt_sweep_rates against the oracle's rates() of the oracle's J_in (eqs. 14-15, 20-23): 1e-5."""
     import paper_1410_0763_b200 as rt
