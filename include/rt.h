@@ -44,6 +44,7 @@ typedef struct rt_ctx rt_ctx;
 #define RT_ENOMEM   -2   /* host or device allocation failed */
 #define RT_ECUDA    -3   /* CUDA runtime error; text via rt_last_cuda_error() */
 #define RT_ESTATE   -4   /* call order: e.g. rt_sweep before rt_set_fields */
+#define RT_ELIMIT   -5   /* size beyond the fixed capacity of an entry point that never allocates (RT_STATIC_MAX_*) */
 
 /* rt_create flags */
 #define RT_OWNED            0u   /* default: atomic-free, one writer per cell (ownership + seam accumulators) */
@@ -195,6 +196,41 @@ int rt_point_sources(rt_ctx *ctx, const int *src_fix_host, const double *lum_hos
 int rt_point_source_rates(rt_ctx *ctx, const float *Q_dev, const float *kappa_sp_dev, const float *n_sp_dev, int nspecies,
                           const double *hnu_host, const double *hnu_thr_host, float *Gamma_dev, float *Heat_dev,
                           void *cuda_stream);
+
+/*
+ * rt_point_sources for callers that cannot allocate device memory: no context, no cudaMalloc / cudaFree /
+ * cudaMallocHost, no allocating library routine, on any call.
+ *
+ * Who needs it: a simulation code that claimed (nearly) all of the GPU's memory for its own arena at start-up, code
+ * running under a framework's caching allocator, a GPU shared through MPS with a per-client memory limit, or the
+ * inside of a time step where the device-wide synchronisation of cudaMalloc / cudaFree would stall the other streams.
+ * For them rt_create + rt_set_fields + rt_point_sources is unusable: those allocate tables, packed copies of the
+ * fields and a pinned staging buffer.  Here the caller passes kappa and the outputs, and the only other memory the
+ * kernel needs -- a device copy of the source tables and the counter of marched ray pieces -- is a fixed array of
+ * 143,616 bytes inside the library image (a file-scope __device__ array in csrc/rt_static.cu).  Every GPU on which
+ * the process uses this library holds that array from the moment the library's code is loaded there until exit.
+ *
+ * Same operation, argument meaning and units as rt_point_sources (eqs. A1-A3), except:
+ *   nx, ny, nz, nbins, cell_width : the mesh (each dimension <= 1024, nx*ny*nz < 2^31), as rt_create would take them
+ *   kappa_dev : DEVICE, fp32 [nbins][nz][ny][nx], read in place (kappa below 2^-60 counts as 2^-60, as in the packed copy);
+ *               must stay valid and unchanged until the enqueued kernel has run
+ *   src_fix_host, lum_host, nsrc, Q_dev, diag_src, diag_bin, tau_dev, steps_host : as rt_point_sources
+ * Capacity: nsrc <= RT_STATIC_MAX_SOURCES and nbins <= RT_STATIC_MAX_BINS; larger -> RT_ELIMIT and nothing is
+ * enqueued (use rt_point_sources, or split the sources over several calls and add the Q arrays).
+ * Device: the CUDA device current at the call; the pointers must belong to it.
+ * First call on a device: looks up the device address of the array (cudaGetSymbolAddress; this is also when the CUDA
+ * runtime loads the kernel's module on that device).  Make this first call before any stream capture begins.
+ * Sharing: all calls on a device use the one array.  Each call clears the counter and overwrites the tables on
+ * `cuda_stream`, so the array never carries state from one call into the next, but two calls whose GPU work overlaps
+ * (different streams without an event between them, or two host threads) race on it and give undefined Q.
+ * Asynchronous on `cuda_stream` apart from the staging of the two small pageable host tables (they may be reused when
+ * the call returns); a call with steps_host != NULL synchronises the stream.
+ */
+#define RT_STATIC_MAX_SOURCES 1024
+#define RT_STATIC_MAX_BINS    16
+int rt_point_sources_static(int nx, int ny, int nz, int nbins, double cell_width, const float *kappa_dev,
+                            const int *src_fix_host, const double *lum_host, int nsrc, float *Q_dev,
+                            int diag_src, int diag_bin, float *tau_dev, unsigned long long *steps_host, void *cuda_stream);
 
 /*
  * Diagnostics required by the parity gates (integer traversal data, summed ds).  They run the same

@@ -10,9 +10,11 @@ from . import build as _build
 
 RT_OWNED, RT_ATOMIC_ABLATION, RT_PAPER_GROUPS = 0, 1, 2
 RT_J_IN, RT_J_TOTAL, RT_SUM_IN = 0, 1, 2
+RT_ELIMIT = -5
+RT_STATIC_MAX_SOURCES, RT_STATIC_MAX_BINS = 1024, 16
 
 EXPORTED_SYMBOLS = [
-    "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_set_inflow_faces", "rt_sweep", "rt_combine", "rt_sweep_rates", "rt_point_sources", "rt_point_source_rates", "rt_segment_counts",
+    "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_set_inflow_faces", "rt_sweep", "rt_combine", "rt_sweep_rates", "rt_point_sources", "rt_point_sources_static", "rt_point_source_rates", "rt_segment_counts",
     "rt_sum_ds", "rt_total_segments", "rt_debug_writer_counts", "rt_working_set_bytes", "rt_probe_bandwidth", "rt_direction_records", "rt_tune", "rt_last_launch_count",
     "rt_last_sweep_kernel_ms", "rt_destroy", "rt_strerror", "rt_last_cuda_error",
 ]
@@ -57,6 +59,9 @@ def load_library():
     L.rt_sweep_rates.restype = C.c_int
     L.rt_point_sources.argtypes = [vp, C.POINTER(C.c_int), dp, C.c_int, vp, C.c_int, C.c_int, vp, C.POINTER(C.c_ulonglong), vp]
     L.rt_point_sources.restype = C.c_int
+    L.rt_point_sources_static.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, vp, C.POINTER(C.c_int), dp, C.c_int, vp,
+                                          C.c_int, C.c_int, vp, C.POINTER(C.c_ulonglong), vp]
+    L.rt_point_sources_static.restype = C.c_int
     L.rt_point_source_rates.argtypes = [vp, vp, vp, vp, C.c_int, dp, dp, vp, vp, vp]
     L.rt_point_source_rates.restype = C.c_int
     L.rt_segment_counts.argtypes = [vp, C.c_int, vp, vp]
@@ -183,6 +188,28 @@ def rt_point_sources(h, src_fix, lum, Q, numel, nbins, tau=None, diag=(0, 0), wa
                                            src.shape[0], _dev_ptr(Q, torch.float32, numel, "Q"), int(diag[0]), int(diag[1]),
                                            None if tau is None else _dev_ptr(tau, torch.float32, numel // nbins, "tau"),
                                            C.byref(steps) if want_steps else None, _stream(stream)), "rt_point_sources")
+    return int(steps.value)
+
+
+def rt_point_sources_static(dims, nbins, kappa, src_fix, lum, Q, cell_width=1.0, tau=None, diag=(0, 0), want_steps=False, stream=None):
+    """rt_point_sources_static: rt_point_sources without a context and without any allocation by the library, for
+    callers whose device memory is spoken for (an arena that owns the GPU, a caching allocator, an MPS memory limit)
+    or that cannot afford cudaMalloc's device-wide synchronisation.  kappa, Q (and tau) are the caller's CUDA tensors
+    on the current device; the source tables go through a fixed 143,616-byte device array inside librt.so, which caps
+    the call at RT_STATIC_MAX_SOURCES sources and RT_STATIC_MAX_BINS bins (RtError with code RT_ELIMIT beyond).  All
+    calls on a device share that array: do not let two of them overlap on the GPU.  Returns the step count (0 unless
+    want_steps)."""
+    import torch
+    nx, ny, nz = (int(v) for v in dims)
+    numel = nx * ny * nz * int(nbins)
+    src = np.ascontiguousarray(src_fix, dtype=np.int32).reshape(-1, 3)
+    lum = np.ascontiguousarray(lum, dtype=np.float64).reshape(src.shape[0], nbins)
+    steps = C.c_ulonglong(0)
+    _check(load_library().rt_point_sources_static(nx, ny, nz, int(nbins), float(cell_width), _dev_ptr(kappa, torch.float32, numel, "kappa"),
+                                                  src.ctypes.data_as(C.POINTER(C.c_int)), lum.ctypes.data_as(C.POINTER(C.c_double)),
+                                                  src.shape[0], _dev_ptr(Q, torch.float32, numel, "Q"), int(diag[0]), int(diag[1]),
+                                                  None if tau is None else _dev_ptr(tau, torch.float32, numel // nbins, "tau"),
+                                                  C.byref(steps) if want_steps else None, _stream(stream)), "rt_point_sources_static")
     return int(steps.value)
 
 

@@ -9,7 +9,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "librt.so")
 SOURCES = ["rt_sweep_nb256.cu", "rt_sweep_nb512.cu", "rt_sweep_nb128.cu", "rt_sweep_nb128x3.cu", "rt_sweep_nb64.cu", "rt_sweep_nb64x3.cu",
-           "rt_sweep_nb32.cu", "rt_sweep_nb32x3.cu", "rt_api.cu", "rt_kernels.cu"]
+           "rt_sweep_nb32.cu", "rt_sweep_nb32x3.cu", "rt_api.cu", "rt_kernels.cu", "rt_static.cu"]
 HEADERS = [os.path.join(CSRC, "rt_internal.h"), os.path.join(CSRC, "rt_sweep.cuh"), os.path.join(os.path.dirname(_HERE), "include", "rt.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-cudart", "static"]

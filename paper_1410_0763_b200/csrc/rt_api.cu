@@ -24,6 +24,7 @@ static int cuda_fail(cudaError_t e)
     return RT_ECUDA;
 }
 #define CK(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return cuda_fail(e__); } while (0)
+int rt::api_cuda_fail(cudaError_t e) { return cuda_fail(e); }
 
 // Every entry point that takes a context makes the context's device current for the duration of the call (a
 // process that drives several GPUs may have switched devices since rt_create) and restores the caller's.
@@ -131,6 +132,7 @@ extern "C" const char *rt_strerror(int code)
     case RT_ENOMEM: return "out of memory";
     case RT_ECUDA: return "CUDA error";
     case RT_ESTATE: return "call order error";
+    case RT_ELIMIT: return "size beyond the fixed capacity of a no-allocation entry point (RT_STATIC_MAX_*)";
     }
     return "unknown error";
 }

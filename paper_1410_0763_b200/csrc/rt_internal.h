@@ -137,6 +137,9 @@ cudaError_t launch_sum_u32(unsigned long long *out, const unsigned *counts, long
 // writer counts of one launch in MODE_OWNERS: out2[0] = max(out2[0], max_i w[i]), out2[1] += sum_i w[i] over n floats
 cudaError_t launch_owner_reduce(unsigned long long *out2, const float *w, long long n, cudaStream_t st);
 
+// records the text of a CUDA error for rt_last_cuda_error() and returns RT_ECUDA (rt_api.cu; for rt_static.cu)
+int api_cuda_fail(cudaError_t e);
+
 // `reps` passes of the streaming probe over n4 float4 in one launch (rmw = 0: read, 1: read-modify-write)
 cudaError_t launch_probe(float4 *buf, size_t n4, int rmw, int reps, int sm_count, cudaStream_t st);
 
