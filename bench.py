@@ -380,6 +380,7 @@ class Runner:
         clocks = sampler.stop() if sampler else None
         kernel_ms = tr.last_sweep_kernel_ms()          # traversal launches of the last timed sweep (library-side CUDA events)
         launches = tr.last_launch_count()
+        graph = tr.last_sweep_was_graph()              # one CUDA-graph replay: kernel_ms then spans the normalisation kernel too
         ms = self.max_over_ranks(ms)
         jobs = 1 if self.sharded else self.world       # replicas: every rank sweeps the whole set
         value = jobs * self.updates * steps / (ms * 1e-3)
@@ -410,12 +411,14 @@ class Runner:
 
         # ---- roofline of the dominant kernel (k_sweep_tma): SURVEY.md 8(d)'s 16 B per cell-direction-bin
         n_sweep_launches = max(1, launches - 1)                             # minus the normalise kernel
+        # (a graph replay is timed as a whole: the normalisation kernel's time is then charged to the traversal launches,
+        # which under-states `achieved`; roofline.timed_interval says which interval it was)
         avg_launch_ms = kernel_ms / n_sweep_launches
         bytes_per_launch = ALGO_BYTES_PER_CELL_DIR_BIN * self.cell_dir_bins / n_sweep_launches
         achieved = bytes_per_launch / (avg_launch_ms * 1e-3) / 1e9
         return {"ms": ms, "steps": steps, "value": value, "e2e": e2e, "clocks": clocks, "launches": launches,
                 "floor_bytes": 8.0 * self.spec.ncell * self.spec.nbins * self.entries, "entries": self.entries,
-                "kernel_ms": kernel_ms, "n_sweep_launches": n_sweep_launches, "avg_launch_ms": avg_launch_ms,
+                "kernel_ms": kernel_ms, "graph_replay": graph, "n_sweep_launches": n_sweep_launches, "avg_launch_ms": avg_launch_ms,
                 "bytes_per_launch": bytes_per_launch, "achieved": achieved}
 
     def close(self):
@@ -437,6 +440,8 @@ def roofline_of(r, name, run, peaks, default_tuning):
            "launches_per_step": run["n_sweep_launches"], "avg_launch_ms": run["avg_launch_ms"],
            "algorithmic_bytes_per_launch": run["bytes_per_launch"],
            "kernel_share_of_step": run["kernel_ms"] / (run["ms"] / run["steps"]),
+           "timed_interval": "whole sweep replayed as one CUDA graph (traversal + normalisation kernels)" if run.get("graph_replay")
+                             else "traversal launches only (library-side CUDA events around them)",
            "frac_of_hbm_peak": run["achieved"] / hbm_peak,
            "note": "a mirror pair of directions shares every field load and accumulator read-modify-write, and the entries "
                    "of a launch find the fields in L2, so the 16-byte model is no upper bound on this schedule and frac "
@@ -557,7 +562,9 @@ def main():
                 "schedule_floor_frac": rf["schedule_floor"]["frac_of_hbm_peak"],
                 "kernel_share_of_step": rf["kernel_share_of_step"],
                 # what a step spends outside the traversal launches: seam-accumulator clears + the normalisation kernel
-                "clear_and_normalise_ms": max(0.0, run["ms"] / run["steps"] - run["kernel_ms"]),
+                # (not separable when the sweep is one graph replay)
+                "clear_and_normalise_ms": None if run.get("graph_replay") else max(0.0, run["ms"] / run["steps"] - run["kernel_ms"]),
+                "graph_replay": bool(run.get("graph_replay")),
                 "working_set_bytes": ws, "l2": "L2 flushed between timed steps" if fl else "working set larger than L2",
             }
             if rr is not None:

@@ -111,6 +111,17 @@ int rt_set_inflow(rt_ctx *ctx, const float *I_bc_host);
 int rt_set_inflow_faces(rt_ctx *ctx, const float *I_face_host);
 
 /*
+ * The same two updates without the device-wide synchronisation: enqueued on `cuda_stream` like every other call, for a
+ * boundary illumination that changes every iteration next to work on other streams.  The values
+ * travel in the parameters of a one-block kernel (no staging buffer): the host array may be reused as soon as the call
+ * returns.  Ordering is the stream's: sweeps enqueued later on `cuda_stream` (CUDA-graph replays included) use the new
+ * values, sweeps enqueued earlier on it the old ones; with respect to sweeps of this context on OTHER streams the
+ * caller orders the update with events, as for any device buffer.  Arguments and value checks as above.
+ */
+int rt_set_inflow_async(rt_ctx *ctx, const float *I_bc_host, void *cuda_stream);
+int rt_set_inflow_faces_async(rt_ctx *ctx, const float *I_face_host, void *cuda_stream);
+
+/*
  * One full sweep over all directions ("one iteration" of PAPER.md:322).
  *   J_dev : DEVICE, fp32 [nbins][nz][ny][nx], caller-owned, fully overwritten
  *   what  : RT_J_IN, RT_J_TOTAL or RT_SUM_IN
@@ -318,8 +329,13 @@ int rt_probe_bandwidth(unsigned long long bytes, int mode, int iters, double *gb
 int rt_last_launch_count(rt_ctx *ctx);
 
 /* Time of the last rt_sweep's traversal kernels only, in ms (cudaEvents on the sweep's stream);
-   synchronises on those events.  Negative if unavailable. */
+   synchronises on those events.  When that sweep was replayed as one CUDA graph (rt_tune "graph"; see
+   rt_last_sweep_was_graph) the interval is the whole sweep, normalisation kernel included.  Negative if unavailable,
+   e.g. when the caller's stream was being captured (no timing events are recorded into a caller's graph). */
 float rt_last_sweep_kernel_ms(rt_ctx *ctx);
+
+/* 1 if the last rt_sweep of this context was replayed as one CUDA graph, 0 if its kernels were launched one by one. */
+int rt_last_sweep_was_graph(rt_ctx *ctx);
 
 /* Free everything the context owns.  Synchronises the device.  NULL is allowed. */
 int rt_destroy(rt_ctx *ctx);

@@ -14,9 +14,9 @@ RT_ELIMIT = -5
 RT_STATIC_MAX_SOURCES, RT_STATIC_MAX_BINS = 1024, 16
 
 EXPORTED_SYMBOLS = [
-    "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_set_inflow_faces", "rt_sweep", "rt_combine", "rt_sweep_rates", "rt_point_sources", "rt_point_sources_static", "rt_point_source_rates", "rt_segment_counts",
+    "rt_healpix_dirs", "rt_create", "rt_set_fields", "rt_set_inflow", "rt_set_inflow_faces", "rt_set_inflow_async", "rt_set_inflow_faces_async", "rt_sweep", "rt_combine", "rt_sweep_rates", "rt_point_sources", "rt_point_sources_static", "rt_point_source_rates", "rt_segment_counts",
     "rt_sum_ds", "rt_total_segments", "rt_debug_writer_counts", "rt_working_set_bytes", "rt_probe_bandwidth", "rt_direction_records", "rt_tune", "rt_last_launch_count",
-    "rt_last_sweep_kernel_ms", "rt_destroy", "rt_strerror", "rt_last_cuda_error",
+    "rt_last_sweep_kernel_ms", "rt_last_sweep_was_graph", "rt_destroy", "rt_strerror", "rt_last_cuda_error",
 ]
 
 _lib = None
@@ -51,6 +51,10 @@ def load_library():
     L.rt_set_inflow.restype = C.c_int
     L.rt_set_inflow_faces.argtypes = [vp, fp]
     L.rt_set_inflow_faces.restype = C.c_int
+    L.rt_set_inflow_async.argtypes = [vp, fp, vp]
+    L.rt_set_inflow_async.restype = C.c_int
+    L.rt_set_inflow_faces_async.argtypes = [vp, fp, vp]
+    L.rt_set_inflow_faces_async.restype = C.c_int
     L.rt_sweep.argtypes = [vp, vp, C.c_uint, vp]
     L.rt_sweep.restype = C.c_int
     L.rt_combine.argtypes = [vp, vp, C.c_longlong, C.c_uint, vp, vp]
@@ -84,6 +88,8 @@ def load_library():
     L.rt_last_launch_count.restype = C.c_int
     L.rt_last_sweep_kernel_ms.argtypes = [vp]
     L.rt_last_sweep_kernel_ms.restype = C.c_float
+    L.rt_last_sweep_was_graph.argtypes = [vp]
+    L.rt_last_sweep_was_graph.restype = C.c_int
     L.rt_destroy.argtypes = [vp]
     L.rt_destroy.restype = C.c_int
     L.rt_strerror.argtypes = [C.c_int]
@@ -155,6 +161,18 @@ def rt_set_inflow_faces(h, I_face, nbins):
     if a.shape[0] != 6 * nbins:
         raise ValueError("I_face must be [nbins][6]")
     _check(load_library().rt_set_inflow_faces(h, a.ctypes.data_as(C.POINTER(C.c_float))), "rt_set_inflow_faces")
+
+
+def rt_set_inflow_async(h, Ibc, stream=None):
+    a = np.ascontiguousarray(Ibc, dtype=np.float32)
+    _check(load_library().rt_set_inflow_async(h, a.ctypes.data_as(C.POINTER(C.c_float)), _stream(stream)), "rt_set_inflow_async")
+
+
+def rt_set_inflow_faces_async(h, I_face, nbins, stream=None):
+    a = np.ascontiguousarray(I_face, dtype=np.float32).reshape(-1)
+    if a.shape[0] != 6 * nbins:
+        raise ValueError("I_face must be [nbins][6]")
+    _check(load_library().rt_set_inflow_faces_async(h, a.ctypes.data_as(C.POINTER(C.c_float)), _stream(stream)), "rt_set_inflow_faces_async")
 
 
 def rt_sweep(h, J, numel, what=RT_J_IN, stream=None):
@@ -315,6 +333,14 @@ class RayTracer:
     def set_inflow_faces(self, I_face):
         rt_set_inflow_faces(self.h, I_face, self.nbins)
 
+    def set_inflow_async(self, Ibc, stream=None):
+        if np.asarray(Ibc).reshape(-1).shape[0] != self.nbins:
+            raise ValueError("Ibc must have one value per bin")
+        rt_set_inflow_async(self.h, Ibc, stream)
+
+    def set_inflow_faces_async(self, I_face, stream=None):
+        rt_set_inflow_faces_async(self.h, I_face, self.nbins, stream)
+
     def sweep(self, out=None, what=RT_J_IN, stream=None):
         import torch
         if out is None:
@@ -380,6 +406,9 @@ class RayTracer:
 
     def last_sweep_kernel_ms(self) -> float:
         return float(load_library().rt_last_sweep_kernel_ms(self.h))
+
+    def last_sweep_was_graph(self) -> bool:
+        return int(load_library().rt_last_sweep_was_graph(self.h)) == 1
 
     def close(self):
         if self.h is not None:

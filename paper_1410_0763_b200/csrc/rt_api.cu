@@ -97,6 +97,7 @@ struct rt_ctx {
     int last_launches = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     bool ev_valid = false;
+    bool last_graph = false;         // the last rt_sweep was a CUDA-graph replay: ev0 / ev1 then bracket the whole sweep
     // overlapped schedule (small meshes): every class of directions (layout, dominant axis, pairs / singles, march
     // sense along b) has its own slot range and runs on its own internal stream ("lane"), so that the classes of a
     // sweep that does not fill the machine run side by side instead of one short launch after the other
@@ -119,7 +120,8 @@ struct rt_ctx {
     size_t src_cap = 0;
     int src_n = 0;
     bool src_valid = false, src_copy_pending = false;
-    cudaEvent_t ev_src = nullptr;
+    cudaEvent_t ev_src = nullptr;    // recorded after the copy into d_src: later calls on any stream wait on it before they read the tables
+    std::map<cudaStream_t, cudaEvent_t> src_readers;   // per stream: recorded after its last kernel that reads d_src (a new copy waits on all)
     long long seg_total = -1;        // rt_total_segments: the geometry never changes, so the count is taken once
     unsigned long long *d_own = nullptr;   // [4] rt_debug_writer_counts: {max, sum} of acc, {max, sum} of accC
 };
@@ -184,6 +186,8 @@ static void free_device(rt_ctx *c)
     cudaFree(c->d_src);
     if (c->src_stage) cudaFreeHost(c->src_stage);
     if (c->ev_src) cudaEventDestroy(c->ev_src);
+    for (auto &kv : c->src_readers) cudaEventDestroy(kv.second);
+    c->src_readers.clear();
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
 }
 
@@ -475,8 +479,23 @@ static int ensure_buffers(rt_ctx *c)
         bool ok = true;
         for (int l = 0; l < 2; ++l)
             if (!c->order[l].empty() && !(c->fast[l] && c->pitch[l] <= 128)) ok = false;
+        // the packed kernel addresses a row's three bins with 32-bit element offsets scaled by 3 (rt_sweep.cuh):
+        // larger layouts stay on bins-as-planes
+        for (int l = 0; l < 2; ++l)
+            if (3 * c->ncell_l[l] >= (1ll << 31)) ok = false;
         if (ok) c->nbp = 3;
     }
+    // every layout that is swept by the owned kernel must have an instantiation for the rows / stages chosen with
+    // rt_tune (e.g. a ring of 4 stages exists only for rows of <= 64 cells): refuse here, before anything is
+    // allocated, so that the caller can still correct the knob
+    if (c->flags == RT_OWNED)
+        for (int l = 0; l < 2; ++l) {
+            if (c->order[l].empty() || !c->fast[l]) continue;
+            const int rows = rows_for(c, l), stages = stages_for(c, l);
+            if (owned_ctas_per_sm(c->pitch[l], rows, stages, false, c->nbp) < 1 ||
+                (c->pair_enable && owned_ctas_per_sm(c->pitch[l], rows, stages, true, c->nbp) < 1))
+                return RT_EINVAL;
+        }
     const size_t field_bytes_l[2] = {sizeof(float2) * (size_t)c->ncell_l[0] * c->nbins, sizeof(float2) * (size_t)c->ncell_l[1] * c->nbins};
     const size_t acc_bytes_l[2] = {sizeof(float) * (size_t)c->ncell_l[0] * c->nbins, sizeof(float) * (size_t)c->ncell_l[1] * c->nbins};
     size_t freeb = 0, totalb = 0;
@@ -616,6 +635,46 @@ extern "C" int rt_set_inflow_faces(rt_ctx *c, const float *I_face_host)
     CK(cudaDeviceSynchronize());        // sweeps in flight on any stream still read the old values
     CK(cudaMemcpy(c->d_Ibc, I_face_host, sizeof(float) * 6 * c->nbins, cudaMemcpyHostToDevice));
     return RT_OK;
+}
+
+// Stream-ordered inflow update: the table (at most 16 bins x 6 faces) travels in the kernel's parameters, so there is no
+// staging buffer to guard, nothing to synchronise and the caller's array is free when the call returns.
+struct InflowTable { float v[6 * 16]; };
+__global__ void k_set_inflow(float *__restrict__ Ibc, const InflowTable t, int n)
+{
+    const int i = threadIdx.x;
+    if (i < n) Ibc[i] = t.v[i];
+}
+
+static int enqueue_inflow(rt_ctx *c, const InflowTable &t, cudaStream_t st)
+{
+    k_set_inflow<<<1, 6 * 16, 0, st>>>(c->d_Ibc, t, 6 * c->nbins);
+    CK(cudaGetLastError());
+    return RT_OK;
+}
+
+extern "C" int rt_set_inflow_async(rt_ctx *c, const float *I_bc_host, void *stream)
+{
+    if (!c || !I_bc_host) return RT_EINVAL;
+    DevGuard dev_guard(c->device);
+    InflowTable t = {};
+    for (int b = 0; b < c->nbins; ++b) {
+        if (!(I_bc_host[b] >= 0.0f) || !std::isfinite(I_bc_host[b])) return RT_EINVAL;
+        for (int f = 0; f < 6; ++f) t.v[6 * b + f] = I_bc_host[b];
+    }
+    return enqueue_inflow(c, t, (cudaStream_t)stream);
+}
+
+extern "C" int rt_set_inflow_faces_async(rt_ctx *c, const float *I_face_host, void *stream)
+{
+    if (!c || !I_face_host) return RT_EINVAL;
+    DevGuard dev_guard(c->device);
+    InflowTable t = {};
+    for (int i = 0; i < 6 * c->nbins; ++i) {
+        if (!(I_face_host[i] >= 0.0f) || !std::isfinite(I_face_host[i])) return RT_EINVAL;
+        t.v[i] = I_face_host[i];
+    }
+    return enqueue_inflow(c, t, (cudaStream_t)stream);
 }
 
 // Enqueue the traversal in `mode` of all directions (only_dir < 0) or of one direction (slot 0 of
@@ -856,8 +915,15 @@ extern "C" int rt_sweep(rt_ctx *c, float *J_dev, unsigned what, void *stream)
     // combination is replayed as one CUDA graph (captured on an internal stream, launched into the caller's).
     const bool want_graph = c->graph == 1 || (c->graph == -1 && c->overlap_on && c->tiny);
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
-    if (want_graph && st != nullptr && st != cudaStreamLegacy && st != cudaStreamPerThread) CK(cudaStreamIsCapturing(st, &cap));
-    if (want_graph && cap == cudaStreamCaptureStatusNone) {
+    if (st != nullptr && st != cudaStreamLegacy && st != cudaStreamPerThread) CK(cudaStreamIsCapturing(st, &cap));
+    c->last_graph = false;
+    if (cap != cudaStreamCaptureStatusNone) {
+        // the caller is capturing this stream: timing events recorded now would become nodes of the caller's graph and
+        // could never be read back, so none are recorded and rt_last_sweep_kernel_ms reports "unavailable"
+        c->ev_valid = false;
+        return enqueue_sweep(c, J_dev, what, st, false);
+    }
+    if (want_graph) {
         if (!c->cap_stream) CK(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
         rt_ctx::SweepGraph *g = nullptr;
         for (auto &e : c->graphs) if (e.J == J_dev && e.what == what) g = &e;
@@ -887,6 +953,7 @@ extern "C" int rt_sweep(rt_ctx *c, float *J_dev, unsigned what, void *stream)
             CK(cudaGraphLaunch(g->exec, st));
             CK(cudaEventRecord(c->ev1, st));
             c->ev_valid = true;                                   // here the events bracket the whole sweep, normalisation included
+            c->last_graph = true;
             return RT_OK;
         }
     }
@@ -936,7 +1003,10 @@ static int upload_sources(rt_ctx *c, const int *src_fix_host, const float *lum, 
     const size_t bytes = sizeof(int) * nsrc3 + sizeof(float) * nlum;
     if (c->src_valid && c->src_n == nsrc && !memcmp(c->src_stage, src_fix_host, sizeof(int) * nsrc3) &&
         !memcmp(c->src_stage + sizeof(int) * nsrc3, lum, sizeof(float) * nlum))
-        return RT_OK;                                            // same sources as last time: the device tables stand
+    {                                                            // same sources as last time: the device tables stand, but the
+        if (c->ev_src) CK(cudaStreamWaitEvent(st, c->ev_src, 0));  // copy that filled them may be in flight on another stream
+        return RT_OK;
+    }
     if (c->src_copy_pending) { CK(cudaEventSynchronize(c->ev_src)); c->src_copy_pending = false; }   // staging buffer still being read
     if (bytes > c->src_cap) {
         CK(cudaDeviceSynchronize());                             // kernels in flight may still read the old tables
@@ -950,12 +1020,32 @@ static int upload_sources(rt_ctx *c, const int *src_fix_host, const float *lum, 
         c->src_cap = cap;
         if (!c->ev_src) CK(cudaEventCreateWithFlags(&c->ev_src, cudaEventDisableTiming));
     }
+    // kernels of earlier calls, on whatever stream they ran, may still be reading the tables this copy overwrites
+    for (auto &kv : c->src_readers)
+        if (kv.first != st) CK(cudaStreamWaitEvent(st, kv.second, 0));
     memcpy(c->src_stage, src_fix_host, sizeof(int) * nsrc3);
     memcpy(c->src_stage + sizeof(int) * nsrc3, lum, sizeof(float) * nlum);
     CK(cudaMemcpyAsync(c->d_src, c->src_stage, bytes, cudaMemcpyHostToDevice, st));
     CK(cudaEventRecord(c->ev_src, st));
     c->src_copy_pending = true;
     c->src_n = nsrc; c->src_valid = true;
+    return RT_OK;
+}
+
+// Remember that a kernel reading d_src has been enqueued on `st` (one event per stream, re-recorded by every call).
+static int note_source_reader(rt_ctx *c, cudaStream_t st)
+{
+    auto it = c->src_readers.find(st);
+    if (it == c->src_readers.end()) {
+        if (c->src_readers.size() >= 64) {                       // a caller cycling through many streams: wait for all readers once, start over
+            for (auto &kv : c->src_readers) { cudaEventSynchronize(kv.second); cudaEventDestroy(kv.second); }
+            c->src_readers.clear();
+        }
+        cudaEvent_t ev = nullptr;
+        CK(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        it = c->src_readers.emplace(st, ev).first;
+    }
+    CK(cudaEventRecord(it->second, st));
     return RT_OK;
 }
 
@@ -986,6 +1076,8 @@ extern "C" int rt_point_sources(rt_ctx *c, const int *src_fix_host, const double
     if (steps_host) CK(cudaMemsetAsync(c->d_u64, 0, sizeof(unsigned long long), st));
     CK(launch_point_sources(Q_dev, tau_dev, c->d_P[0], c->pp[0], c->nx, c->ny, c->nz, c->pitch[0], d_src, d_lum, nsrc,
                             c->nbins, c->nbp, (float)c->cell_width, diag_src, diag_bin, steps_host ? c->d_u64 : nullptr, st));
+    rc = note_source_reader(c, st);
+    if (rc != RT_OK) return rc;
     c->last_launches = 1;
     if (steps_host) {                                            // the one synchronising variant: the count comes back to the host
         CK(cudaMemcpyAsync(steps_host, c->d_u64, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
@@ -1191,6 +1283,8 @@ extern "C" int rt_probe_bandwidth(unsigned long long bytes, int mode, int iters,
 }
 
 extern "C" int rt_last_launch_count(rt_ctx *c) { return c ? c->last_launches : RT_EINVAL; }
+
+extern "C" int rt_last_sweep_was_graph(rt_ctx *c) { return c ? (c->last_graph ? 1 : 0) : RT_EINVAL; }
 
 extern "C" float rt_last_sweep_kernel_ms(rt_ctx *c)
 {

@@ -486,6 +486,29 @@ def test_error_codes():
         rt.rt_destroy(h)
 
 
+def test_unsupported_tuning_is_refused_before_allocation(orc):
+    """A ring of 4 TMA stages exists only for rows of <= 64 cells.  On 128-cell rows rt_set_fields refuses it with
+    RT_EINVAL before any buffer exists, so that rt_tune can still correct the knob and the context then sweeps as usual."""
+    import paper_1410_0763_b200 as rt
+    torch = _torch()
+    dims = (128, 16, 8)
+    kap, S = _rand(dims, 5)
+    dirs = rt.healpix_dirs(1)
+    tr = rt.RayTracer(dims, 1, dirs, stages=4)
+    try:
+        kd, sd = torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda()
+        with pytest.raises(rt.RtError) as ei:
+            tr.set_fields(kd, sd)
+        assert ei.value.code == -1
+        rt.rt_tune(tr.h, "stages", 2)                   # still allowed: nothing was allocated
+        tr.set_fields(kd, sd)
+        Jin = tr.sweep(what=rt.RT_J_IN).cpu().numpy()
+    finally:
+        tr.close()
+    ref = orc.sweep(kap, S, dirs)
+    assert rel_err(Jin, ref["Jin"]).max() <= J_TOL
+
+
 @pytest.mark.parametrize("tune", [{"overlap": 0}, {"overlap": 1, "graph": 0}, {"overlap": 1, "graph": 1}, {"overlap": 1, "wave_div": 4},
                                   {"overlap": 0, "graph": 1}])
 def test_schedules_agree(orc, tune):
@@ -524,6 +547,49 @@ def test_schedules_agree(orc, tune):
     assert rel_err(Jtot, ref["J"]).max() <= J_TOL
     ref2 = orc.sweep(kap2, S, dirs, Ibc=[0.2, 0.0, 0.1], want_counts=False)
     assert rel_err(again, ref2["Jin"]).max() <= J_TOL
+
+
+@pytest.mark.parametrize("tune", [{"overlap": 1, "graph": 1}, {"overlap": 0, "graph": 0}])
+def test_async_inflow_between_sweeps_on_a_side_stream(orc, tune):
+    """rt_set_inflow_faces_async / rt_set_inflow_async are ordered by the stream they are enqueued on, with no device
+    synchronisation (a boundary illumination that changes every iteration): sweeps, inflow updates and
+    more sweeps (CUDA-graph replays when the graph is on) are all enqueued on a side stream before the host waits once;
+    every sweep must carry the inflow that was current at its place in the stream."""
+    import paper_1410_0763_b200 as rt
+    torch = _torch()
+    dims = (64, 32, 16)
+    kap, S = _rand(dims, 41, nb=2)
+    kap *= 0.2                                           # thin enough that the inflow reaches every cell
+    dirs = orc.healpix_dirs(2)
+    faces = np.array([[0.1, 0.9, 0.3, 0.7, 0.5, 0.2], [1.5, 0.0, 0.0, 2.5, 0.25, 0.75]])
+    tr = rt.RayTracer(dims, 2, dirs, tune=tune)
+    try:
+        tr.set_fields(torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda())
+        torch.cuda.synchronize()
+        st = torch.cuda.Stream()
+        out = torch.empty(tr.shape(), dtype=torch.float32, device="cuda")
+        got = []
+        with torch.cuda.stream(st):
+            for _ in range(3):                           # inflow 0; from the second use on a graph replay
+                tr.sweep(out=out, stream=st)
+            got.append(out.clone())
+            tr.set_inflow_faces_async(faces, stream=st)
+            for _ in range(2):
+                tr.sweep(out=out, stream=st)
+            got.append(out.clone())
+            tr.set_inflow_async([0.4, 0.0], stream=st)
+            tr.sweep(out=out, stream=st)
+            got.append(out.clone())
+        st.synchronize()
+        got = [g.cpu().numpy() for g in got]
+        with pytest.raises(rt.RtError):
+            tr.set_inflow_async([-1.0, 0.0])
+    finally:
+        tr.close()
+    refs = [orc.sweep(kap, S, dirs, want_counts=False), orc.sweep(kap, S, dirs, Ibc_faces=faces, want_counts=False),
+            orc.sweep(kap, S, dirs, Ibc=[0.4, 0.0], want_counts=False)]
+    for g, r in zip(got, refs):
+        assert rel_err(g, r["Jin"]).max() <= J_TOL
 
 
 @pytest.mark.parametrize("dims,nb,rows,rays,nside", [

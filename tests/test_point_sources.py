@@ -229,6 +229,44 @@ def test_point_sources_parity(orc, dims, nb, cw):
 
 
 @pytest.mark.gpu
+def test_point_sources_two_streams():
+    """rt_point_sources is asynchronous on the caller's stream, whichever stream that is: calls that alternate between two
+    streams and between two source tables, with no host synchronisation in between, each give the result of their own
+    tables (the device copy of the tables is shared by all calls of a context: a call with the same tables on another
+    stream has to wait for the copy, a call with new tables for the kernels that still read the old ones)."""
+    import torch
+    import paper_1410_0763_b200 as rt
+    dims, nb = (96, 96, 96), 1
+    nx, ny, nz = dims
+    rng = np.random.default_rng(62)
+    kap = torch.from_numpy(rng.uniform(0.02, 0.6, (nb, nz, ny, nx)).astype(np.float32)).cuda()
+    tables = []
+    for t in range(2):
+        src = np.stack([rng.integers(0, nx * FIX + 1, 12), rng.integers(0, ny * FIX + 1, 12), rng.integers(0, nz * FIX + 1, 12)], axis=1).astype(np.int32)
+        tables.append((src, rng.uniform(0.5, 2.0, (12, nb))))
+    tr = rt.RayTracer(dims, nb, rt.healpix_dirs(1))
+    try:
+        tr.set_fields(kap, torch.zeros_like(kap))
+        ref = []
+        for src, lum in tables:                                  # one stream, synchronised: the reference
+            Q = torch.empty_like(kap)
+            rt.rt_point_sources(tr.h, src, lum, Q, tr.numel, nb)
+            torch.cuda.synchronize()
+            ref.append(Q.clone())
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        order = [(0, 0), (1, 0), (0, 1), (1, 1), (1, 0), (0, 0), (1, 1), (0, 1), (0, 0), (1, 1)]      # (stream, table)
+        outs = [torch.full_like(kap, -1.0) for _ in order]
+        torch.cuda.synchronize()
+        for (si, ti), Q in zip(order, outs):
+            rt.rt_point_sources(tr.h, tables[ti][0], tables[ti][1], Q, tr.numel, nb, stream=streams[si])
+        torch.cuda.synchronize()
+        for (si, ti), Q in zip(order, outs):
+            assert torch.equal(Q, ref[ti]), "call on stream %d with table %d" % (si, ti)
+    finally:
+        tr.close()
+
+
+@pytest.mark.gpu
 def test_point_sources_c3_sampled(orc):
     """128^3 (config C3's mesh and kappa), 4 sources: full oracle comparison (the oracle takes seconds)."""
     import torch
