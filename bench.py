@@ -159,8 +159,13 @@ def run_reference(args):
     cores = host_cores()
     if args.ref_dirs:
         nd = args.ref_dirs
-    else:                      # about 480 direction-sweeps in all, whole multiples of the core count, at most 96 per step
-        nd = min(96, max(cores, -(-(480 // max(1, args.steps)) // cores) * cores))
+    else:
+        # the same sample as the cpu_baseline leg of the GPU arm (--cpu-dirs, 96 directions: about 12 s per step at C4),
+        # whatever --steps is, so that the two legs quote one rate: with fewer directions per step each thread's
+        # start-up cost (its private accumulators are allocated and first touched per call) weighs more and the rate
+        # drops (round 2's driver record: 1.34e8 with 32 per step against 2.02e8 with 96).  Only a run of more than
+        # 24 steps is thinned, to stay within a few minutes.
+        nd = args.cpu_dirs if args.steps <= 24 else max(cores, (args.cpu_dirs * 24 // args.steps) // cores * cores)
     nd = max(1, min(spec.ndirs, nd))
     stride = max(1, spec.ndirs // nd)
     sub = dirs[::stride][:nd]
@@ -436,6 +441,9 @@ def roofline_of(r, name, run, peaks, default_tuning):
     peak, kind = (hbm_peak, hbm_kind) if bound == "hbm" else (peaks["l2_read"], "measured in this run (rt_probe_bandwidth, 48 MB read)")
     out = {"bound": bound, "achieved": run["achieved"], "peak": peak, "unit": "GB/s", "frac": run["achieved"] / peak,
            "traffic": None, "peak_kind": kind, "kernel": "k_sweep_tma",
+           # the 16-byte model is SURVEY.md 8(d)'s figure, not a bound on this schedule (see note): the fraction that is
+           # held against a ceiling is dram_frac_from_traffic (measured DRAM bytes over the HBM copy peak)
+           "frac_is_ceiling": False,
            "model": "16 B per cell-direction-bin (read kappa,S 8 B + accumulator read-modify-write 8 B) x cell-direction-bins per launch",
            "launches_per_step": run["n_sweep_launches"], "avg_launch_ms": run["avg_launch_ms"],
            "algorithmic_bytes_per_launch": run["bytes_per_launch"],
@@ -451,6 +459,12 @@ def roofline_of(r, name, run, peaks, default_tuning):
     floor_gbs = run["floor_bytes"] / (run["kernel_ms"] * 1e-3) / 1e9
     out["schedule_floor"] = {"what": "accumulator read-modify-write, 8 B per cell, bin and work entry", "entries": run["entries"],
                              "bytes_per_step": run["floor_bytes"], "gbs": floor_gbs, "frac_of_hbm_peak": floor_gbs / hbm_peak}
+    if bound == "l2" and r.working_set > r.l2_bytes:
+        # the packed fields stay in L2, the slot accumulators do not: a mixed bound, so the model against the L2 peak is
+        # an upper estimate of nothing; the two measured fractions below are what each level really carries
+        out["bound_detail"] = ("mixed: packed fields L2-resident, working set %.0f MB (fields + slot accumulators) streams through "
+                               "HBM (L2 %.0f MB); read dram_frac_from_traffic and l2_frac_from_traffic, not frac") % (
+                                   r.working_set / 1e6, r.l2_bytes / 1e6)
     table, state = traffic_table()
     out["traffic_table"] = state
     if default_tuning and name in table:
@@ -557,7 +571,7 @@ def main():
                 "workload": workload_name(sp), "ms_per_step": run["ms"] / run["steps"], "steps": run["steps"], "value": run["value"],
                 "unit": UNIT, "updates_per_step": upd, "gpu_launches_per_step": run["launches"],
                 "e2e": {k: run["e2e"][k] for k in ("value", "ms_per_step", "h2d_ms", "pack_ms", "sweep_ms", "d2h_ms")},
-                "bound": rf["bound"], "peak": rf["peak"], "model_frac": rf["frac"], "model_frac_of_hbm_peak": rf["frac_of_hbm_peak"],
+                "bound": rf["bound"], "bound_detail": rf.get("bound_detail"), "peak": rf["peak"], "model_frac": rf["frac"], "model_frac_of_hbm_peak": rf["frac_of_hbm_peak"],
                 "dram_frac_from_traffic": rf.get("dram_frac_from_traffic"), "l2_frac_from_traffic": rf.get("l2_frac_from_traffic"),
                 "schedule_floor_frac": rf["schedule_floor"]["frac_of_hbm_peak"],
                 "kernel_share_of_step": rf["kernel_share_of_step"],

@@ -5,13 +5,17 @@ on the box's host cores (full C3 sweep ~ 30 s on 16 threads; sampled cells of C4
   C3 (128^3 x 3072):  EVERY cell: J_in and J within tolerance, direction-summed counts identical, per-direction
                       count arrays for 16 sampled directions, total segments == oracle == tests/golden, sum ds of
                       all 3072 directions vs the oracle and vs N_m L; two further seeds of the recipe (J only).
-  C4, C5:             >= 4096 sampled cells through orc_sweep_cells (random + three full axis lines through the
-                      most opaque cell + the eight corners), counts at those cells, total segments == the oracle's
-                      exact totals in tests/golden/segment_totals.txt, sum ds of a 128-direction subset vs oracle.
+  C4 (256^3 x 3072):  EVERY cell once: J_in against the whole oracle sweep (4-8 min of host time on 16 threads).
+  C4, C5:             >= 4096 (C5: >= 16384) sampled cells through orc_sweep_cells (random + three full axis lines
+                      through the most opaque cell + the eight corners), counts at those cells, total segments == the
+                      oracle's exact totals in tests/golden/segment_totals.txt, SHA-256 of the per-cell counts summed
+                      over the directions == the oracle's (same file: every cell, bit-exact), sum ds of a 128-direction
+                      subset vs oracle.
   128^3 x 12288:      N_side = 32 on the C3 mesh, 1024 sampled cells (four times the directions in the fp32 sums).
 
 Every test appends its maxima to gpurun_out/parity_report.txt (scratch) so that a run leaves the numbers behind.
 """
+import hashlib
 import json
 import os
 import time
@@ -35,6 +39,22 @@ def golden_totals():
             k, v = line.split()[:2]
             out[k] = int(v)
     return out
+
+
+def golden_count_hashes():
+    """SHA-256 of the oracle's per-cell segment counts summed over the directions (uint32 little-endian, [nz][ny][nx]),
+    written by tests/golden/make_segment_totals.py from oracle/ alone."""
+    out = {}
+    for line in open(os.path.join(ROOT, "tests", "golden", "segment_totals.txt")):
+        w = line.split()
+        if w and not line.startswith("#"):
+            assert len(w) >= 5 and len(w[4]) == 64, "segment_totals.txt has no count hash for %s" % w[0]
+            out[w[0]] = w[4]
+    return out
+
+
+def count_hash(cnt):
+    return hashlib.sha256(np.ascontiguousarray(cnt, dtype="<u4").tobytes()).hexdigest()
 
 
 def report(**kw):
@@ -96,6 +116,7 @@ def test_c3_every_cell(orc):
     assert np.array_equal(cnt, ref["cnt_sum"])
     assert np.array_equal(cnt_d, ref["cnt_dirs"])
     assert seg_total == ref["seg_total"] == golden_totals()["C3"]
+    assert count_hash(cnt) == count_hash(ref["cnt_sum"]) == golden_count_hashes()["C3"]
     # sum ds of every direction: vs the oracle and vs the closed form N_m L (pin P3)
     assert np.abs(sum_ds / ref["sum_ds"] - 1).max() <= DS_TOL
     assert np.abs(sum_ds / (spec.ncell * L) - 1).max() <= DS_TOL
@@ -130,6 +151,34 @@ def test_c3_further_seeds_every_cell(orc, seed):
     assert m[0] <= J_MARGIN, "C3 seed %d J_in max rel err %.3e (p99.9 %.3e, median %.3e)" % ((seed,) + m)
 
 
+def test_c4_every_cell(orc):
+    """Config 4 (the benchmark's headline workload) in full, once: J_in of the whole GPU sweep against the whole oracle
+    sweep, every one of the 16.8 M cells (the sampled gate below cannot see an error in a cell it did not draw)."""
+    from rt_inputs import make_fields, CONFIGS
+    import paper_1410_0763_b200 as rt
+    torch = _torch()
+    spec = CONFIGS["C4"]
+    kap, S = make_fields("C4")
+    dirs = orc.healpix_dirs(spec.nside)
+    tr = rt.RayTracer(spec.dims, 1, dirs)
+    try:
+        tr.set_fields(torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda())
+        Jin = tr.sweep(what=rt.RT_J_IN).cpu().numpy()
+        rec, _ = tr.direction_records()
+    finally:
+        tr.close()
+    assert np.all(rec[:, 4] == 0)
+    t0 = time.time()
+    ref = orc.sweep(kap, S, dirs, want_counts=False)
+    dt = time.time() - t0
+    assert ref["seg_total"] == golden_totals()["C4"]
+    e = rel_err(Jin, ref["Jin"])
+    m = stats(e)
+    report(test="c4_every_cell", cells=int(e.size), J_in_max=m[0], J_in_p999=m[1], J_in_median=m[2], oracle_s=dt,
+           oracle_threads=orc.num_threads(), oracle_updates_per_s=ref["seg_total"] / dt)
+    assert m[0] <= J_MARGIN, "C4 J_in max rel err %.3e (p99.9 %.3e, median %.3e) over %d cells" % (m + (e.size,))
+
+
 @pytest.mark.parametrize("name", ["C4", "C5"])
 def test_full_size_4096_cells(orc, name):
     """Configs 4 and 5 at full size: >= 4096 sampled cells computed by the oracle ray by ray, exact totals, sum ds."""
@@ -140,8 +189,9 @@ def test_full_size_4096_cells(orc, name):
     kap, S = make_fields(name)
     nb = kap.shape[0]
     dirs = orc.healpix_dirs(spec.nside)
-    cells = sample_cells(spec.dims, 4096, 7, kap)
-    assert len(cells) >= 4096
+    nsample = 4096 if name == "C4" else 16384          # C4 is also compared on every cell (test_c4_every_cell)
+    cells = sample_cells(spec.dims, nsample, 7, kap)
+    assert len(cells) >= nsample
     sub = np.arange(0, spec.ndirs, 24)                 # 128 of the 3072 directions for the sum-of-ds gate
     tr = rt.RayTracer(spec.dims, nb, dirs)
     try:
@@ -158,8 +208,20 @@ def test_full_size_4096_cells(orc, name):
         got_cnt = cnt[ix[:, 2], ix[:, 1], ix[:, 0]].cpu().numpy().astype(np.uint32)
         assert bool(torch.isfinite(Jin).all()) and float(Jin.min()) >= 0.0
         cnt_total = int(cnt.to(torch.int64).sum().item())
+        cnt_sha = count_hash(cnt.cpu().numpy())
     finally:
         tr.close()
+    got_packed = None
+    if nb % 3 == 0:                                    # C5: the multi-bin packed kernel (three bins per row) at full size
+        tr = rt.RayTracer(spec.dims, nb, dirs, tune={"binpack": 1})
+        try:
+            tr.set_fields(torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda())
+            Jp = tr.sweep(what=rt.RT_J_IN)
+            got_packed = Jp[:, ix[:, 2], ix[:, 1], ix[:, 0]].cpu().numpy()
+            assert bool(torch.isfinite(Jp).all()) and float(Jp.min()) >= 0.0
+            del Jp
+        finally:
+            tr.close()
     tr = rt.RayTracer(spec.dims, 1, dirs[sub])
     try:
         sum_ds, mn, mx = tr.sum_ds()
@@ -168,6 +230,8 @@ def test_full_size_4096_cells(orc, name):
         tr.close()
     # integer data: the oracle's exact totals (tests/golden/segment_totals.txt, written from oracle/ alone)
     assert seg_total == cnt_total == golden_totals()[name]
+    # ... and on every cell: the hash of the whole direction-summed count array is the oracle's
+    assert cnt_sha == golden_count_hashes()[name], "%s: per-cell segment counts differ from the oracle's somewhere in the mesh" % name
     t0 = time.time()
     ref = orc.sweep_cells(kap, S, dirs, cells)
     dt = time.time() - t0
@@ -184,6 +248,10 @@ def test_full_size_4096_cells(orc, name):
            J_in_median=m_in[2], J_max=m_J[0], seg_total=seg_total, oracle_cells_s=dt)
     assert m_in[0] <= J_MARGIN, "%s J_in max rel err %.3e (p99.9 %.3e, median %.3e)" % ((name,) + m_in)
     assert m_J[0] <= J_MARGIN, "%s J max rel err %.3e (p99.9 %.3e, median %.3e)" % ((name,) + m_J)
+    if got_packed is not None:
+        m_p = stats(rel_err(got_packed, ref["Jin"]))
+        report(test="full_size_packed_bins", config=name, cells=int(len(cells)), J_in_max=m_p[0], J_in_p999=m_p[1], J_in_median=m_p[2])
+        assert m_p[0] <= J_MARGIN, "%s binpack J_in max rel err %.3e (p99.9 %.3e, median %.3e)" % ((name,) + m_p)
 
 
 def test_c3_mesh_nside32_sampled(orc):

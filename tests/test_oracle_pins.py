@@ -513,3 +513,22 @@ def test_p13_per_face_inflow_bruteforce_and_vacuum(orc):
     a = orc.sweep(kap, S, dirs, Ibc=[0.6])["Jin"]
     b = orc.sweep(kap, S, dirs, Ibc_faces=[[0.6] * 6])["Jin"]
     assert np.allclose(a, b, rtol=1e-14, atol=0)            # (thread reduction order differs between runs)
+
+
+def test_golden_count_hashes_are_the_oracles(orc):
+    """tests/golden/segment_totals.txt (totals + SHA-256 of the direction-summed per-cell counts, the every-cell integer
+    gate of the full-size GPU tests) is what oracle/ computes: re-derived here for the two configs that take seconds."""
+    import hashlib
+    from rt_inputs import CONFIGS
+    rows = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "segment_totals.txt")):
+        w = line.split()
+        if w and not line.startswith("#"):
+            rows[w[0]] = (int(w[1]), w[4])
+    assert sorted(rows) == ["C1", "C2", "C3", "C4", "C5"] and all(len(v[1]) == 64 for v in rows.values())
+    for name in ("C1", "C2"):
+        spec = CONFIGS[name]
+        nx, ny, nz = spec.dims
+        r = orc.sweep(np.ones((1, nz, ny, nx), np.float32), np.zeros((1, nz, ny, nx), np.float32), orc.healpix_dirs(spec.nside))
+        sha = hashlib.sha256(np.ascontiguousarray(r["cnt_sum"], dtype="<u4").tobytes()).hexdigest()
+        assert (r["seg_total"], sha) == rows[name]
