@@ -190,8 +190,14 @@ def run_reference(args):
 
 
 def run_point(args):
-    """--workload point: rt_point_sources on the config's mesh and kappa with seeded sources (one at a box corner,
-    one at the centre, the rest uniform in the box, positions in 1/256 cell).  One JSON line of its own."""
+    """--workload point: one JSON line of its own."""
+    print(json.dumps(point_line(args, cpu=not args.no_cpu_baseline)))
+
+
+def point_line(args, cpu=True):
+    """rt_point_sources on the config's mesh and kappa with seeded sources (one at a box corner, one at the centre,
+    the rest uniform in the box, positions in 1/256 cell): the record --workload point prints, also carried by the
+    default line under "point" so that the driver's record holds the paper's second workload."""
     import torch
     import paper_1410_0763_b200 as rt
     from rt_inputs import make_fields, CONFIGS
@@ -223,8 +229,8 @@ def run_point(args):
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1) / args.steps
     tr.close()
-    cpu = None
-    if not args.no_cpu_baseline:
+    want_cpu, cpu = cpu, None
+    if want_cpu:
         from oracle import oracle
         ns = min(args.sources, 2)
         t0 = time.perf_counter()
@@ -250,7 +256,7 @@ def run_point(args):
             note = "stale: %s changed since the ncu capture" % t["kernel_source"]
     except Exception:
         pass
-    print(json.dumps({
+    return {
         "metric": "point_source_ray_steps_per_sec", "value": steps * spec.nbins / (ms * 1e-3), "unit": "ray steps/s",
         "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64 path sums over f32 kappa", "data": "synthetic",
@@ -258,7 +264,7 @@ def run_point(args):
                    "ray_steps_per_step": steps * spec.nbins, "rays_per_step": args.sources * spec.ncell * spec.nbins},
         "clocks": clocks, "gpu_launches": args.steps,
         "roofline": roof, "note": note,
-        "cpu_baseline": cpu}))
+        "cpu_baseline": cpu}
 
 
 def run_probe(args):
@@ -619,6 +625,10 @@ def main():
     }
     if configs:
         line["configs"] = configs
+        # the paper's second workload (RT from point sources) on the same mesh, outside the timed region
+        # of the headline: its own metric, time and issue-slot roofline (bench.py --workload point prints the same record)
+        p = point_line(args, cpu=False)
+        line["point"] = {k: p[k] for k in ("metric", "value", "unit", "ms_per_step", "config", "roofline", "note")}
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -76,6 +76,10 @@ def test_default_line_carries_all_five_configs():
         assert c["value"] > 0 and c["ms_per_step"] > 0 and c["e2e"]["value"] > 0 and c["model_frac"] > 0
         assert c["bound"] == ("hbm" if name in ("C4", "C5") else "l2")
     assert d["configs"]["C4"]["ms_per_step"] == d["ms_per_step"]
+    assert d["roofline"]["frac_is_ceiling"] is False and d["configs"]["C1"]["graph_replay"] is True
+    assert d["configs"]["C3"]["bound_detail"].startswith("mixed") and d["configs"]["C4"]["bound_detail"] is None
+    p = d["point"]                                                     # the second workload rides on the default line
+    assert p["metric"] == "point_source_ray_steps_per_sec" and p["value"] > 0 and p["ms_per_step"] > 0 and p["config"]["sources"] == 8
     t = d["roofline"]
     assert t["traffic_table"] == "ok" or t["traffic"] is None        # never a stale ncu figure
 
