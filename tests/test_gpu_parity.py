@@ -549,6 +549,38 @@ def test_schedules_agree(orc, tune):
     assert rel_err(again, ref2["Jin"]).max() <= J_TOL
 
 
+@pytest.mark.parametrize("tune", [{"overlap": 0}, {"overlap": 1}])
+def test_sweep_inside_a_callers_stream_capture(tune):
+    """A caller may capture rt_sweep into a CUDA graph of its own.  The library then records no timing events into that
+    graph (rt_last_sweep_kernel_ms says "unavailable" instead of failing on events that were never executed) and does not
+    start a graph of its own inside the capture; replays of the caller's graph give the bits of a plain sweep."""
+    import paper_1410_0763_b200 as rt
+    torch = _torch()
+    dims = (64, 32, 16)
+    kap, S = _rand(dims, 43)
+    tr = rt.RayTracer(dims, 1, rt.healpix_dirs(2), tune=tune)
+    try:
+        tr.set_fields(torch.from_numpy(kap).cuda(), torch.from_numpy(S).cuda())
+        plain = tr.sweep().clone()                       # also the first launch of every kernel, outside any capture
+        assert tr.last_sweep_kernel_ms() > 0.0
+        out = torch.zeros_like(plain)
+        st = torch.cuda.Stream()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st, capture_error_mode="thread_local"):
+            tr.sweep(out=out, stream=torch.cuda.current_stream())
+        assert tr.last_sweep_kernel_ms() < 0.0 and not tr.last_sweep_was_graph()
+        for _ in range(2):
+            out.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            assert torch.equal(out, plain)
+        again = tr.sweep()                               # and the context still sweeps, and times, outside the capture
+        assert torch.equal(again, plain) and tr.last_sweep_kernel_ms() > 0.0
+    finally:
+        tr.close()
+
+
 @pytest.mark.parametrize("tune", [{"overlap": 1, "graph": 1}, {"overlap": 0, "graph": 0}])
 def test_async_inflow_between_sweeps_on_a_side_stream(orc, tune):
     """rt_set_inflow_faces_async / rt_set_inflow_async are ordered by the stream they are enqueued on, with no device
